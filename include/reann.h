@@ -1,0 +1,126 @@
+/*
+ * reann.h -- C ABI of libreann_b200.so: the REANN energy + force (+ virial) hot path on one B200.
+ *
+ * The model is the recursively embedded atom neural network of arXiv 2505.06711
+ * (Eqs. 1-2; forces by the chain rule of PAPER.md:59-80, Eqs. 3-5), with the
+ * readings of SURVEY.md section 8(c) / DESIGN.md where the paper is silent. Everything behind
+ * these calls runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *  - Units: Angstrom, eV, eV/Angstrom.
+ *  - `pos`, `E`, `F`, `virial`, `species`, `weights` may each be HOST or DEVICE pointers
+ *    (detected with cudaPointerGetAttributes). `box` is always a HOST pointer to 9 doubles:
+ *    row-major lattice vectors; only orthorhombic boxes (off-diagonals exactly 0) are
+ *    supported and every box length must be >= rc + skin (so only images -1,0,+1 occur).
+ *    Positions need not be wrapped into the box.
+ *  - Ownership: the caller owns every array it passes; the library copies what it keeps
+ *    (weights, species) and never retains caller pointers past the call.
+ *  - With device pointers the work is enqueued on the handle's stream; the call synchronises
+ *    the stream once (to read the skin-check flag) and returns with the output kernels
+ *    enqueued, not necessarily finished. With host pointers the call returns after the
+ *    results are copied back.
+ *  - Every function returns a REANN_* code, never throws or aborts; reann_last_error() gives
+ *    text for the last failure on that handle.
+ *  - Determinism: same inputs give bitwise-identical outputs (no floating-point atomics;
+ *    fixed reduction order).
+ */
+#ifndef REANN_H
+#define REANN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct reann reann_t; /* opaque; owns all device memory */
+
+enum {
+    REANN_OK = 0,
+    REANN_ERR_ARG = 1,          /* NULL / out-of-range argument                         */
+    REANN_ERR_WEIGHTS = 2,      /* bad blob, or blob header disagrees with arguments    */
+    REANN_ERR_BOX = 3,          /* box length < rc + skin, or non-positive              */
+    REANN_ERR_NO_NEIGHBORS = 4, /* reann_energy_forces before any reann_build_neighbors */
+    REANN_ERR_CUDA = 5,         /* a CUDA runtime call failed (text in last_error)      */
+    REANN_ERR_OOM = 6,          /* device allocation failed                             */
+    REANN_ERR_UNSUPPORTED = 7   /* triclinic box, n_gauss > 16, L > 3, row too long ... */
+};
+
+/*
+ * reann_create -- build a model instance for a fixed set of atoms (per-element
+ * orbital coefficients, per-element atomic NNs, T message-passing layers).
+ *   weights, weights_bytes : the blob described in gen/weights.py (header + float64 arrays:
+ *                            r_center, alpha [T][S][n_gauss]; c0 [S][n_gauss];
+ *                            Wc [T][L+1][n_gauss][n_orb]; per (t, s) W1,b1,W2,b2,W3,b3).
+ *                            Copied; folded/converted to FP32 device copies.
+ *   species[n_atoms]       : 0..S-1 in caller order; copied.
+ *   rc, skin               : cutoff of Eq. 1 and the neighbour-list skin.
+ *   T, L, n_gauss          : must equal the blob header (else REANN_ERR_WEIGHTS);
+ *                            T >= 1, 0 <= L <= 3, 1 <= n_gauss <= 16 in this version.
+ */
+int reann_create(reann_t **out, const void *weights, size_t weights_bytes, const int32_t *species,
+                 int64_t n_atoms, double rc, double skin, int T, int L, int n_gauss);
+
+/*
+ * reann_build_neighbors -- force a rebuild of the skin neighbour list (one list
+ * with cutoff rc(+skin), reused by every layer; local atoms, ghost atoms).
+ * Sorts atoms by cell (Morton order), generates the periodic-image ("ghost") map, and emits
+ * CSR rows of all (i, j_image) with |r_j + S o box - r_i|^2 < (rc+skin)^2, strict, FP64,
+ * plus the index of every reverse edge.   pos: [n_atoms][3] doubles.
+ */
+int reann_build_neighbors(reann_t *h, const double *pos, const double *box9);
+
+/*
+ * reann_energy_forces -- one evaluation of E = sum_i E_i, F_k = -dE/dr_k
+ * (Eq. 3) and optionally the virial  -sum_e r_e (x) dE/dr_e  (3x3 row-major, eV; = -dE/d(strain)).
+ * Runs the skin check itself (rebuild when any atom moved > skin/2 since the last build, or
+ * the box changed), then T forward layers (Eq. 1, Eq. 2) and the analytic reverse pass
+ * (Eqs. 3-5).   E: 1 double; F: [n_atoms][3] doubles, caller order; virial: 9 doubles or NULL.
+ */
+int reann_energy_forces(reann_t *h, const double *pos, const double *box9, double *E, double *F,
+                        double *virial);
+
+void reann_destroy(reann_t *h);
+const char *reann_last_error(const reann_t *h); /* h may be NULL: error of the last failed create */
+
+/* ---- introspection for the parity tests and bench.py (not needed by an MD code) ---- */
+
+typedef struct {
+    int64_t n_atoms, n_ext;          /* local atoms, local + image ("ghost") atoms            */
+    int64_t n_edges_list, n_edges_rc;/* list entries (r < rc+skin); entries with r < rc now   */
+    int64_t n_rebuilds, n_calls;     /* builds so far; reann_energy_forces calls so far       */
+    int64_t n_launches;              /* kernels launched by this handle so far                */
+    double ms_build;                 /* accumulated, only while profiling is on (ms):         */
+    double ms_prep, ms_edge_fwd, ms_dense_fwd, ms_gather, ms_dense_bwd, ms_edge_bwd,
+           ms_rev_gather, ms_output;
+    int64_t n_profiled_calls;        /* calls the ms_* fields (except ms_build) accumulate    */
+    size_t bytes_device;             /* device memory currently held by the handle            */
+} reann_stats_t;
+
+/* Neighbour list in the CALLER's order and frame (for exact pair-set parity):
+ *   call with row_ptr = j = shift = NULL to get *n_edges; then with arrays of sizes
+ *   row_ptr[n_atoms+1], j[n_edges] (caller index of the neighbour), shift[n_edges][3] such
+ *   that the edge vector is pos[j] + shift o box - pos[i] for the positions given at build.
+ *   All three are HOST pointers. */
+int reann_get_neighbors(reann_t *h, int64_t *n_edges, int64_t *row_ptr, int32_t *j, int8_t *shift);
+
+int reann_get_stats(reann_t *h, reann_stats_t *out);
+int reann_set_profiling(reann_t *h, int on);            /* CUDA-event timing of kernel groups  */
+int reann_set_stream(reann_t *h, void *cuda_stream);    /* e.g. torch.cuda.current_stream().cuda_stream */
+
+/* Per-atom energies E_i of the last evaluation, caller order (host or device pointer). */
+int reann_get_atomic_energies(reann_t *h, double *Ei);
+
+/*
+ * Harness support, outside the energy/force path: one velocity-Verlet step on device arrays
+ * (all DEVICE pointers, caller order): v += dt/2 * F * acc_unit / m ; x += dt * v  (kick_drift),
+ * or only the half kick. inv_mass[n_atoms] in 1/amu, acc_unit converts eV/(A amu) to A/fs^2.
+ */
+int reann_verlet(reann_t *h, double *pos, double *vel, const double *F, const double *inv_mass,
+                 double dt, double acc_unit, int drift);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* REANN_H */

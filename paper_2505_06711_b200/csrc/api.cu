@@ -1,0 +1,568 @@
+// api.cu -- the C ABI of include/reann.h: handle, weights folding/upload, the evaluation schedule.
+// Host logic only; every arithmetic step of the path runs in the kernels of neighbor.cu, edge.cu,
+// dense.cu, scan.cu. There is deliberately no CPU fallback: without a CUDA device every call fails.
+#include <math.h>
+#include <stdarg.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "handle.cuh"
+
+static thread_local std::string g_create_error;
+
+int set_err(reann *h, int code, const char *fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    if (h) h->err = buf; else g_create_error = buf;
+    return code;
+}
+
+int dev_ensure(reann *h, DevBuf &b, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    if (b.bytes >= bytes) return REANN_OK;
+    if (b.p) { cudaFree(b.p); h->bytes_device -= b.bytes; b.p = nullptr; b.bytes = 0; }
+    const size_t want = (bytes + 255) & ~(size_t)255;
+    cudaError_t e = cudaMalloc(&b.p, want);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        b.p = nullptr;
+        return set_err(h, REANN_ERR_OOM, "cudaMalloc(%zu bytes) failed: %s", want, cudaGetErrorString(e));
+    }
+    b.bytes = want;
+    h->bytes_device += want;
+    return REANN_OK;
+}
+
+static void dev_free(reann *h, DevBuf &b) {
+    if (b.p) { cudaFree(b.p); h->bytes_device -= b.bytes; }
+    b.p = nullptr; b.bytes = 0;
+}
+
+static bool is_device_ptr(const void *p) {
+    if (!p) return false;
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static int pad_pow2_16(int H) { int p = 16; while (p < H) p <<= 1; return p; }
+
+// ---------------------------------------------------------------------------------------------
+// Blob parsing (layout: gen/weights.py) -- this side's own parser.
+struct BlobView {
+    int S, T, L, nphi, norb, H1c, H2c, H1e, H2e;
+    double rc;
+    const double *rcen, *alpha, *c0, *Wc;
+    std::vector<const double *> W1, b1, W2, b2, W3, b3;
+};
+
+static int parse_blob(const unsigned char *p, size_t nbytes, BlobView &v, std::string &why) {
+    if (nbytes < 64 || memcmp(p, "REANNB2\0", 8) != 0) { why = "bad magic or truncated header"; return REANN_ERR_WEIGHTS; }
+    uint32_t hd[12];
+    memcpy(hd, p + 8, sizeof(hd));
+    if (hd[0] != 1 || hd[10] != 0) { why = "unsupported version or activation"; return REANN_ERR_WEIGHTS; }
+    v.S = hd[1]; v.T = hd[2]; v.L = hd[3]; v.nphi = hd[4]; v.norb = hd[5];
+    v.H1c = hd[6]; v.H2c = hd[7]; v.H1e = hd[8]; v.H2e = hd[9];
+    memcpy(&v.rc, p + 56, 8);
+    if (v.S < 1 || v.T < 1 || v.nphi < 1 || v.norb < 1 || v.L < 0 || !(v.rc > 0) || v.H1c < 1 || v.H2c < 1 || v.H1e < 1 ||
+        v.H2e < 1 || v.S > 1024 || v.T > 1024 || v.nphi > 4096 || v.L > 64) {
+        why = "header fields out of range"; return REANN_ERR_WEIGHTS;
+    }
+    size_t need = (size_t)2 * v.T * v.S * v.nphi + (size_t)v.S * v.nphi + (size_t)v.T * (v.L + 1) * v.nphi * v.norb;
+    for (int t = 0; t < v.T; ++t) {
+        const bool last = t == v.T - 1;
+        const size_t H1 = last ? v.H1e : v.H1c, H2 = last ? v.H2e : v.H2c, out = last ? 1 : v.nphi;
+        need += (size_t)v.S * ((size_t)v.norb * H1 + H1 + H1 * H2 + H2 + H2 * out + out);
+    }
+    if (nbytes != 64 + 8 * need) { why = "blob size does not match its header"; return REANN_ERR_WEIGHTS; }
+    const double *q = reinterpret_cast<const double *>(p + 64);
+    v.rcen = q; q += (size_t)v.T * v.S * v.nphi;
+    v.alpha = q; q += (size_t)v.T * v.S * v.nphi;
+    v.c0 = q; q += (size_t)v.S * v.nphi;
+    v.Wc = q; q += (size_t)v.T * (v.L + 1) * v.nphi * v.norb;
+    for (int t = 0; t < v.T; ++t) {
+        const bool last = t == v.T - 1;
+        const size_t H1 = last ? v.H1e : v.H1c, H2 = last ? v.H2e : v.H2c, out = last ? 1 : v.nphi;
+        for (int s = 0; s < v.S; ++s) {
+            v.W1.push_back(q); q += (size_t)v.norb * H1;
+            v.b1.push_back(q); q += H1;
+            v.W2.push_back(q); q += H1 * H2;
+            v.b2.push_back(q); q += H2;
+            v.W3.push_back(q); q += H2 * out;
+            v.b3.push_back(q); q += out;
+        }
+    }
+    return REANN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_bytes, const int32_t *species,
+                            int64_t n_atoms, double rc, double skin, int T, int L, int n_gauss) {
+    if (!out) return set_err(nullptr, REANN_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    if (!weights || !species || n_atoms < 0 || !(rc > 0) || !(skin >= 0) || T < 1)
+        return set_err(nullptr, REANN_ERR_ARG, "bad argument (NULL pointer, n_atoms < 0, rc <= 0, skin < 0 or T < 1)");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return set_err(nullptr, REANN_ERR_CUDA, "no CUDA device: this library has no CPU path");
+    }
+    if (n_atoms >= ((int64_t)1 << 28)) return set_err(nullptr, REANN_ERR_UNSUPPORTED, "n_atoms >= 2^28");
+    // bring blob and species to the host
+    std::vector<unsigned char> blob(weights_bytes);
+    if (is_device_ptr(weights)) {
+        if (cudaMemcpy(blob.data(), weights, weights_bytes, cudaMemcpyDeviceToHost) != cudaSuccess)
+            return set_err(nullptr, REANN_ERR_CUDA, "copy of weights failed");
+    } else memcpy(blob.data(), weights, weights_bytes);
+    std::vector<int32_t> sp((size_t)n_atoms);
+    if (n_atoms > 0) {
+        if (is_device_ptr(species)) {
+            if (cudaMemcpy(sp.data(), species, sizeof(int32_t) * (size_t)n_atoms, cudaMemcpyDeviceToHost) != cudaSuccess)
+                return set_err(nullptr, REANN_ERR_CUDA, "copy of species failed");
+        } else memcpy(sp.data(), species, sizeof(int32_t) * (size_t)n_atoms);
+    }
+    BlobView v;
+    std::string why;
+    int rcode = parse_blob(blob.data(), weights_bytes, v, why);
+    if (rcode) return set_err(nullptr, rcode, "weights blob: %s", why.c_str());
+    if (v.T != T || v.L != L || v.nphi != n_gauss || fabs(v.rc - rc) > 1e-12 * rc)
+        return set_err(nullptr, REANN_ERR_WEIGHTS, "blob header (T=%d L=%d n_gauss=%d rc=%g) disagrees with arguments (T=%d L=%d n_gauss=%d rc=%g)",
+                       v.T, v.L, v.nphi, v.rc, T, L, n_gauss, rc);
+    if (L > 3 || n_gauss > REANN_MAX_NPHI || T > REANN_MAX_T || v.S > REANN_MAX_S)
+        return set_err(nullptr, REANN_ERR_UNSUPPORTED, "this version supports L <= 3, n_gauss <= %d, T <= %d, S <= %d",
+                       REANN_MAX_NPHI, REANN_MAX_T, REANN_MAX_S);
+    if (std::max(std::max(v.H1c, v.H2c), std::max(v.H1e, v.H2e)) > 128)
+        return set_err(nullptr, REANN_ERR_UNSUPPORTED, "MLP hidden width > 128 not supported in this version");
+    for (int64_t i = 0; i < n_atoms; ++i)
+        if (sp[(size_t)i] < 0 || sp[(size_t)i] >= v.S) return set_err(nullptr, REANN_ERR_ARG, "species[%lld] = %d out of range", (long long)i, sp[(size_t)i]);
+
+    reann *h = new reann();
+    h->N = n_atoms;
+    ModelDims &md = h->md;
+    md.S = v.S; md.T = T; md.L = L; md.nphi = n_gauss; md.nphip = (n_gauss + 3) & ~3;
+    md.Na = (L + 1) * (L + 2) * (L + 3) / 6; md.NB = md.nphip * md.Na; md.norb = v.norb;
+    md.npairs = n_gauss * (n_gauss + 1) / 2; md.NPp = (md.npairs + 15) & ~15; md.nqp = (L + 1) * md.NPp;
+    md.rc = rc; md.skin = skin;
+    h->zs = 0;
+    for (int t = 0; t < T; ++t) {
+        const bool last = t == T - 1;
+        h->ld[t].H1p = pad_pow2_16(last ? v.H1e : v.H1c);
+        h->ld[t].H2p = pad_pow2_16(last ? v.H2e : v.H2c);
+        h->ld[t].nout = last ? 1 : n_gauss;
+        h->ld[t].noutp = h->ld[t].nout;
+        h->zs = std::max(h->zs, h->ld[t].H1p + h->ld[t].H2p);
+    }
+#define CREATE_FAIL(code, ...) do { int c_ = set_err(nullptr, code, __VA_ARGS__); reann_destroy(h); return c_; } while (0)
+#define CCU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) CREATE_FAIL(REANN_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); } while (0)
+#define CRC(call) do { int r_ = (call); if (r_ != REANN_OK) { g_create_error = h->err; reann_destroy(h); return r_; } } while (0)
+
+    // ---- radial tables and c0 (FP32, padded to nphip) ----
+    const double LOG2E = 1.4426950408889634;
+    {
+        const size_t n = (size_t)T * md.S * md.nphip;
+        std::vector<float> rcen(n, 0.f), al(n, 0.f), c0((size_t)md.S * md.nphip, 0.f);
+        for (int t = 0; t < T; ++t)
+            for (int s = 0; s < md.S; ++s)
+                for (int k = 0; k < md.nphi; ++k) {
+                    rcen[((size_t)t * md.S + s) * md.nphip + k] = (float)v.rcen[((size_t)t * md.S + s) * md.nphi + k];
+                    al[((size_t)t * md.S + s) * md.nphip + k] = (float)(v.alpha[((size_t)t * md.S + s) * md.nphi + k] * LOG2E);
+                }
+        for (int s = 0; s < md.S; ++s)
+            for (int k = 0; k < md.nphi; ++k) c0[(size_t)s * md.nphip + k] = (float)v.c0[(size_t)s * md.nphi + k];
+        CRC(dev_ensure(h, h->rcen, n * 4)); CRC(dev_ensure(h, h->alpha, n * 4)); CRC(dev_ensure(h, h->c0, c0.size() * 4));
+        CCU(cudaMemcpy(h->rcen.p, rcen.data(), n * 4, cudaMemcpyHostToDevice));
+        CCU(cudaMemcpy(h->alpha.p, al.data(), n * 4, cudaMemcpyHostToDevice));
+        CCU(cudaMemcpy(h->c0.p, c0.data(), c0.size() * 4, cudaMemcpyHostToDevice));
+    }
+    // ---- fold the contraction into the first MLP layer (FP64), pad, transpose (see dense.cu) ----
+    {
+        std::vector<float> all;
+        auto reserve = [&](size_t n) { size_t o = all.size(); all.resize(o + ((n + 3) & ~(size_t)3), 0.f); return o; };
+        struct Off { size_t U, UT, b1, W2, W2T, b2, W3, W3T, b3; };
+        std::vector<Off> offs((size_t)T * md.S);
+        std::vector<double> Vq((size_t)v.norb);
+        for (int t = 0; t < T; ++t) {
+            const bool last = t == T - 1;
+            const int H1 = last ? v.H1e : v.H1c, H2 = last ? v.H2e : v.H2c, nout = h->ld[t].nout;
+            const int H1p = h->ld[t].H1p, H2p = h->ld[t].H2p;
+            for (int s = 0; s < md.S; ++s) {
+                const int k = t * md.S + s;
+                Off o;
+                o.U = reserve((size_t)md.nqp * H1p); o.UT = reserve((size_t)(L + 1) * H1p * md.NPp);
+                o.b1 = reserve(H1p); o.W2 = reserve((size_t)H1p * H2p); o.W2T = reserve((size_t)H2p * H1p);
+                o.b2 = reserve(H2p); o.W3 = reserve((size_t)H2p * nout); o.W3T = reserve((size_t)nout * H2p);
+                o.b3 = reserve(nout);
+                offs[(size_t)k] = o;
+                const double *W1 = v.W1[(size_t)k];
+                for (int l = 0; l <= L; ++l) {
+                    const double *Wl = v.Wc + ((size_t)t * (L + 1) + l) * md.nphi * v.norb;
+                    int pp = 0;
+                    for (int n = 0; n < md.nphi; ++n)
+                        for (int n2 = n; n2 < md.nphi; ++n2, ++pp) {
+                            const double fac = (n == n2) ? 1.0 : 2.0;
+                            for (int m = 0; m < v.norb; ++m) Vq[(size_t)m] = fac * Wl[(size_t)n * v.norb + m] * Wl[(size_t)n2 * v.norb + m];
+                            const size_t q = (size_t)l * md.NPp + pp;
+                            for (int hh = 0; hh < H1; ++hh) {
+                                double acc = 0.0;
+                                for (int m = 0; m < v.norb; ++m) acc += Vq[(size_t)m] * W1[(size_t)m * H1 + hh];
+                                all[o.U + q * H1p + hh] = (float)acc;
+                                all[o.UT + ((size_t)l * H1p + hh) * md.NPp + pp] = (float)acc;
+                            }
+                        }
+                }
+                for (int a = 0; a < H1; ++a) all[o.b1 + a] = (float)v.b1[(size_t)k][a];
+                for (int a = 0; a < H1; ++a)
+                    for (int b = 0; b < H2; ++b) {
+                        const float w = (float)v.W2[(size_t)k][(size_t)a * H2 + b];
+                        all[o.W2 + (size_t)a * H2p + b] = w;
+                        all[o.W2T + (size_t)b * H1p + a] = w;
+                    }
+                for (int b = 0; b < H2; ++b) all[o.b2 + b] = (float)v.b2[(size_t)k][b];
+                for (int b = 0; b < H2; ++b)
+                    for (int c = 0; c < nout; ++c) {
+                        const float w = (float)v.W3[(size_t)k][(size_t)b * nout + c];
+                        all[o.W3 + (size_t)b * nout + c] = w;
+                        all[o.W3T + (size_t)c * H2p + b] = w;
+                    }
+                for (int c = 0; c < nout; ++c) all[o.b3 + c] = (float)v.b3[(size_t)k][c];
+            }
+        }
+        CRC(dev_ensure(h, h->w_all, all.size() * 4));
+        CCU(cudaMemcpy(h->w_all.p, all.data(), all.size() * 4, cudaMemcpyHostToDevice));
+        const float *base = (const float *)h->w_all.p;
+        h->h_wtab.resize((size_t)T * md.S);
+        for (size_t k = 0; k < offs.size(); ++k) {
+            const Off &o = offs[k];
+            h->h_wtab[k] = DenseW{base + o.U, base + o.UT, base + o.b1, base + o.W2, base + o.W2T, base + o.b2,
+                                  base + o.W3, base + o.W3T, base + o.b3};
+        }
+        CRC(dev_ensure(h, h->w_tab, sizeof(DenseW) * h->h_wtab.size()));
+        CCU(cudaMemcpy(h->w_tab.p, h->h_wtab.data(), sizeof(DenseW) * h->h_wtab.size(), cudaMemcpyHostToDevice));
+        // radial-pair table
+        std::vector<int32_t> qtab((size_t)md.nqp, 0);
+        for (int l = 0; l <= L; ++l) {
+            const int a0 = l * (l + 1) * (l + 2) / 6, ac = (l + 1) * (l + 2) / 2;
+            int pp = 0;
+            for (int n = 0; n < md.nphi; ++n)
+                for (int n2 = n; n2 < md.nphi; ++n2, ++pp)
+                    qtab[(size_t)l * md.NPp + pp] = n | (n2 << 8) | (a0 << 16) | (ac << 24);
+        }
+        CRC(dev_ensure(h, h->qtab, qtab.size() * 4));
+        CCU(cudaMemcpy(h->qtab.p, qtab.data(), qtab.size() * 4, cudaMemcpyHostToDevice));
+    }
+    // ---- atoms: species, dense tiles ----
+    CRC(dev_ensure(h, h->species_caller, sizeof(int32_t) * (size_t)std::max<int64_t>(n_atoms, 1)));
+    if (n_atoms > 0) CCU(cudaMemcpy(h->species_caller.p, sp.data(), sizeof(int32_t) * (size_t)n_atoms, cudaMemcpyHostToDevice));
+    h->species_count.assign((size_t)md.S, 0);
+    for (int64_t i = 0; i < n_atoms; ++i) h->species_count[(size_t)sp[(size_t)i]]++;
+    {
+        std::vector<DenseTile> tiles;
+        int64_t base = 0;
+        for (int s = 0; s < md.S; ++s) {
+            for (int64_t o = 0; o < h->species_count[(size_t)s]; o += DENSE_TM)
+                tiles.push_back(DenseTile{s, (int32_t)(base + o), (int32_t)std::min<int64_t>(DENSE_TM, h->species_count[(size_t)s] - o)});
+            base += h->species_count[(size_t)s];
+        }
+        h->n_tiles = (int)tiles.size();
+        CRC(dev_ensure(h, h->tiles, sizeof(DenseTile) * std::max<size_t>(tiles.size(), 1)));
+        if (!tiles.empty()) CCU(cudaMemcpy(h->tiles.p, tiles.data(), sizeof(DenseTile) * tiles.size(), cudaMemcpyHostToDevice));
+    }
+    CRC(dev_ensure(h, h->flags, 64));
+    CCU(cudaMemset(h->flags.p, 0, 64));
+    CCU(cudaMallocHost((void **)&h->h_flags, 64));
+    *out = h;
+    return REANN_OK;
+}
+
+extern "C" void reann_destroy(reann_t *h) {
+    if (!h) return;
+    if (h->stream) cudaStreamSynchronize(h->stream); else cudaDeviceSynchronize();
+    DevBuf *bufs[] = {&h->w_all, &h->w_tab, &h->rcen, &h->alpha, &h->c0, &h->qtab, &h->species_caller, &h->tiles,
+                      &h->pos_build, &h->wshift, &h->perm, &h->inv_perm, &h->xrec, &h->img_index, &h->cell_start,
+                      &h->cell_rank, &h->row_ptr, &h->col, &h->rev, &h->sp_list, &h->scratch_a, &h->scratch_b,
+                      &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
+                      &h->geom, &h->rev_rc, &h->c_ext, &h->b, &h->z_stash, &h->bbar, &h->cbar, &h->kappa, &h->gst,
+                      &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch};
+    for (DevBuf *b : bufs) dev_free(h, *b);
+    if (h->h_flags) cudaFreeHost(h->h_flags);
+    for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+    delete h;
+}
+
+extern "C" const char *reann_last_error(const reann_t *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+extern "C" int reann_set_stream(reann_t *h, void *cuda_stream) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->stream) cudaStreamSynchronize(h->stream); else cudaDeviceSynchronize();
+    h->stream = (cudaStream_t)cuda_stream;
+    return REANN_OK;
+}
+
+extern "C" int reann_set_profiling(reann_t *h, int on) {
+    if (!h) return REANN_ERR_ARG;
+    h->profiling = on != 0;
+    return REANN_OK;
+}
+
+static int check_box(reann *h, const double *box9) {
+    if (!box9) return set_err(h, REANN_ERR_ARG, "box is NULL");
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c)
+            if (r != c && box9[3 * r + c] != 0.0) return set_err(h, REANN_ERR_UNSUPPORTED, "only orthorhombic boxes are supported");
+    const double R = h->md.rc + h->md.skin;
+    for (int d = 0; d < 3; ++d)
+        if (!(box9[4 * d] >= R)) return set_err(h, REANN_ERR_BOX, "box length %g < rc + skin = %g", box9[4 * d], R);
+    return REANN_OK;
+}
+
+// positions on the device (staged when the caller passed a host pointer)
+static int device_positions(reann *h, const double *pos, const double **d_pos) {
+    if (h->N == 0) { *d_pos = nullptr; return REANN_OK; }
+    if (!pos) return set_err(h, REANN_ERR_ARG, "pos is NULL");
+    if (is_device_ptr(pos)) { *d_pos = pos; return REANN_OK; }
+    RC(dev_ensure(h, h->pos_stage, sizeof(double) * 3 * (size_t)h->N));
+    CU(h, cudaMemcpyAsync(h->pos_stage.p, pos, sizeof(double) * 3 * (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
+    *d_pos = (const double *)h->pos_stage.p;
+    return REANN_OK;
+}
+
+static int do_build(reann *h, const double *d_pos, const double *box9) {
+    memcpy(h->box_build, box9, sizeof(double) * 9);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (h->profiling) { cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventRecord(e0, h->stream); }
+    h->have_list = false;
+    if (h->N > 0) RC(neighbor_build(h, d_pos));
+    const ModelDims &md = h->md;
+    const int64_t N = h->N;
+    if (N == 0) { h->G = 0; h->n_ext = 0; h->E_list = 0; h->E_rc_build = 0; }
+    // per-evaluation buffers whose size follows the list
+    RC(dev_ensure(h, h->rank16, sizeof(uint16_t) * (size_t)std::max<int64_t>(h->E_list, 1)));
+    RC(dev_ensure(h, h->rc_cnt, sizeof(int32_t) * (size_t)(N + 1)));
+    RC(dev_ensure(h, h->rc_ptr, sizeof(int64_t) * (size_t)(N + 1)));
+    RC(dev_ensure(h, h->scan_ws, scan_workspace_bytes(N + 1)));
+    {
+        const size_t need = sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(h->n_ext, 1) * md.nphip;
+        if (h->c_ext.bytes < need) { RC(dev_ensure(h, h->c_ext, need + need / 16)); }
+        CU(h, cudaMemsetAsync(h->c_ext.p, 0, h->c_ext.bytes, h->stream)); // padded coefficients stay 0
+    }
+    if (!h->b.p) {
+        RC(dev_ensure(h, h->b, sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(N, 1) * md.NB));
+        RC(dev_ensure(h, h->z_stash, sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(N, 1) * h->zs));
+        RC(dev_ensure(h, h->bbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.NB));
+        CU(h, cudaMemsetAsync(h->bbar.p, 0, h->bbar.bytes, h->stream));       // padded rows stay 0
+        RC(dev_ensure(h, h->cbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.nphip));
+        RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
+        RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
+        RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
+        h->n_vir_blocks = edge_bwd_blocks(std::max<int64_t>(N, 1));
+        RC(dev_ensure(h, h->vir_part, sizeof(double) * 9 * (size_t)h->n_vir_blocks));
+        RC(dev_ensure(h, h->red_scratch, sizeof(double) * ((size_t)N / 256 + 2)));
+        RC(dev_ensure(h, h->out_stage, sizeof(double) * (16 + 3 * (size_t)N)));
+    }
+    h->have_list = true;
+    h->n_rebuilds++;
+    if (h->profiling) {
+        cudaEventRecord(e1, h->stream); cudaEventSynchronize(e1);
+        float ms = 0; cudaEventElapsedTime(&ms, e0, e1); h->ms[0] += ms;
+        cudaEventDestroy(e0); cudaEventDestroy(e1);
+    }
+    return REANN_OK;
+}
+
+extern "C" int reann_build_neighbors(reann_t *h, const double *pos, const double *box9) {
+    if (!h) return REANN_ERR_ARG;
+    RC(check_box(h, box9));
+    const double *d_pos = nullptr;
+    RC(device_positions(h, pos, &d_pos));
+    return do_build(h, d_pos, box9);
+}
+
+// profiling marks: event before each kernel group; slot = index into h->ms of the group that follows
+struct Marks {
+    reann *h; std::vector<std::pair<int, int>> m; // (event index, slot)
+    void mark(int slot) {
+        if (!h->profiling) return;
+        const size_t k = m.size();
+        if (h->ev.size() <= k) { cudaEvent_t e; cudaEventCreate(&e); h->ev.push_back(e); }
+        cudaEventRecord(h->ev[k], h->stream);
+        m.push_back({(int)k, slot});
+    }
+    void finish() {
+        if (!h->profiling || m.size() < 2) return;
+        cudaEventSynchronize(h->ev[(size_t)m.back().first]);
+        for (size_t k = 0; k + 1 < m.size(); ++k) {
+            float ms = 0; cudaEventElapsedTime(&ms, h->ev[(size_t)m[k].first], h->ev[(size_t)m[k + 1].first]);
+            h->ms[m[k].second] += ms;
+        }
+        h->n_prof_calls++;
+    }
+};
+
+// skin check + speculative rc-filter count on the current list; ONE stream sync to read both
+static int prep_and_sync(reann *h, const double *d_pos, bool *rebuild, int64_t *n_rc) {
+    LaunchCtx ctx = h->ctx();
+    const int64_t N = h->N;
+    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
+    int32_t *flags = (int32_t *)h->flags.p;
+    CU(h, cudaMemsetAsync(flags, 0, 16, h->stream));
+    const double thr = 0.5 * h->md.skin;
+    launch_skin_check(ctx, d_pos, (const double *)h->pos_build.p, N, thr * thr, flags);
+    launch_refresh(ctx, (XRec *)h->xrec.p, h->n_ext, (const int32_t *)h->perm.p, (const int32_t *)h->wshift.p, d_pos,
+                   Lx, Ly, Lz, (float *)h->c_ext.p, (const float *)h->c0.p, h->md.nphip);
+    launch_filter_count(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p, N, Lx,
+                        Ly, Lz, h->md.rc * h->md.rc, (uint16_t *)h->rank16.p, (int32_t *)h->rc_cnt.p);
+    exclusive_scan_i32_to_i64(ctx, (const int32_t *)h->rc_cnt.p, (int64_t *)h->rc_ptr.p, N, h->scan_ws.p);
+    CU(h, cudaMemcpyAsync(h->h_flags, flags, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaMemcpyAsync(h->h_flags + 2, (int64_t *)h->rc_ptr.p + N, 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    *rebuild = (h->h_flags[0] & 1) != 0;
+    memcpy(n_rc, h->h_flags + 2, 8);
+    return REANN_OK;
+}
+
+extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *box9, double *E, double *F,
+                                   double *virial) {
+    if (!h) return REANN_ERR_ARG;
+    if (!h->have_list) return set_err(h, REANN_ERR_NO_NEIGHBORS, "call reann_build_neighbors first");
+    RC(check_box(h, box9));
+    const ModelDims &md = h->md;
+    const int64_t N = h->N;
+    const double *d_pos = nullptr;
+    RC(device_positions(h, pos, &d_pos));
+    h->n_calls++;
+    Marks mk{h, {}};
+    mk.mark(1);
+    LaunchCtx ctx = h->ctx();
+
+    // ---- A4 + rc-filter count; rebuild when the skin criterion or a box change asks for it ----
+    bool rebuild = false;
+    int64_t n_rc = 0;
+    const bool box_changed = memcmp(box9, h->box_build, sizeof(double) * 9) != 0;
+    if (N > 0) {
+        if (!box_changed) RC(prep_and_sync(h, d_pos, &rebuild, &n_rc));
+        if (box_changed || rebuild) {
+            RC(do_build(h, d_pos, box9));
+            RC(prep_and_sync(h, d_pos, &rebuild, &n_rc));
+        }
+    }
+    h->E_rc = n_rc;
+    if (n_rc > h->cap_rc) {
+        const int64_t cap = n_rc + n_rc / 16 + 1024;
+        RC(dev_ensure(h, h->col_rc, sizeof(uint32_t) * (size_t)cap));
+        RC(dev_ensure(h, h->rev_rc, sizeof(uint32_t) * (size_t)cap));
+        RC(dev_ensure(h, h->geom, sizeof(float4) * (size_t)cap));
+        RC(dev_ensure(h, h->gst, sizeof(float4) * (size_t)cap));
+        RC(dev_ensure(h, h->kappa, sizeof(float) * (size_t)cap * md.nphip));
+        h->cap_rc = cap;
+    }
+    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
+    launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
+                       (const uint32_t *)h->rev.p, N, Lx, Ly, Lz, (const uint16_t *)h->rank16.p,
+                       (const int64_t *)h->rc_ptr.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
+
+    // ---- forward: T layers (Eq. 1, Eq. 2) ----
+    const size_t cstride = (size_t)h->n_ext * md.nphip, bstride = (size_t)N * md.NB, zstride = (size_t)N * h->zs;
+    float *c_ext = (float *)h->c_ext.p, *b = (float *)h->b.p, *zst = (float *)h->z_stash.p;
+    const DenseW *wtab = (const DenseW *)h->w_tab.p;
+    for (int t = 0; t < md.T; ++t) {
+        mk.mark(2);
+        int rcode = launch_edge_fwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
+                                    (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
+                                    (const float *)h->alpha.p, b + t * bstride);
+        if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
+        mk.mark(3);
+        const bool last = t == md.T - 1;
+        rcode = launch_dense_fwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                 (const int32_t *)h->sp_list.p, (const int32_t *)h->qtab.p, b + t * bstride,
+                                 zst + t * zstride, h->zs, last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride,
+                                 last ? 1 : md.nphip);
+        if (rcode) return set_err(h, rcode, "dense forward: unsupported MLP shape or shared-memory size");
+        if (!last) {
+            mk.mark(4);
+            launch_ghost_gather(ctx, c_ext + (t + 1) * cstride, (const XRec *)h->xrec.p, N, h->n_ext, md.nphip);
+        }
+    }
+    // ---- reverse: T layers (Eqs. 3-5) ----
+    if (N > 0) {
+        CU(h, cudaMemsetAsync(h->Fc.p, 0, sizeof(double) * 3 * (size_t)N, h->stream));
+        CU(h, cudaMemsetAsync(h->vir_part.p, 0, sizeof(double) * 9 * (size_t)h->n_vir_blocks, h->stream));
+    }
+    for (int t = md.T - 1; t >= 0; --t) {
+        mk.mark(5);
+        const bool last = t == md.T - 1;
+        int rcode = launch_dense_bwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                     (const int32_t *)h->sp_list.p, b + t * bstride, zst + t * zstride, h->zs,
+                                     last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->bbar.p);
+        if (rcode) return set_err(h, rcode, "dense backward: unsupported MLP shape or shared-memory size");
+        mk.mark(6);
+        rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
+                                (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
+                                (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
+                                (float4 *)h->gst.p, (double *)h->Fc.p, (double *)h->vir_part.p, h->n_vir_blocks);
+        if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
+        mk.mark(7);
+        launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
+                          (const float4 *)h->gst.p, md.nphip, t >= 1, (float *)h->cbar.p, (double *)h->Fc.p);
+    }
+    // ---- outputs (A12) ----
+    mk.mark(8);
+    const bool E_dev = is_device_ptr(E), F_dev = is_device_ptr(F), V_dev = is_device_ptr(virial);
+    double *stage = (double *)h->out_stage.p;
+    double *dE = E ? (E_dev ? E : stage) : stage;
+    double *dV = virial ? (V_dev ? virial : stage + 1) : nullptr;
+    double *dF = F ? (F_dev ? F : stage + 16) : nullptr;
+    launch_output(ctx, N, (const int32_t *)h->inv_perm.p, (const double *)h->Fc.p, (const float *)h->Ei.p,
+                  (const double *)h->vir_part.p, N > 0 ? h->n_vir_blocks : 0, dE, dF, dV, (double *)h->Ei_caller.p,
+                  (double *)h->red_scratch.p);
+    bool need_sync = false;
+    if (E && !E_dev) { CU(h, cudaMemcpyAsync(E, stage, 8, cudaMemcpyDeviceToHost, h->stream)); need_sync = true; }
+    if (virial && !V_dev) { CU(h, cudaMemcpyAsync(virial, stage + 1, 72, cudaMemcpyDeviceToHost, h->stream)); need_sync = true; }
+    if (F && !F_dev && N > 0) { CU(h, cudaMemcpyAsync(F, stage + 16, sizeof(double) * 3 * (size_t)N, cudaMemcpyDeviceToHost, h->stream)); need_sync = true; }
+    mk.mark(8);
+    if (need_sync) CU(h, cudaStreamSynchronize(h->stream));
+    mk.finish();
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}
+
+extern "C" int reann_get_neighbors(reann_t *h, int64_t *n_edges, int64_t *row_ptr, int32_t *j, int8_t *shift) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->N == 0) { if (n_edges) *n_edges = 0; if (row_ptr) row_ptr[0] = 0; return REANN_OK; }
+    return neighbor_export(h, n_edges, row_ptr, j, shift);
+}
+
+extern "C" int reann_get_stats(reann_t *h, reann_stats_t *out) {
+    if (!h || !out) return REANN_ERR_ARG;
+    memset(out, 0, sizeof(*out));
+    out->n_atoms = h->N; out->n_ext = h->n_ext; out->n_edges_list = h->E_list; out->n_edges_rc = h->E_rc;
+    out->n_rebuilds = h->n_rebuilds; out->n_calls = h->n_calls; out->n_launches = h->n_launches;
+    out->ms_build = h->ms[0]; out->ms_prep = h->ms[1]; out->ms_edge_fwd = h->ms[2]; out->ms_dense_fwd = h->ms[3];
+    out->ms_gather = h->ms[4]; out->ms_dense_bwd = h->ms[5]; out->ms_edge_bwd = h->ms[6]; out->ms_rev_gather = h->ms[7];
+    out->ms_output = h->ms[8]; out->n_profiled_calls = h->n_prof_calls; out->bytes_device = h->bytes_device;
+    return REANN_OK;
+}
+
+extern "C" int reann_get_atomic_energies(reann_t *h, double *Ei) {
+    if (!h || !Ei) return REANN_ERR_ARG;
+    if (!h->have_list || h->n_calls == 0) return set_err(h, REANN_ERR_NO_NEIGHBORS, "no evaluation yet");
+    if (h->N == 0) return REANN_OK;
+    CU(h, cudaMemcpyAsync(Ei, h->Ei_caller.p, sizeof(double) * (size_t)h->N,
+                          is_device_ptr(Ei) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    return REANN_OK;
+}
+
+extern "C" int reann_verlet(reann_t *h, double *pos, double *vel, const double *F, const double *inv_mass, double dt,
+                            double acc_unit, int drift) {
+    if (!h || !pos || !vel || !F || !inv_mass) return REANN_ERR_ARG;
+    if (!is_device_ptr(pos) || !is_device_ptr(vel) || !is_device_ptr(F) || !is_device_ptr(inv_mass))
+        return set_err(h, REANN_ERR_ARG, "reann_verlet takes device pointers");
+    launch_verlet(h->ctx(), h->N, pos, vel, F, inv_mass, dt, acc_unit, drift);
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}

@@ -1,0 +1,139 @@
+// common.cuh -- shared declarations of the CUDA implementation (sm_100a only).
+// Notation follows the paper / SURVEY.md section 8: N atoms, G ghosts (periodic images),
+// N_ext = N + G, nphi = N_phi primitives, Na Cartesian monomials, NB = nphip * Na,
+// n_q = (L+1) nphi (nphi+1) / 2 radial-pair products (see dense.cu), H1/H2 MLP widths.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/reann.h"
+
+#define REANN_MAX_S 16
+#define REANN_MAX_T 8
+#define REANN_MAX_NA 20
+#define REANN_MAX_NPHI 16
+
+// ---------------------------------------------------------------------------------------------
+// Ext-atom record, 32 B (one DRAM sector): the WRAPPED position of the owner in FP64, the owner's
+// internal index and the image shift. Edge vectors are formed as (x_owner(j) - x_i) + S*L in
+// FP64, which is exactly antisymmetric under (i <-> j, S <-> -S): both directions of an edge
+// take the same r < rc decision and the same |r|.
+struct __align__(32) XRec {
+    double x, y, z;
+    int32_t owner;     // internal index of the owning local atom (== own index for locals)
+    int8_t sx, sy, sz; // image shift in {-1,0,1}
+    uint8_t species;
+};
+static_assert(sizeof(XRec) == 32, "XRec must be 32 bytes");
+
+// shift code 0..26 = (sx+1)*9 + (sy+1)*3 + (sz+1); 13 = no shift; reverse code = 26 - code
+__host__ __device__ inline int shift_code(int sx, int sy, int sz) { return (sx + 1) * 9 + (sy + 1) * 3 + (sz + 1); }
+
+// col_rc entries carry the neighbour's species in the top 4 bits (N_ext < 2^28)
+#define COL_IDX_MASK 0x0FFFFFFFu
+#define COL_SPECIES_SHIFT 28
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t bytes = 0;
+};
+
+// Per-(layer, species) dense weights, FP32, padded (see dense.cu / api.cu fold_weights()).
+struct DenseW {
+    const float *U;   // [n_qp][H1p]      folded  U = V . W1   (K-major for the forward GEMM)
+    const float *UT;  // [L+1][H1p][NPp]  transposed per-l blocks (for the backward GEMM)
+    const float *b1;  // [H1p]
+    const float *W2;  // [H1p][H2p]
+    const float *W2T; // [H2p][H1p]
+    const float *b2;  // [H2p]
+    const float *W3;  // [H2p][noutp]
+    const float *W3T; // [noutp][H2p]
+    const float *b3;  // [noutp]
+};
+
+struct LayerDims {
+    int H1p, H2p, nout, noutp;
+};
+
+struct ModelDims {
+    int S, T, L, nphi, nphip, Na, NB, norb;
+    int npairs, NPp, nqp; // pairs n<=n' per l; padded to 16; (L+1)*NPp
+    double rc, skin;
+};
+
+// launch counter (kernels launched by the handle) -- every launch goes through LAUNCH()
+struct LaunchCtx {
+    cudaStream_t stream;
+    int64_t *n_launches;
+};
+#define LAUNCH(ctx, kernel, grid, block, smem, ...)                          \
+    do {                                                                     \
+        kernel<<<(grid), (block), (smem), (ctx).stream>>>(__VA_ARGS__);      \
+        ++*(ctx).n_launches;                                                 \
+    } while (0)
+
+static inline unsigned div_up(int64_t a, int64_t b) { return (unsigned)((a + b - 1) / b); }
+
+// ---- scan.cu ----
+// exclusive scan of int32 counts into int64 offsets: out[0] = 0, out[i+1] = sum_{k<=i} in[k]
+size_t scan_workspace_bytes(int64_t n);
+void exclusive_scan_i32_to_i64(const LaunchCtx &ctx, const int32_t *in, int64_t *out, int64_t n, void *workspace);
+
+// ---- neighbor.cu ----
+struct NeighborArgs {
+    int64_t N;
+    double Lb[3];
+    int nc[3];
+    int64_t ncell;
+    double R2;      // (rc+skin)^2
+    double R;       // rc+skin
+    double rc2;     // rc^2
+};
+struct reann; // handle (api.cu)
+int neighbor_build(reann *h, const double *d_pos);   // returns REANN_* code
+int neighbor_export(reann *h, int64_t *n_edges, int64_t *row_ptr, int32_t *j, int8_t *shift);
+
+// ---- edge.cu ----
+void launch_skin_check(const LaunchCtx &ctx, const double *pos, const double *pos_build, int64_t N, double thr2,
+                       int32_t *flag);
+void launch_refresh(const LaunchCtx &ctx, XRec *xrec, int64_t n_ext, const int32_t *perm, const int32_t *wshift,
+                    const double *pos, double Lx, double Ly, double Lz, float *c_ext0, const float *c0, int nphip);
+void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
+                         int64_t N, double Lx, double Ly, double Lz, double rc2, uint16_t *rank16, int32_t *rc_cnt);
+void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
+                        const uint32_t *rev, int64_t N, double Lx, double Ly, double Lz, const uint16_t *rank16,
+                        const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc);
+void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip);
+int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
+                    const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
+                    const float *alpha, float *b);
+int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
+                    const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
+                    const float *alpha, const float *bbar, float *kappa, float4 *gst, double *Fc, double *vir_part,
+                    int n_vir_blocks);
+int edge_bwd_blocks(int64_t N);
+void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *rev_rc,
+                       const float *kappa, const float4 *gst, int nphip, int want_cbar, float *cbar, double *Fc);
+void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, const double *Fc, const float *Ei,
+                   const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
+                   double *Ei_sorted, double *scratch);
+void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
+                   double dt, double acc_unit, int drift);
+
+// ---- dense.cu ----
+struct DenseTile {
+    int32_t species, start, count; // atoms sp_list[start .. start+count) all of `species`
+};
+int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w /*[S]*/,
+                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const int32_t *qtab, const float *b,
+                     float *z_stash, int zs, float *out /* c_ext[t+1] rows (stride nphip) or Ei (stride 1) */,
+                     int out_stride);
+int launch_dense_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w,
+                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *b, const float *z_stash,
+                     int zs, const float *outbar /* cbar rows or NULL for the energy layer */, int outbar_stride,
+                     float *bbar);
+#define DENSE_TM 64 // atoms per dense tile

@@ -1,0 +1,599 @@
+// edge.cu -- per-evaluation edge work: rows A4 (skin check), A5 (edge forward), A8 (ghost gather),
+// A10 (edge backward), A11 (reverse gather) and A12 (outputs) of SURVEY.md section 8(a), plus the
+// per-step rc-filter that compacts the skin list into the r < rc edges all layers reuse
+// (one list, reused by every MP layer).
+//
+// Orbitals (Eq. 1; readings A-2..A-5 of SURVEY.md 8(c)):
+//   x_e[n] = c_j[n] * exp(-alpha_n (r_e - r_n)^2) * f_c(r_e),   f_c(r) = (1 + cos(pi r / rc)) / 2
+//   A_a(r_e) = x^lx y^ly z^lz,  a = (lx,ly,lz), lx+ly+lz <= L (graded order, see monomials<>())
+//   b_i[n,a] = sum_{e in row(i), r_e < rc} x_e[n] A_a(r_e)
+// Backward (Eqs. 3-5, vector-Jacobian products):
+//   S_n = sum_a bbar_i[n,a] A_a;  P_a = sum_n bbar_i[n,a] x_e[n]
+//   g_e = (sum_n c_j[n] R'_n S_n) r_hat + sum_a P_a grad A_a;   kappa_e[n] = R_n S_n  (t >= 1)
+//   cbar_k[n] = sum_{e in row(k)} kappa_{rev(e)}[n];   F_k = sum_{e in row(k)} (g_e - g_{rev(e)})
+// No floating-point atomics anywhere: the neighbour-side sums are gathers through rev[].
+#include "common.cuh"
+
+namespace {
+
+constexpr int EW = 4; // warps per block in the edge kernels
+
+// ------------------------------------------------------------------------------------------ A4
+__global__ void k_skin_check(const double *__restrict__ pos, const double *__restrict__ pos_build, int64_t n3,
+                             double thr2, int32_t *__restrict__ flag) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i * 3 < n3) {
+        double dx = pos[3 * i] - pos_build[3 * i], dy = pos[3 * i + 1] - pos_build[3 * i + 1],
+               dz = pos[3 * i + 2] - pos_build[3 * i + 2];
+        moved = (dx * dx + dy * dy + dz * dz) > thr2;
+    }
+    if (__syncthreads_or(moved) && threadIdx.x == 0) atomicOr(flag, 1);
+}
+
+// positions of all ext atoms in the build-time wrapped frame; layer-0 coefficients c^0 = c0[species]
+__global__ void k_refresh(XRec *__restrict__ xrec, int64_t n_ext, const int32_t *__restrict__ perm,
+                          const int32_t *__restrict__ wshift, const double *__restrict__ pos, double Lx, double Ly,
+                          double Lz, float *__restrict__ c_ext0, const float *__restrict__ c0, int nphip) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_ext) return;
+    XRec r = xrec[k];
+    const int64_t i = perm[r.owner];
+    r.x = __dsub_rn(pos[3 * i], __dmul_rn((double)wshift[3 * i], Lx));
+    r.y = __dsub_rn(pos[3 * i + 1], __dmul_rn((double)wshift[3 * i + 1], Ly));
+    r.z = __dsub_rn(pos[3 * i + 2], __dmul_rn((double)wshift[3 * i + 2], Lz));
+    xrec[k] = r;
+    for (int n = 0; n < nphip; ++n) c_ext0[k * nphip + n] = c0[r.species * nphip + n];
+}
+
+__device__ __forceinline__ double edge_d2(const XRec &me, const XRec &o, double Lx, double Ly, double Lz, double *dx,
+                                          double *dy, double *dz) {
+    *dx = __dadd_rn(__dsub_rn(o.x, me.x), __dmul_rn((double)o.sx, Lx));
+    *dy = __dadd_rn(__dsub_rn(o.y, me.y), __dmul_rn((double)o.sy, Ly));
+    *dz = __dadd_rn(__dsub_rn(o.z, me.z), __dmul_rn((double)o.sz, Lz));
+    return __dadd_rn(__dadd_rn(__dmul_rn(*dx, *dx), __dmul_rn(*dy, *dy)), __dmul_rn(*dz, *dz));
+}
+
+// rc-filter, pass 1: rank of every accepted list entry inside its row (0xFFFF = rejected)
+__global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict__ xrec,
+                                                          const int64_t *__restrict__ row_ptr,
+                                                          const int32_t *__restrict__ col, int64_t N, double Lx,
+                                                          double Ly, double Lz, double rc2,
+                                                          uint16_t *__restrict__ rank16, int32_t *__restrict__ rc_cnt) {
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (int64_t)blockIdx.x * EW + (threadIdx.x >> 5);
+    if (i >= N) return;
+    const XRec me = xrec[i];
+    const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1];
+    int cnt = 0;
+    for (int64_t eb = r0; eb < r1; eb += 32) {
+        const int64_t e = eb + lane;
+        bool in = false;
+        if (e < r1) {
+            double dx, dy, dz;
+            in = edge_d2(me, xrec[col[e]], Lx, Ly, Lz, &dx, &dy, &dz) < rc2;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, in);
+        if (e < r1) rank16[e] = in ? (uint16_t)(cnt + __popc(m & ((1u << lane) - 1))) : (uint16_t)0xFFFF;
+        cnt += __popc(m);
+    }
+    if (lane == 0) rc_cnt[i] = cnt;
+}
+
+// rc-filter, pass 2: compact rows (neighbour ext index | species<<28, edge vector + length in FP32
+// rounded once from the FP64 difference, index of the reverse compact edge)
+__global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict__ xrec,
+                                                         const int64_t *__restrict__ row_ptr,
+                                                         const int32_t *__restrict__ col,
+                                                         const uint32_t *__restrict__ rev, int64_t N, double Lx,
+                                                         double Ly, double Lz, const uint16_t *__restrict__ rank16,
+                                                         const int64_t *__restrict__ rc_ptr,
+                                                         uint32_t *__restrict__ col_rc, float4 *__restrict__ geom,
+                                                         uint32_t *__restrict__ rev_rc) {
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (int64_t)blockIdx.x * EW + (threadIdx.x >> 5);
+    if (i >= N) return;
+    const XRec me = xrec[i];
+    const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1], c0 = rc_ptr[i];
+    for (int64_t e = r0 + lane; e < r1; e += 32) {
+        const uint16_t rk = rank16[e];
+        if (rk == 0xFFFF) continue;
+        const int32_t j = col[e];
+        const XRec o = xrec[j];
+        double dx, dy, dz;
+        const double d2 = edge_d2(me, o, Lx, Ly, Lz, &dx, &dy, &dz);
+        const int64_t ce = c0 + rk;
+        col_rc[ce] = (uint32_t)j | ((uint32_t)o.species << COL_SPECIES_SHIFT);
+        geom[ce] = make_float4((float)dx, (float)dy, (float)dz, (float)sqrt(d2));
+        rev_rc[ce] = (uint32_t)(rc_ptr[o.owner] + rank16[rev[e]]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ A8
+// c_ext[N+g][:] = c[owner[g]][:]  -- the paper's forward LA -> GA message.
+__global__ void k_ghost_gather(float *__restrict__ c_ext, const XRec *__restrict__ xrec, int64_t N, int64_t n_ext,
+                               int nphip) {
+    const int q4 = nphip >> 2;
+    int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t g = N + idx / q4;
+    if (g >= n_ext) return;
+    int part = (int)(idx % q4);
+    const float4 *src = reinterpret_cast<const float4 *>(c_ext + (int64_t)xrec[g].owner * nphip);
+    reinterpret_cast<float4 *>(c_ext + g * nphip)[part] = src[part];
+}
+
+// ------------------------------------------------------------------------------------------ orbitals
+// Cartesian monomials in graded order: 1 | x y z | xx xy xz yy yz zz | xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz
+template <int NA>
+__device__ __forceinline__ void monomials(float x, float y, float z, float *A) {
+    A[0] = 1.0f;
+    if constexpr (NA > 1) { A[1] = x; A[2] = y; A[3] = z; }
+    if constexpr (NA > 4) { A[4] = x * x; A[5] = x * y; A[6] = x * z; A[7] = y * y; A[8] = y * z; A[9] = z * z; }
+    if constexpr (NA > 10) {
+        A[10] = A[4] * x; A[11] = A[4] * y; A[12] = A[4] * z; A[13] = A[7] * x; A[14] = A[5] * z;
+        A[15] = A[9] * x; A[16] = A[7] * y; A[17] = A[7] * z; A[18] = A[9] * y; A[19] = A[9] * z;
+    }
+}
+// sum_a P_a grad A_a
+template <int NA>
+__device__ __forceinline__ void monomial_vjp(const float *A, const float *P, float &gx, float &gy, float &gz) {
+    gx = gy = gz = 0.0f;
+    if constexpr (NA > 1) { gx = P[1]; gy = P[2]; gz = P[3]; }
+    if constexpr (NA > 4) {
+        const float x = A[1], y = A[2], z = A[3];
+        gx += 2.0f * x * P[4] + y * P[5] + z * P[6];
+        gy += x * P[5] + 2.0f * y * P[7] + z * P[8];
+        gz += x * P[6] + y * P[8] + 2.0f * z * P[9];
+    }
+    if constexpr (NA > 10) {
+        gx += 3.0f * A[4] * P[10] + 2.0f * A[5] * P[11] + 2.0f * A[6] * P[12] + A[7] * P[13] + A[8] * P[14] + A[9] * P[15];
+        gy += A[4] * P[11] + 2.0f * A[5] * P[13] + A[6] * P[14] + 3.0f * A[7] * P[16] + 2.0f * A[8] * P[17] + A[9] * P[18];
+        gz += A[4] * P[12] + A[5] * P[14] + 2.0f * A[6] * P[15] + A[7] * P[17] + 2.0f * A[8] * P[18] + 3.0f * A[9] * P[19];
+    }
+}
+
+struct RadialTab { // per layer: [S][NPHIP]; alpha pre-multiplied by log2(e)
+    const float *rcen, *alpha2;
+    float inv_rc;
+};
+
+// ------------------------------------------------------------------------------------------ A5
+// Warp-autonomous: a warp owns APW = 32/LPA atoms. Per chunk of 32 edges of one atom the lanes
+// first work one-edge-per-lane (radial functions x_e[n], monomials A_a -> shared memory), then
+// every lane accumulates its PN x PA block of b_i[n,a] over the staged edges (operands read as
+// broadcast vectors from shared memory, accumulators in registers, no atomics).
+template <int NPHIP, int NA, int PN, int PA>
+struct FwdCfg {
+    static constexpr int NG = NPHIP / PN, AG = (NA + PA - 1) / PA, LPA = NG * AG, APW = 32 / LPA;
+    static constexpr int AST = (PA <= 4) ? 4 : 8;       // floats reserved per a-group (16-B aligned)
+    static constexpr int ROW = NPHIP + AG * AST + 4;     // +4: de-phase rows across banks
+    static constexpr int SMEM = EW * APW * 32 * ROW * 4;
+    static_assert(NPHIP % PN == 0 && 32 % LPA == 0 && NPHIP % 4 == 0, "bad edge-forward tiling");
+};
+
+template <int NPHIP, int NA, int PN, int PA>
+__global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *__restrict__ rc_ptr,
+                                                      const uint32_t *__restrict__ col_rc,
+                                                      const float4 *__restrict__ geom,
+                                                      const float *__restrict__ c_ext, RadialTab rt,
+                                                      float *__restrict__ b) {
+    using C = FwdCfg<NPHIP, NA, PN, PA>;
+    extern __shared__ __align__(16) float smem_f[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *stage = smem_f + (size_t)warp * C::APW * 32 * C::ROW;
+    const int sub = lane / C::LPA, sl = lane % C::LPA, p = sl % C::NG, q = sl / C::NG;
+    const int64_t atom0 = ((int64_t)blockIdx.x * EW + warp) * C::APW;
+    if (atom0 >= N) return;
+    const int64_t my_atom = atom0 + sub;
+    int64_t my_beg = 0, my_end = 0;
+    if (my_atom < N) { my_beg = rc_ptr[my_atom]; my_end = rc_ptr[my_atom + 1]; }
+    int64_t maxlen = my_end - my_beg;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, d));
+    float acc[PN][PA];
+#pragma unroll
+    for (int a = 0; a < PN; ++a)
+#pragma unroll
+        for (int c = 0; c < PA; ++c) acc[a][c] = 0.0f;
+
+    for (int64_t c0 = 0; c0 < maxlen; c0 += 32) {
+        // ---- phase 1: one edge per lane ----
+#pragma unroll
+        for (int s = 0; s < C::APW; ++s) {
+            const int64_t beg = __shfl_sync(0xffffffffu, my_beg, s * C::LPA);
+            const int64_t end = __shfl_sync(0xffffffffu, my_end, s * C::LPA);
+            const int64_t e = beg + c0 + lane;
+            if (e < end) {
+                const float4 g = geom[e];
+                const uint32_t cj = col_rc[e];
+                const int sj = cj >> COL_SPECIES_SHIFT;
+                const float4 *cptr = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
+                const float fc = 0.5f + 0.5f * cospif(g.w * rt.inv_rc);
+                float *row = stage + (size_t)(s * 32 + lane) * C::ROW;
+#pragma unroll
+                for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
+                    const float4 cv = cptr[n4];
+                    const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[n4];
+                    const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[n4];
+                    float4 xv;
+                    float d;
+                    d = g.w - rc4.x; xv.x = cv.x * (exp2f(-al4.x * d * d) * fc);
+                    d = g.w - rc4.y; xv.y = cv.y * (exp2f(-al4.y * d * d) * fc);
+                    d = g.w - rc4.z; xv.z = cv.z * (exp2f(-al4.z * d * d) * fc);
+                    d = g.w - rc4.w; xv.w = cv.w * (exp2f(-al4.w * d * d) * fc);
+                    reinterpret_cast<float4 *>(row)[n4] = xv;
+                }
+                float A[C::AG * PA];
+#pragma unroll
+                for (int a = NA; a < C::AG * PA; ++a) A[a] = 0.0f;
+                monomials<NA>(g.x, g.y, g.z, A);
+#pragma unroll
+                for (int ag = 0; ag < C::AG; ++ag)
+#pragma unroll
+                    for (int pa = 0; pa < PA; ++pa) row[NPHIP + ag * C::AST + pa] = A[ag * PA + pa];
+            }
+        }
+        __syncwarp();
+        // ---- phase 2: register-tiled accumulation over the staged edges of my atom ----
+        int64_t cnt64 = my_end - (my_beg + c0);
+        const int cnt = cnt64 > 32 ? 32 : (cnt64 < 0 ? 0 : (int)cnt64);
+        const float *rowb = stage + (size_t)(sub * 32) * C::ROW;
+#pragma unroll 4
+        for (int k = 0; k < cnt; ++k) {
+            const float *row = rowb + (size_t)k * C::ROW;
+            float xv[PN], av[PA];
+            if constexpr (PN == 4) {
+                const float4 v = *reinterpret_cast<const float4 *>(row + p * 4);
+                xv[0] = v.x; xv[1] = v.y; xv[2] = v.z; xv[3] = v.w;
+            } else if constexpr (PN == 2) {
+                const float2 v = *reinterpret_cast<const float2 *>(row + p * 2);
+                xv[0] = v.x; xv[1] = v.y;
+            } else {
+#pragma unroll
+                for (int a = 0; a < PN; ++a) xv[a] = row[p * PN + a];
+            }
+            const float *ar = row + NPHIP + q * C::AST;
+            if constexpr (PA >= 4) {
+                const float4 v = *reinterpret_cast<const float4 *>(ar);
+                av[0] = v.x; av[1] = v.y; av[2] = v.z; av[3] = v.w;
+#pragma unroll
+                for (int c = 4; c < PA; ++c) av[c] = ar[c];
+            } else {
+#pragma unroll
+                for (int c = 0; c < PA; ++c) av[c] = ar[c];
+            }
+#pragma unroll
+            for (int a = 0; a < PN; ++a)
+#pragma unroll
+                for (int c = 0; c < PA; ++c) acc[a][c] = fmaf(xv[a], av[c], acc[a][c]);
+        }
+        __syncwarp();
+    }
+    if (my_atom < N) {
+        float *bi = b + my_atom * (int64_t)(NPHIP * NA);
+#pragma unroll
+        for (int a = 0; a < PN; ++a)
+#pragma unroll
+            for (int c = 0; c < PA; ++c)
+                if (q * PA + c < NA) bi[(p * PN + a) * NA + q * PA + c] = acc[a][c];
+    }
+}
+
+// ------------------------------------------------------------------------------------------ A10
+// Warp per atom, one edge per lane; bbar_i is broadcast from shared memory, S_n and P_a stay in the
+// lane's registers, so there is no cross-lane reduction per edge. Orbitals are recomputed (nothing
+// per-edge is kept from the forward pass). Writes the per-edge stash g_e (float4) and kappa_e.
+template <int NPHIP, int NA>
+__global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
+                                                      const uint32_t *__restrict__ col_rc,
+                                                      const float4 *__restrict__ geom,
+                                                      const float *__restrict__ c_ext, RadialTab rt,
+                                                      const float *__restrict__ bbar, int want_kappa,
+                                                      float *__restrict__ kappa, float4 *__restrict__ gst,
+                                                      double *__restrict__ Fc, double *__restrict__ vir_part) {
+    constexpr int NB = NPHIP * NA;
+    __shared__ __align__(16) float bb_s[EW][NB];
+    __shared__ double vir_s[EW][9];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t i = (int64_t)blockIdx.x * EW + warp;
+    float aF[3] = {0.f, 0.f, 0.f}, aV[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) aV[k] = 0.f;
+    if (i < N) {
+        const float4 *src = reinterpret_cast<const float4 *>(bbar + i * (int64_t)NB);
+        for (int k = lane; k < NB / 4; k += 32) reinterpret_cast<float4 *>(bb_s[warp])[k] = src[k];
+        __syncwarp();
+        const int64_t beg = rc_ptr[i], end = rc_ptr[i + 1];
+        const float pi_rc = 3.14159265358979f * rt.inv_rc;
+        for (int64_t e = beg + lane; e < end; e += 32) {
+            const float4 g = geom[e];
+            const uint32_t cj = col_rc[e];
+            const int sj = cj >> COL_SPECIES_SHIFT;
+            const float4 *cptr = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
+            float sn, cs;
+            sincospif(g.w * rt.inv_rc, &sn, &cs);
+            const float fc = 0.5f + 0.5f * cs, dfc = -0.5f * pi_rc * sn;
+            float A[NA], P[NA];
+            monomials<NA>(g.x, g.y, g.z, A);
+#pragma unroll
+            for (int a = 0; a < NA; ++a) P[a] = 0.f;
+            // four rows n of bbar_i per outer iteration (one float4 of c_j / r_n / alpha_n / kappa);
+            // the outer loop is kept rolled so that the shared-memory loads are not all hoisted.
+            float radial = 0.f;
+            float4 *kp = reinterpret_cast<float4 *>(kappa + e * (int64_t)NPHIP);
+#pragma unroll 1
+            for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
+                const float4 cv = cptr[n4];
+                const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[n4];
+                const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[n4];
+                const float cva[4] = {cv.x, cv.y, cv.z, cv.w}, rca[4] = {rc4.x, rc4.y, rc4.z, rc4.w},
+                            ala[4] = {al4.x, al4.y, al4.z, al4.w};
+                float Rn[4], xn[4], yn[4], S[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const float d = g.w - rca[u];
+                    const float ex = exp2f(-ala[u] * d * d);
+                    // alpha2 = alpha*log2(e): d/dr exp(-alpha d^2) = -2 ln2 alpha2 d ex
+                    Rn[u] = ex * fc;
+                    xn[u] = cva[u] * Rn[u];
+                    yn[u] = cva[u] * ((-1.3862943611198906f * ala[u] * d * fc + dfc) * ex);
+                    S[u] = 0.f;
+                }
+                const float4 *bb4 = reinterpret_cast<const float4 *>(bb_s[warp] + n4 * 4 * NA);
+#pragma unroll
+                for (int f4 = 0; f4 < NA; ++f4) { // 4 rows x NA values = NA float4
+                    const float4 v = bb4[f4];
+                    const float va[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int f = f4 * 4 + u, nl = f / NA, a = f % NA;
+                        S[nl] = fmaf(va[u], A[a], S[nl]);
+                        P[a] = fmaf(va[u], xn[nl], P[a]);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) radial = fmaf(yn[u], S[u], radial);
+                if (want_kappa) kp[n4] = make_float4(Rn[0] * S[0], Rn[1] * S[1], Rn[2] * S[2], Rn[3] * S[3]);
+            }
+            float gx, gy, gz;
+            monomial_vjp<NA>(A, P, gx, gy, gz);
+            const float rr = radial / g.w;
+            gx = fmaf(rr, g.x, gx); gy = fmaf(rr, g.y, gy); gz = fmaf(rr, g.z, gz);
+            gst[e] = make_float4(gx, gy, gz, 0.f);
+            aF[0] += gx; aF[1] += gy; aF[2] += gz;
+            aV[0] -= g.x * gx; aV[1] -= g.x * gy; aV[2] -= g.x * gz;
+            aV[3] -= g.y * gx; aV[4] -= g.y * gy; aV[5] -= g.y * gz;
+            aV[6] -= g.z * gx; aV[7] -= g.z * gy; aV[8] -= g.z * gz;
+        }
+    }
+    // fixed-order reductions: lanes (butterfly), then warps, then one slot per block
+    double dF[3], dV[9];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dF[k] = (double)aF[k];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) dV[k] = (double)aV[k];
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) dF[k] += __shfl_xor_sync(0xffffffffu, dF[k], d);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) dV[k] += __shfl_xor_sync(0xffffffffu, dV[k], d);
+    }
+    if (lane == 0) {
+        if (i < N) { Fc[3 * i] += dF[0]; Fc[3 * i + 1] += dF[1]; Fc[3 * i + 2] += dF[2]; }
+#pragma unroll
+        for (int k = 0; k < 9; ++k) vir_s[warp][k] = dV[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 9) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < EW; ++w) s += vir_s[w][threadIdx.x];
+        vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x] += s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ A11
+// Reverse gather (the paper's backward GA -> LA gradient message as a vJp of N_phi numbers per
+// edge): cbar_k[n] = sum_e kappa[rev(e)][n];  F_k -= sum_e g[rev(e)].
+template <int NPHIP>
+__global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t *__restrict__ rc_ptr,
+                                                        const uint32_t *__restrict__ rev_rc,
+                                                        const float *__restrict__ kappa,
+                                                        const float4 *__restrict__ gst, int want_cbar,
+                                                        float *__restrict__ cbar, double *__restrict__ Fc) {
+    constexpr int PARTS = NPHIP / 4, EPS = 32 / PARTS; // float4 parts per edge, edges per warp step
+    __shared__ float4 red_s[EW][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * EW + warp;
+    if (k >= N) return;
+    const int64_t beg = rc_ptr[k], end = rc_ptr[k + 1];
+    double f0 = 0.0, f1 = 0.0, f2 = 0.0;
+    for (int64_t e = beg + lane; e < end; e += 32) {
+        const float4 g = gst[rev_rc[e]];
+        f0 -= (double)g.x; f1 -= (double)g.y; f2 -= (double)g.z;
+    }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) {
+        f0 += __shfl_xor_sync(0xffffffffu, f0, d);
+        f1 += __shfl_xor_sync(0xffffffffu, f1, d);
+        f2 += __shfl_xor_sync(0xffffffffu, f2, d);
+    }
+    if (lane == 0) { Fc[3 * k] += f0; Fc[3 * k + 1] += f1; Fc[3 * k + 2] += f2; }
+    if (!want_cbar) return;
+    const int eo = lane / PARTS, part = lane % PARTS;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (eo < EPS)
+        for (int64_t e = beg + eo; e < end; e += EPS) {
+            const float4 v = reinterpret_cast<const float4 *>(kappa + (int64_t)rev_rc[e] * NPHIP)[part];
+            acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+        }
+    red_s[warp][lane] = (eo < EPS) ? acc : make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+    if (lane < PARTS) {
+        float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int q = 0; q < EPS; ++q) {
+            const float4 v = red_s[warp][q * PARTS + lane];
+            s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
+        }
+        reinterpret_cast<float4 *>(cbar + k * (int64_t)NPHIP)[lane] = s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ A12
+constexpr int OUT_TPB = 256;
+__global__ void __launch_bounds__(OUT_TPB) k_output_a(int64_t N, const int32_t *__restrict__ inv_perm,
+                                                      const double *__restrict__ Fc, const float *__restrict__ Ei,
+                                                      double *__restrict__ F_out, double *__restrict__ Ei_caller,
+                                                      double *__restrict__ partial) {
+    __shared__ double red[OUT_TPB];
+    const int64_t i = (int64_t)blockIdx.x * OUT_TPB + threadIdx.x; // caller index
+    double e = 0.0;
+    if (i < N) {
+        const int64_t k = inv_perm[i];
+        e = (double)Ei[k];
+        if (Ei_caller) Ei_caller[i] = e;
+        if (F_out) { F_out[3 * i] = Fc[3 * k]; F_out[3 * i + 1] = Fc[3 * k + 1]; F_out[3 * i + 2] = Fc[3 * k + 2]; }
+    }
+    red[threadIdx.x] = e;
+    __syncthreads();
+    for (int s = OUT_TPB / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = red[0];
+}
+__global__ void __launch_bounds__(OUT_TPB) k_output_b(int n_part, const double *__restrict__ partial,
+                                                      const double *__restrict__ vir_part, int n_vir,
+                                                      double *__restrict__ E_out, double *__restrict__ vir_out) {
+    __shared__ double red[OUT_TPB];
+    for (int q = 0; q < 10; ++q) {
+        double s = 0.0;
+        if (q == 0) { for (int k = threadIdx.x; k < n_part; k += OUT_TPB) s += partial[k]; }
+        else if (vir_out) { for (int k = threadIdx.x; k < n_vir; k += OUT_TPB) s += vir_part[(int64_t)k * 9 + (q - 1)]; }
+        red[threadIdx.x] = s;
+        __syncthreads();
+        for (int st = OUT_TPB / 2; st > 0; st >>= 1) {
+            if (threadIdx.x < st) red[threadIdx.x] += red[threadIdx.x + st];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) {
+            if (q == 0) { if (E_out) *E_out = red[0]; }
+            else if (vir_out) vir_out[q - 1] = red[0];
+        }
+        __syncthreads();
+    }
+}
+
+__global__ void k_verlet(int64_t N, double *__restrict__ pos, double *__restrict__ vel, const double *__restrict__ F,
+                         const double *__restrict__ inv_mass, double dt, double acc_unit, int drift) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double s = 0.5 * dt * acc_unit * inv_mass[i];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        double v = vel[3 * i + d] + s * F[3 * i + d];
+        vel[3 * i + d] = v;
+        if (drift) pos[3 * i + d] += dt * v;
+    }
+}
+
+} // namespace
+
+// ============================================================================================ host
+void launch_skin_check(const LaunchCtx &ctx, const double *pos, const double *pos_build, int64_t N, double thr2,
+                       int32_t *flag) {
+    if (N > 0) LAUNCH(ctx, k_skin_check, div_up(N, 256), 256, 0, pos, pos_build, 3 * N, thr2, flag);
+}
+void launch_refresh(const LaunchCtx &ctx, XRec *xrec, int64_t n_ext, const int32_t *perm, const int32_t *wshift,
+                    const double *pos, double Lx, double Ly, double Lz, float *c_ext0, const float *c0, int nphip) {
+    if (n_ext > 0) LAUNCH(ctx, k_refresh, div_up(n_ext, 256), 256, 0, xrec, n_ext, perm, wshift, pos, Lx, Ly, Lz, c_ext0, c0, nphip);
+}
+void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
+                         int64_t N, double Lx, double Ly, double Lz, double rc2, uint16_t *rank16, int32_t *rc_cnt) {
+    if (N > 0) LAUNCH(ctx, k_filter_count, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, N, Lx, Ly, Lz, rc2, rank16, rc_cnt);
+}
+void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
+                        const uint32_t *rev, int64_t N, double Lx, double Ly, double Lz, const uint16_t *rank16,
+                        const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc) {
+    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, rev, N, Lx, Ly, Lz, rank16, rc_ptr, col_rc, geom, rev_rc);
+}
+void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip) {
+    const int64_t work = (n_ext - N) * (nphip / 4);
+    if (work > 0) LAUNCH(ctx, k_ghost_gather, div_up(work, 256), 256, 0, c_ext, xrec, N, n_ext, nphip);
+}
+
+template <int NPHIP, int NA, int PN, int PA>
+static int run_edge_fwd(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
+                        const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
+    using C = FwdCfg<NPHIP, NA, PN, PA>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_edge_fwd<NPHIP, NA, PN, PA>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) != cudaSuccess)
+            return REANN_ERR_CUDA;
+        attr_set = true;
+    }
+    LAUNCH(ctx, (k_edge_fwd<NPHIP, NA, PN, PA>), div_up(N, (int64_t)EW * C::APW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    return REANN_OK;
+}
+
+#define EDGE_DISPATCH(M)                                                                                 \
+    switch (md.nphip * 100 + md.Na) {                                                                    \
+        case 401: M(4, 1, 1, 1) case 404: M(4, 4, 1, 4) case 410: M(4, 10, 1, 5) case 420: M(4, 20, 1, 5)      \
+        case 801: M(8, 1, 2, 1) case 804: M(8, 4, 2, 4) case 810: M(8, 10, 2, 5) case 820: M(8, 20, 2, 5)      \
+        case 1201: M(12, 1, 3, 1) case 1204: M(12, 4, 3, 4) case 1210: M(12, 10, 3, 5) case 1220: M(12, 20, 3, 5) \
+        case 1601: M(16, 1, 2, 1) case 1604: M(16, 4, 2, 4) case 1610: M(16, 10, 2, 5) case 1620: M(16, 20, 2, 5) \
+        default: return REANN_ERR_UNSUPPORTED;                                                           \
+    }
+
+int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
+                    const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
+                    const float *alpha, float *b) {
+    if (N <= 0) return REANN_OK;
+    RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
+#define M(NP, NA_, PN_, PA_) return run_edge_fwd<NP, NA_, PN_, PA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    EDGE_DISPATCH(M)
+#undef M
+}
+
+int edge_bwd_blocks(int64_t N) { return (int)div_up(N, EW); }
+
+int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
+                    const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
+                    const float *alpha, const float *bbar, float *kappa, float4 *gst, double *Fc, double *vir_part,
+                    int n_vir_blocks) {
+    if (N <= 0) return REANN_OK;
+    (void)n_vir_blocks;
+    RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
+    const int want_kappa = t >= 1;
+#define M(NP, NA_, PN_, PA_)                                                                                  \
+    LAUNCH(ctx, (k_edge_bwd<NP, NA_>), div_up(N, EW), EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt, bbar,   \
+           want_kappa, kappa, gst, Fc, vir_part);                                                             \
+    return REANN_OK;
+    EDGE_DISPATCH(M)
+#undef M
+}
+
+void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *rev_rc,
+                       const float *kappa, const float4 *gst, int nphip, int want_cbar, float *cbar, double *Fc) {
+    if (N <= 0) return;
+    switch (nphip) {
+        case 4: LAUNCH(ctx, k_rev_gather<4>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc); break;
+        case 8: LAUNCH(ctx, k_rev_gather<8>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc); break;
+        case 12: LAUNCH(ctx, k_rev_gather<12>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc); break;
+        default: LAUNCH(ctx, k_rev_gather<16>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc); break;
+    }
+}
+
+void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, const double *Fc, const float *Ei,
+                   const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
+                   double *Ei_caller, double *scratch) {
+    const int nb = (int)div_up(N > 0 ? N : 1, OUT_TPB);
+    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, scratch);
+    LAUNCH(ctx, k_output_b, 1, OUT_TPB, 0, nb, (const double *)scratch, vir_part, n_vir_blocks, E_out, vir_out);
+}
+
+void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
+                   double dt, double acc_unit, int drift) {
+    if (N > 0) LAUNCH(ctx, k_verlet, div_up(N, 256), 256, 0, N, pos, vel, F, inv_mass, dt, acc_unit, drift);
+}
