@@ -193,7 +193,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
             for (int s = 0; s < md.S; ++s) {
                 const int k = t * md.S + s;
                 Off o;
-                o.U = reserve((size_t)md.nqp * H1p); o.UT = reserve((size_t)(L + 1) * H1p * md.NPp);
+                o.U = reserve((size_t)md.nqp * H1p); o.UT = reserve((size_t)H1p * md.nqp);
                 o.b1 = reserve(H1p); o.W2 = reserve((size_t)H1p * H2p); o.W2T = reserve((size_t)H2p * H1p);
                 o.b2 = reserve(H2p); o.W3 = reserve((size_t)H2p * nout); o.W3T = reserve((size_t)nout * H2p);
                 o.b3 = reserve(nout);
@@ -211,7 +211,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
                                 double acc = 0.0;
                                 for (int m = 0; m < v.norb; ++m) acc += Vq[(size_t)m] * W1[(size_t)m * H1 + hh];
                                 all[o.U + q * H1p + hh] = (float)acc;
-                                all[o.UT + ((size_t)l * H1p + hh) * md.NPp + pp] = (float)acc;
+                                all[o.UT + (size_t)hh * md.nqp + q] = (float)acc;
                             }
                         }
                 }
@@ -287,7 +287,7 @@ extern "C" void reann_destroy(reann_t *h) {
                       &h->cell_rank, &h->row_ptr, &h->col, &h->rev, &h->sp_list, &h->scratch_a, &h->scratch_b,
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
                       &h->geom, &h->rev_rc, &h->c_ext, &h->b, &h->z_stash, &h->bbar, &h->cbar, &h->kappa, &h->gst,
-                      &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch};
+                      &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch, &h->Qbuf};
     for (DevBuf *b : bufs) dev_free(h, *b);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
@@ -356,6 +356,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->bbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.NB));
         CU(h, cudaMemsetAsync(h->bbar.p, 0, h->bbar.bytes, h->stream));       // padded rows stay 0
         RC(dev_ensure(h, h->cbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.nphip));
+        RC(dev_ensure(h, h->Qbuf, sizeof(float) * ((size_t)std::max<int64_t>(N, 1) + DENSE_TM * 2) * md.nqp));
         RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
@@ -477,10 +478,11 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
         mk.mark(3);
         const bool last = t == md.T - 1;
+        launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, (const int32_t *)h->qtab.p, b + t * bstride,
+                        (float *)h->Qbuf.p);
         rcode = launch_dense_fwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                 (const int32_t *)h->sp_list.p, (const int32_t *)h->qtab.p, b + t * bstride,
-                                 zst + t * zstride, h->zs, last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride,
-                                 last ? 1 : md.nphip);
+                                 (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
+                                 last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip);
         if (rcode) return set_err(h, rcode, "dense forward: unsupported MLP shape or shared-memory size");
         if (!last) {
             mk.mark(4);
@@ -496,9 +498,11 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         mk.mark(5);
         const bool last = t == md.T - 1;
         int rcode = launch_dense_bwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                     (const int32_t *)h->sp_list.p, b + t * bstride, zst + t * zstride, h->zs,
-                                     last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->bbar.p);
+                                     (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
+                                     last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);
         if (rcode) return set_err(h, rcode, "dense backward: unsupported MLP shape or shared-memory size");
+        launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, b + t * bstride, (const float *)h->Qbuf.p,
+                        (float *)h->bbar.p);
         mk.mark(6);
         rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
                                 (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,

@@ -45,7 +45,7 @@ struct DevBuf {
 // Per-(layer, species) dense weights, FP32, padded (see dense.cu / api.cu fold_weights()).
 struct DenseW {
     const float *U;   // [n_qp][H1p]      folded  U = V . W1   (K-major for the forward GEMM)
-    const float *UT;  // [L+1][H1p][NPp]  transposed per-l blocks (for the backward GEMM)
+    const float *UT;  // [H1p][n_qp]      transposed (K-major for the backward GEMM)
     const float *b1;  // [H1p]
     const float *W2;  // [H1p][H2p]
     const float *W2T; // [H2p][H1p]
@@ -128,12 +128,15 @@ void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, co
 struct DenseTile {
     int32_t species, start, count; // atoms sp_list[start .. start+count) all of `species`
 };
+int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const int32_t *qtab,
+                    const float *b, float *Q /* [N][nqp], rows in sp_list (tile) order */);
+int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
+                    const float *Qbar, float *bbar);
 int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w /*[S]*/,
-                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const int32_t *qtab, const float *b,
-                     float *z_stash, int zs, float *out /* c_ext[t+1] rows (stride nphip) or Ei (stride 1) */,
-                     int out_stride);
+                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash,
+                     int zs, float *out /* c_ext[t+1] rows (stride nphip) or Ei (stride 1) */, int out_stride);
 int launch_dense_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w,
-                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *b, const float *z_stash,
-                     int zs, const float *outbar /* cbar rows or NULL for the energy layer */, int outbar_stride,
-                     float *bbar);
+                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *z_stash, int zs,
+                     const float *outbar /* cbar rows or NULL for the energy layer */, int outbar_stride,
+                     float *Qbar /* [N][nqp], tile order */);
 #define DENSE_TM 64 // atoms per dense tile

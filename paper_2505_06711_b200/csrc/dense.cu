@@ -1,5 +1,6 @@
 // dense.cu -- rows A6+A7 (contraction, density, per-species MLP) and A9 (their reverse pass) of
-// SURVEY.md section 8(a), FP32 SIMT tile kernels (64 atoms of one species per CTA).
+// gram kernels (b <-> radial-pair products Q) and FP32 SIMT GEMM-chain tile
+// kernels (64 atoms of one species per CTA; the tcgen05 version of the chain lives in dense_tc.cu).
 //
 // Eq. 1 with the learned contraction (reading A-1):
 //     d[a,m] = sum_n Wc[l(a)][n][m] b[n,a],   rho[m] = sum_a mu_a d[a,m]^2
@@ -95,94 +96,144 @@ __device__ __forceinline__ void gemm_smemA(float (&acc)[4][NC], const float *__r
     }
 }
 
+
+// ============================================================================ gram kernels
+// Q[p][q] = sum_{|a|=l} mu_a b[n,a] b[n',a]  for q = (l, n <= n'), row p = position in sp_list (tile order).
+constexpr int GW = 4; // warps per block (warp per atom)
+
+__global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *__restrict__ sp_list,
+                                                      const int32_t *__restrict__ qtab, const float *__restrict__ b,
+                                                      float *__restrict__ Q, int NB, int Na, int nphip, int nqp) {
+    extern __shared__ __align__(16) float sm[];
+    const int NAP = Na | 1;                       // odd row stride: conflict-free over n'
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *bs = sm + (size_t)warp * nphip * NAP;
+    const int64_t p = (int64_t)blockIdx.x * GW + warp;
+    if (p >= N) return;
+    const int64_t atom = sp_list[p];
+    const float *bi = b + atom * NB;
+    for (int f = lane; f < NB; f += 32) bs[(f / Na) * NAP + (f % Na)] = __ldg(bi + f);
+    __syncwarp();
+    float *qo = Q + p * nqp;
+    for (int q = lane; q < nqp; q += 32) {
+        const int32_t e = __ldg(qtab + q);
+        const int n = e & 255, n2 = (e >> 8) & 255, a0 = (e >> 16) & 255, ac = (e >> 24) & 255;
+        const float *p1 = bs + n * NAP + a0, *p2 = bs + n2 * NAP + a0;
+        float qv = 0.f;
+        for (int a = 0; a < ac; ++a) qv = fmaf(c_mu[a0 + a] * p1[a], p2[a], qv);
+        qo[q] = qv;
+    }
+}
+
+// bbar[n,a] = mu_a sum_n' G_l(a)[n,n'] b[n',a],  G_l[n,n'] = Qbar[l, min, max] (1 + delta_nn')
+__global__ void __launch_bounds__(GW * 32) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
+                                                      const float *__restrict__ b, const float *__restrict__ Qbar,
+                                                      float *__restrict__ bbar, int NB, int Na, int nphi, int nphip,
+                                                      int NPp, int nqp) {
+    extern __shared__ __align__(16) float sm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *bs = sm + (size_t)warp * (NB + nqp), *qs = bs + NB;
+    const int64_t p = (int64_t)blockIdx.x * GW + warp;
+    if (p >= N) return;
+    const int64_t atom = sp_list[p];
+    const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
+    const float4 *qi = reinterpret_cast<const float4 *>(Qbar + p * nqp);
+    for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
+    for (int f = lane; f < nqp / 4; f += 32) reinterpret_cast<float4 *>(qs)[f] = __ldg(qi + f);
+    __syncwarp();
+    float *bo = bbar + atom * NB;
+    for (int o = lane; o < nphi * Na; o += 32) {
+        const int n = o / Na, a = o % Na;
+        const int l = (a >= 10) ? 3 : (a >= 4) ? 2 : (a >= 1) ? 1 : 0;
+        const float *ql = qs + l * NPp;
+        float s = 0.f;
+        for (int n2 = 0; n2 < nphi; ++n2) {
+            const int lo = min(n, n2), hi = max(n, n2);
+            float gq = ql[lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo)];
+            if (n == n2) gq *= 2.0f;
+            s = fmaf(gq, bs[n2 * Na + a], s);
+        }
+        bo[o] = c_mu[a] * s;
+    }
+    // rows n in [nphi, nphip) of bbar stay zero (buffer zero-initialised once)
+}
+
+// ============================================================================ GEMM-chain tile kernels (SIMT)
 struct FwdArgs {
     const DenseW *w;        // [S]
     const DenseTile *tiles;
     const int32_t *sp_list;
-    const int32_t *qtab;    // [nqp] packed n | n'<<8 | a0<<16 | acnt<<24 (acnt = 0: padding)
-    const float *b;         // [N][NB]
-    float *z_stash;         // [N][zs]
-    float *out;             // rows of stride out_stride
-    int out_stride, NB, NBP, Na, nqp, H1p, H2p, nout, zs;
+    const float *Q;         // [N][nqp], tile order
+    float *z_stash;         // [N][zs], tile order
+    float *out;             // rows of stride out_stride, atom order
+    int out_stride, nqp, H1p, H2p, nout, zs;
 };
 
-// ---------------------------------------------------------------------------------- forward
+// A chunk from row-major global rows -> K-major shared [KC][TM]
+__device__ __forceinline__ void load_a_chunk(float *__restrict__ As, const float *__restrict__ Ag, int ldg, int k0,
+                                             int kc, int rows_valid) {
+    // thread -> (row m = tid % TM, k-quad = tid / TM + 4 j): lanes run over m => conflict-free stores
+    const int m = threadIdx.x & (TM - 1);
+    for (int kq = threadIdx.x / TM; kq * 4 < kc; kq += DT / TM) {
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (m < rows_valid) v = __ldg(reinterpret_cast<const float4 *>(Ag + (size_t)m * ldg + k0) + kq);
+        As[(kq * 4 + 0) * TM + m] = v.x; As[(kq * 4 + 1) * TM + m] = v.y;
+        As[(kq * 4 + 2) * TM + m] = v.z; As[(kq * 4 + 3) * TM + m] = v.w;
+    }
+}
+
 template <int NC1, int NC2>
 __global__ void __launch_bounds__(DT) k_dense_fwd(FwdArgs A) {
     extern __shared__ __align__(16) float sm[];
     const DenseTile tile = A.tiles[blockIdx.x];
     const DenseW W = A.w[tile.species];
     const int tid = threadIdx.x, tm = tid >> 4, tn = tid & 15;
-    // shared-memory carve-up (floats): region R0 = max(TM*NBP, TM*(H1p+H2p)) holds the b rows, later
-    // the activations h1, h2 (K-major); then the Q chunk [KC][TM]; then the B-operand chunk.
-    const int R0 = max(TM * A.NBP, TM * (A.H1p + A.H2p));
-    float *bs = sm, *Qc = sm + R0, *Bs = Qc + KC * TM;
-    float *Hs = sm, *H2s = sm + TM * A.H1p;
+    // carve-up (floats): Ac [KC][TM] | Bs [KC][128] | Hs [H1p][TM] | H2s [H2p][TM]
+    float *Ac = sm, *Bs = Ac + KC * TM, *Hs = Bs + KC * 128, *H2s = Hs + A.H1p * TM;
     __shared__ int32_t atom_s[TM];
     if (tid < TM) atom_s[tid] = (tid < tile.count) ? A.sp_list[tile.start + tid] : -1;
-    __syncthreads();
-    // 1. gather the b rows of the tile
-    for (int idx = tid; idx < TM * (A.NB / 4); idx += DT) {
-        const int m = idx / (A.NB / 4), f4 = idx % (A.NB / 4);
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (atom_s[m] >= 0) v = __ldg(reinterpret_cast<const float4 *>(A.b + (size_t)atom_s[m] * A.NB) + f4);
-        float *d = bs + m * A.NBP + f4 * 4;
-        d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
-    }
-    // 2. z1 = U^T Q + b1, Q generated chunk by chunk from the b rows
+    const float *Qt = A.Q + (size_t)tile.start * A.nqp;
+    // 1. z1 = U^T Q + b1
     float acc1[4][NC1];
 #pragma unroll
     for (int r = 0; r < 4; ++r)
 #pragma unroll
         for (int c = 0; c < NC1; ++c) acc1[r][c] = 0.f;
     for (int q0 = 0; q0 < A.nqp; q0 += KC) {
+        const int kc = min(KC, A.nqp - q0);
         __syncthreads();
-        {   // Q chunk: thread -> atom m = tid % 64, q = q0 + tid/64 + 4 j
-            const int m = tid & (TM - 1);
-            const float *bm = bs + m * A.NBP;
-            for (int kq = tid / TM; kq < KC; kq += DT / TM) {
-                float qv = 0.f;
-                if (q0 + kq < A.nqp) {
-                    const int32_t e = __ldg(A.qtab + q0 + kq);
-                    const int n = e & 255, n2 = (e >> 8) & 255, a0 = (e >> 16) & 255, ac = (e >> 24) & 255;
-                    const float *p1 = bm + n * A.Na + a0, *p2 = bm + n2 * A.Na + a0;
-                    for (int a = 0; a < ac; ++a) qv = fmaf(c_mu[a0 + a] * p1[a], p2[a], qv);
-                }
-                Qc[kq * TM + m] = qv;
-            }
-        }
-        load_b_chunk<NC1>(Bs, W.U, A.H1p, q0, min(KC, A.nqp - q0), 0);
+        load_a_chunk(Ac, Qt, A.nqp, q0, kc, tile.count);
+        load_b_chunk<NC1>(Bs, W.U, A.H1p, q0, kc, 0);
         __syncthreads();
-        mm_chunk<NC1>(acc1, Qc, Bs, min(KC, A.nqp - q0), tm, tn);
+        mm_chunk<NC1>(acc1, Ac, Bs, kc, tm, tn);
     }
-    __syncthreads(); // all reads of bs done: region R0 is reused for h1 / h2
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int m = tm * 4 + r, atom = atom_s[m];
+        const int m = tm * 4 + r;
 #pragma unroll
         for (int c = 0; c < NC1; ++c) {
             const int n = col_of<NC1>(tn, c);
             const float z = acc1[r][c] + __ldg(W.b1 + n);
-            if (atom >= 0) A.z_stash[(size_t)atom * A.zs + n] = z;
+            if (m < tile.count) A.z_stash[(size_t)(tile.start + m) * A.zs + n] = z;
             Hs[n * TM + m] = silu_f(z);
         }
     }
-    // 3. z2 = W2^T h1 + b2
+    // 2. z2 = W2^T h1 + b2
     float acc2[4][NC2];
     gemm_smemA<NC2>(acc2, Hs, A.H1p, W.W2, A.H2p, 0, Bs, tm, tn);
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int m = tm * 4 + r, atom = atom_s[m];
+        const int m = tm * 4 + r;
 #pragma unroll
         for (int c = 0; c < NC2; ++c) {
             const int n = col_of<NC2>(tn, c);
             const float z = acc2[r][c] + __ldg(W.b2 + n);
-            if (atom >= 0) A.z_stash[(size_t)atom * A.zs + A.H1p + n] = z;
+            if (m < tile.count) A.z_stash[(size_t)(tile.start + m) * A.zs + A.H1p + n] = z;
             H2s[n * TM + m] = silu_f(z);
         }
     }
     __syncthreads();
-    // 4. out = W3^T h2 + b3   (nout = N_phi or 1)
+    // 3. out = W3^T h2 + b3   (nout = N_phi or 1)
     for (int idx = tid; idx < TM * A.nout; idx += DT) {
         const int m = idx & (TM - 1), o = idx / TM;
         float s = __ldg(W.b3 + o);
@@ -192,14 +243,13 @@ __global__ void __launch_bounds__(DT) k_dense_fwd(FwdArgs A) {
     }
 }
 
-// ---------------------------------------------------------------------------------- backward
 struct BwdArgs {
     const DenseW *w;
     const DenseTile *tiles;
     const int32_t *sp_list;
-    const float *b, *z_stash, *outbar; // outbar == nullptr: energy layer, outbar = 1
-    float *bbar;
-    int outbar_stride, NB, NBP, Na, nphi, L, npairs, NPp, H1p, H2p, nout, zs;
+    const float *z_stash, *outbar; // outbar == nullptr: energy layer, outbar = 1
+    float *Qbar;                   // [N][nqp], tile order
+    int outbar_stride, nqp, H1p, H2p, nout, zs;
 };
 
 template <int NC1, int NC2>
@@ -208,21 +258,11 @@ __global__ void __launch_bounds__(DT) k_dense_bwd(BwdArgs A) {
     const DenseTile tile = A.tiles[blockIdx.x];
     const DenseW W = A.w[tile.species];
     const int tid = threadIdx.x, tm = tid >> 4, tn = tid & 15;
-    // carve-up: bs [TM][NBP] | Z1s [H1p][TM] | X = max(Z2s [H2p][TM], Qb [TM][NPp+1]) | Bs [KC][128] | ob [TM][nout+1]
-    const int QLD = A.NPp + 1;
-    float *bs = sm, *Z1s = bs + TM * A.NBP, *X = Z1s + A.H1p * TM;
-    float *Bs = X + max(A.H2p * TM, TM * QLD), *ob = Bs + KC * 128;
-    float *Z2s = X, *Qb = X;
+    // carve-up: Z1s [H1p][TM] | Z2s [H2p][TM] | Bs [KC][128] | ob [TM][nout+1]
+    float *Z1s = sm, *Z2s = Z1s + A.H1p * TM, *Bs = Z2s + A.H2p * TM, *ob = Bs + KC * 128;
     __shared__ int32_t atom_s[TM];
     if (tid < TM) atom_s[tid] = (tid < tile.count) ? A.sp_list[tile.start + tid] : -1;
     __syncthreads();
-    for (int idx = tid; idx < TM * (A.NB / 4); idx += DT) {
-        const int m = idx / (A.NB / 4), f4 = idx % (A.NB / 4);
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (atom_s[m] >= 0) v = __ldg(reinterpret_cast<const float4 *>(A.b + (size_t)atom_s[m] * A.NB) + f4);
-        float *d = bs + m * A.NBP + f4 * 4;
-        d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
-    }
     const int OLD = A.nout + 1;
     for (int idx = tid; idx < TM * A.nout; idx += DT) {
         const int m = idx / A.nout, o = idx % A.nout;
@@ -235,10 +275,9 @@ __global__ void __launch_bounds__(DT) k_dense_bwd(BwdArgs A) {
     for (int idx = tid; idx < TM * A.H2p; idx += DT) {
         const int m = idx & (TM - 1), g = idx / TM;
         float s = 0.f;
-        const float *w3 = W.W3 + (size_t)g * A.nout; // [H2p][nout] row-major (unpadded nout)
+        const float *w3 = W.W3 + (size_t)g * A.nout;
         for (int o = 0; o < A.nout; ++o) s = fmaf(__ldg(w3 + o), ob[m * OLD + o], s);
-        const int atom = atom_s[m];
-        const float z2 = (atom >= 0) ? __ldg(A.z_stash + (size_t)atom * A.zs + A.H1p + g) : 0.f;
+        const float z2 = (m < tile.count) ? __ldg(A.z_stash + (size_t)(tile.start + m) * A.zs + A.H1p + g) : 0.f;
         Z2s[g * TM + m] = s * dsilu_f(z2);
     }
     // 2. z1bar = (W2 z2bar) * SiLU'(z1)  -> Z1s [h][m]      (B operand: W2T [H2p][H1p])
@@ -246,80 +285,55 @@ __global__ void __launch_bounds__(DT) k_dense_bwd(BwdArgs A) {
     gemm_smemA<NC1>(acc1, Z2s, A.H2p, W.W2T, A.H1p, 0, Bs, tm, tn);
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int m = tm * 4 + r, atom = atom_s[m];
+        const int m = tm * 4 + r;
 #pragma unroll
         for (int c = 0; c < NC1; ++c) {
             const int n = col_of<NC1>(tn, c);
-            const float z1 = (atom >= 0) ? __ldg(A.z_stash + (size_t)atom * A.zs + n) : 0.f;
+            const float z1 = (m < tile.count) ? __ldg(A.z_stash + (size_t)(tile.start + m) * A.zs + n) : 0.f;
             Z1s[n * TM + m] = acc1[r][c] * dsilu_f(z1);
         }
     }
-    // 3. per l: Qbar_l = z1bar . UT[l]  ([TM][NPp]) then bbar[n,a] = mu_a sum_n' G_l[n,n'] b[n',a]
-    for (int l = 0; l <= A.L; ++l) {
-        const float *UTl = W.UT + (size_t)l * A.H1p * A.NPp;
-        for (int col0 = 0; col0 < A.NPp;) {   // column blocks of 128 / 64 / 32 / 16
-            const int rem = A.NPp - col0;
-            if (rem >= 128) {
-                float acc[4][8];
-                gemm_smemA<8>(acc, Z1s, A.H1p, UTl, A.NPp, col0, Bs, tm, tn);
+    // 3. Qbar = z1bar . UT  ([TM][nqp]),  UT: [H1p][nqp] row-major; column blocks of 128 / 64 / 32 / 16
+    float *Qt = A.Qbar + (size_t)tile.start * A.nqp;
+    for (int col0 = 0; col0 < A.nqp;) {
+        const int rem = A.nqp - col0;
+        if (rem >= 128) {
+            float acc[4][8];
+            gemm_smemA<8>(acc, Z1s, A.H1p, W.UT, A.nqp, col0, Bs, tm, tn);
 #pragma unroll
-                for (int r = 0; r < 4; ++r)
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) Qb[(tm * 4 + r) * QLD + col0 + col_of<8>(tn, c)] = acc[r][c];
-                col0 += 128;
-            } else if (rem >= 64) {
-                float acc[4][4];
-                gemm_smemA<4>(acc, Z1s, A.H1p, UTl, A.NPp, col0, Bs, tm, tn);
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) Qb[(tm * 4 + r) * QLD + col0 + col_of<4>(tn, c)] = acc[r][c];
-                col0 += 64;
-            } else if (rem >= 32) {
-                float acc[4][2];
-                gemm_smemA<2>(acc, Z1s, A.H1p, UTl, A.NPp, col0, Bs, tm, tn);
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-#pragma unroll
-                    for (int c = 0; c < 2; ++c) Qb[(tm * 4 + r) * QLD + col0 + col_of<2>(tn, c)] = acc[r][c];
-                col0 += 32;
-            } else {
-                float acc[4][1];
-                gemm_smemA<1>(acc, Z1s, A.H1p, UTl, A.NPp, col0, Bs, tm, tn);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) Qb[(tm * 4 + r) * QLD + col0 + tn] = acc[r][0];
-                col0 += 16;
-            }
-        }
-        __syncthreads();
-        {   // thread -> atom m = tid % 64, rows n = tid/64 + 4 j
-            const int m = tid & (TM - 1), atom = atom_s[m];
-            const float *bm = bs + m * A.NBP, *qm = Qb + m * QLD;
-            const int a0 = l * (l + 1) * (l + 2) / 6, ac = (l + 1) * (l + 2) / 2;
-            for (int n = tid / TM; n < A.nphi; n += DT / TM) {
-                float s[10];
-#pragma unroll
-                for (int a = 0; a < 10; ++a) s[a] = 0.f;
-                for (int n2 = 0; n2 < A.nphi; ++n2) {
-                    const int lo = min(n, n2), hi = max(n, n2);
-                    float gq = qm[lo * A.nphi - (lo * (lo - 1)) / 2 + (hi - lo)];
-                    if (n == n2) gq *= 2.0f;
-                    const float *bp = bm + n2 * A.Na + a0;
-#pragma unroll
-                    for (int a = 0; a < 10; ++a)
-                        if (a < ac) s[a] = fmaf(gq, bp[a], s[a]);
+            for (int r = 0; r < 4; ++r)
+                if (tm * 4 + r < tile.count) {
+                    float *d = Qt + (size_t)(tm * 4 + r) * A.nqp + col0;
+                    *reinterpret_cast<float4 *>(d + tn * 4) = make_float4(acc[r][0], acc[r][1], acc[r][2], acc[r][3]);
+                    *reinterpret_cast<float4 *>(d + 64 + tn * 4) = make_float4(acc[r][4], acc[r][5], acc[r][6], acc[r][7]);
                 }
-                if (atom >= 0) {
-                    float *dst = A.bbar + (size_t)atom * A.NB + n * A.Na + a0;
+            col0 += 128;
+        } else if (rem >= 64) {
+            float acc[4][4];
+            gemm_smemA<4>(acc, Z1s, A.H1p, W.UT, A.nqp, col0, Bs, tm, tn);
 #pragma unroll
-                    for (int a = 0; a < 10; ++a)
-                        if (a < ac) dst[a] = c_mu[a0 + a] * s[a];
-                }
-            }
+            for (int r = 0; r < 4; ++r)
+                if (tm * 4 + r < tile.count)
+                    *reinterpret_cast<float4 *>(Qt + (size_t)(tm * 4 + r) * A.nqp + col0 + tn * 4) =
+                        make_float4(acc[r][0], acc[r][1], acc[r][2], acc[r][3]);
+            col0 += 64;
+        } else if (rem >= 32) {
+            float acc[4][2];
+            gemm_smemA<2>(acc, Z1s, A.H1p, W.UT, A.nqp, col0, Bs, tm, tn);
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+                if (tm * 4 + r < tile.count)
+                    *reinterpret_cast<float2 *>(Qt + (size_t)(tm * 4 + r) * A.nqp + col0 + tn * 2) = make_float2(acc[r][0], acc[r][1]);
+            col0 += 32;
+        } else {
+            float acc[4][1];
+            gemm_smemA<1>(acc, Z1s, A.H1p, W.UT, A.nqp, col0, Bs, tm, tn);
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+                if (tm * 4 + r < tile.count) Qt[(size_t)(tm * 4 + r) * A.nqp + col0 + tn] = acc[r][0];
+            col0 += 16;
         }
-        __syncthreads();
     }
-    // padded rows n in [nphi, nphip) of bbar stay zero (buffer is zero-initialised once)
 }
 
 template <int NC1, int NC2>
@@ -360,28 +374,41 @@ int run_bwd(const LaunchCtx &ctx, const BwdArgs &A, int n_tiles, size_t smem) {
 
 } // namespace
 
+int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const int32_t *qtab,
+                    const float *b, float *Q) {
+    if (N <= 0) return REANN_OK;
+    const size_t smem = sizeof(float) * GW * md.nphip * (md.Na | 1);
+    LAUNCH(ctx, k_gram_fwd, div_up(N, GW), GW * 32, smem, N, sp_list, qtab, b, Q, md.NB, md.Na, md.nphip, md.nqp);
+    return REANN_OK;
+}
+
+int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
+                    const float *Qbar, float *bbar) {
+    if (N <= 0) return REANN_OK;
+    const size_t smem = sizeof(float) * GW * (md.NB + md.nqp);
+    LAUNCH(ctx, k_gram_bwd, div_up(N, GW), GW * 32, smem, N, sp_list, b, Qbar, bbar, md.NB, md.Na, md.nphi, md.nphip,
+           md.NPp, md.nqp);
+    return REANN_OK;
+}
+
 int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w,
-                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const int32_t *qtab, const float *b,
-                     float *z_stash, int zs, float *out, int out_stride) {
+                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash, int zs,
+                     float *out, int out_stride) {
     if (n_tiles <= 0) return REANN_OK;
     FwdArgs A;
-    A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.qtab = qtab; A.b = b; A.z_stash = z_stash; A.out = out;
-    A.out_stride = out_stride; A.NB = md.NB; A.NBP = md.NB | 1; A.Na = md.Na; A.nqp = md.nqp; A.H1p = ld.H1p;
-    A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs;
-    const int R0 = std::max(TM * A.NBP, TM * (A.H1p + A.H2p));
-    const size_t smem = sizeof(float) * ((size_t)R0 + KC * TM + KC * 128);
+    A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.Q = Q; A.z_stash = z_stash; A.out = out;
+    A.out_stride = out_stride; A.nqp = md.nqp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs;
+    const size_t smem = sizeof(float) * ((size_t)KC * TM + KC * 128 + (size_t)TM * (A.H1p + A.H2p));
     NC_DISPATCH(run_fwd, ctx, A, n_tiles, smem)
 }
 
 int launch_dense_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w,
-                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *b, const float *z_stash,
-                     int zs, const float *outbar, int outbar_stride, float *bbar) {
+                     const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *z_stash, int zs,
+                     const float *outbar, int outbar_stride, float *Qbar) {
     if (n_tiles <= 0) return REANN_OK;
     BwdArgs A;
-    A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.b = b; A.z_stash = z_stash; A.outbar = outbar; A.bbar = bbar;
-    A.outbar_stride = outbar_stride; A.NB = md.NB; A.NBP = md.NB | 1; A.Na = md.Na; A.nphi = md.nphi; A.L = md.L;
-    A.npairs = md.npairs; A.NPp = md.NPp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs;
-    const size_t smem = sizeof(float) * ((size_t)TM * A.NBP + (size_t)A.H1p * TM +
-                                         std::max(A.H2p * TM, TM * (A.NPp + 1)) + KC * 128 + TM * (A.nout + 1));
+    A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.z_stash = z_stash; A.outbar = outbar; A.Qbar = Qbar;
+    A.outbar_stride = outbar_stride; A.nqp = md.nqp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs;
+    const size_t smem = sizeof(float) * ((size_t)TM * (A.H1p + A.H2p) + KC * 128 + TM * (A.nout + 1));
     NC_DISPATCH(run_bwd, ctx, A, n_tiles, smem)
 }

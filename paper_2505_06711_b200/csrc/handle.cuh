@@ -53,6 +53,7 @@ struct reann {
     DevBuf z_stash;               // float [T][N][zs]  (z1 | z2 pre-activations)
     int zs = 0;
     DevBuf bbar;                  // float [N][NB]
+    DevBuf Qbuf;                  // float [N][nqp] radial-pair products Q (forward) / Qbar (reverse), tile order
     DevBuf cbar;                  // float [N][nphip]
     DevBuf kappa;                 // float [cap_rc][nphip]
     DevBuf gst;                   // float4 [cap_rc]
