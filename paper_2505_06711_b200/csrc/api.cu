@@ -3,6 +3,7 @@
 // dense.cu, scan.cu. There is deliberately no CPU fallback: without a CUDA device every call fails.
 #include <math.h>
 #include <stdarg.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -50,7 +51,35 @@ static bool is_device_ptr(const void *p) {
     return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
-static int pad_pow2_16(int H) { int p = 16; while (p < H) p <<= 1; return p; }
+static int pad_pow2_32(int H) { int p = 32; while (p < H) p <<= 1; return p; }
+
+// x = hi + lo with hi rounded to TF32 (10 mantissa bits), lo = x - hi exact (same split as dense_tc.cu)
+static void split_tf32_host(float x, float *hi, float *lo) {
+    uint32_t u;
+    memcpy(&u, &x, 4);
+    u = (u + 0x1000u) & 0xFFFFE000u;
+    memcpy(hi, &u, 4);
+    *lo = x - *hi;                 // exact; then rounded to TF32 as well
+    memcpy(&u, lo, 4);
+    u = (u + 0x1000u) & 0xFFFFE000u;
+    memcpy(lo, &u, 4);
+}
+
+// Append the chunk images of a K-major operand B[n][k] (n < N, k < K, K % 32 == 0) in the shared-memory
+// layout of dense_tc.cu: per chunk of 32 k: hi image [k/4][n][k%4], then the lo image.
+template <class F>
+static size_t push_images(std::vector<float> &img, int N, int K, F Bnk) {
+    const size_t off = img.size();
+    img.resize(off + (size_t)2 * N * K, 0.f);
+    for (int kc = 0; kc < K / 32; ++kc) {
+        float *hi = img.data() + off + (size_t)kc * 2 * N * 32, *lo = hi + (size_t)N * 32;
+        for (int ki = 0; ki < 8; ++ki)
+            for (int n = 0; n < N; ++n)
+                for (int j = 0; j < 4; ++j)
+                    split_tf32_host(Bnk(n, kc * 32 + ki * 4 + j), &hi[((size_t)ki * N + n) * 4 + j], &lo[((size_t)ki * N + n) * 4 + j]);
+    }
+    return off;
+}
 
 // ---------------------------------------------------------------------------------------------
 // Blob parsing (layout: gen/weights.py) -- this side's own parser.
@@ -147,12 +176,17 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
     md.S = v.S; md.T = T; md.L = L; md.nphi = n_gauss; md.nphip = (n_gauss + 3) & ~3;
     md.Na = (L + 1) * (L + 2) * (L + 3) / 6; md.NB = md.nphip * md.Na; md.norb = v.norb;
     md.npairs = n_gauss * (n_gauss + 1) / 2; md.NPp = (md.npairs + 15) & ~15; md.nqp = (L + 1) * md.NPp;
+    md.K1 = (md.nqp + 31) & ~31;
+    {
+        const char *e = getenv("REANN_DENSE");
+        h->dense_tc = !(e && strcmp(e, "simt") == 0);
+    }
     md.rc = rc; md.skin = skin;
     h->zs = 0;
     for (int t = 0; t < T; ++t) {
         const bool last = t == T - 1;
-        h->ld[t].H1p = pad_pow2_16(last ? v.H1e : v.H1c);
-        h->ld[t].H2p = pad_pow2_16(last ? v.H2e : v.H2c);
+        h->ld[t].H1p = pad_pow2_32(last ? v.H1e : v.H1c);
+        h->ld[t].H2p = pad_pow2_32(last ? v.H2e : v.H2c);
         h->ld[t].nout = last ? 1 : n_gauss;
         h->ld[t].noutp = h->ld[t].nout;
         h->zs = std::max(h->zs, h->ld[t].H1p + h->ld[t].H2p);
@@ -243,6 +277,40 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         }
         CRC(dev_ensure(h, h->w_tab, sizeof(DenseW) * h->h_wtab.size()));
         CCU(cudaMemcpy(h->w_tab.p, h->h_wtab.data(), sizeof(DenseW) * h->h_wtab.size(), cudaMemcpyHostToDevice));
+        // tensor-core chunk images (dense_tc.cu): pre-split hi | lo TF32 operands
+        {
+            std::vector<float> img;
+            struct OffT { size_t g1, g2, g3, r1, r2, r3; };
+            std::vector<OffT> ot(offs.size());
+            for (int t = 0; t < T; ++t) {
+                const int H1p = h->ld[t].H1p, H2p = h->ld[t].H2p, nout = h->ld[t].nout;
+                for (int s = 0; s < md.S; ++s) {
+                    const Off &o = offs[(size_t)t * md.S + s];
+                    OffT &q = ot[(size_t)t * md.S + s];
+                    const float *A = all.data();
+                    auto Uqh = [&](int qq, int hh) { return qq < md.nqp ? A[o.U + (size_t)qq * H1p + hh] : 0.f; };
+                    q.g1 = push_images(img, H1p, md.K1, [&](int n, int k) { return Uqh(k, n); });
+                    q.g2 = push_images(img, H2p, H1p, [&](int n, int k) { return A[o.W2 + (size_t)k * H2p + n]; });
+                    q.g3 = push_images(img, 16, H2p, [&](int n, int k) { return n < nout ? A[o.W3 + (size_t)k * nout + n] : 0.f; });
+                    q.r1 = push_images(img, H2p, 32, [&](int n, int k) { return k < nout ? A[o.W3 + (size_t)n * nout + k] : 0.f; });
+                    q.r2 = push_images(img, H1p, H2p, [&](int n, int k) { return A[o.W2 + (size_t)n * H2p + k]; });
+                    q.r3 = img.size();
+                    for (int nb = 0; nb * 128 < md.K1; ++nb) {
+                        const int rows = std::min(128, md.K1 - nb * 128);
+                        push_images(img, rows, H1p, [&](int n, int k) { return Uqh(nb * 128 + n, k); });
+                    }
+                }
+            }
+            CRC(dev_ensure(h, h->wt_all, img.size() * 4));
+            CCU(cudaMemcpy(h->wt_all.p, img.data(), img.size() * 4, cudaMemcpyHostToDevice));
+            const float *ib = (const float *)h->wt_all.p;
+            std::vector<DenseWT> wt(offs.size());
+            for (size_t k = 0; k < offs.size(); ++k)
+                wt[k] = DenseWT{ib + ot[k].g1, ib + ot[k].g2, ib + ot[k].g3, ib + ot[k].r1, ib + ot[k].r2, ib + ot[k].r3,
+                                base + offs[k].b1, base + offs[k].b2, base + offs[k].b3};
+            CRC(dev_ensure(h, h->wt_tab, sizeof(DenseWT) * wt.size()));
+            CCU(cudaMemcpy(h->wt_tab.p, wt.data(), sizeof(DenseWT) * wt.size(), cudaMemcpyHostToDevice));
+        }
         // radial-pair table
         std::vector<int32_t> qtab((size_t)md.nqp, 0);
         for (int l = 0; l <= L; ++l) {
@@ -262,10 +330,11 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
     for (int64_t i = 0; i < n_atoms; ++i) h->species_count[(size_t)sp[(size_t)i]]++;
     {
         std::vector<DenseTile> tiles;
+        h->tile_rows = h->dense_tc ? DENSE_TC_TM : DENSE_TM;
         int64_t base = 0;
         for (int s = 0; s < md.S; ++s) {
-            for (int64_t o = 0; o < h->species_count[(size_t)s]; o += DENSE_TM)
-                tiles.push_back(DenseTile{s, (int32_t)(base + o), (int32_t)std::min<int64_t>(DENSE_TM, h->species_count[(size_t)s] - o)});
+            for (int64_t o = 0; o < h->species_count[(size_t)s]; o += h->tile_rows)
+                tiles.push_back(DenseTile{s, (int32_t)(base + o), (int32_t)std::min<int64_t>(h->tile_rows, h->species_count[(size_t)s] - o)});
             base += h->species_count[(size_t)s];
         }
         h->n_tiles = (int)tiles.size();
@@ -282,7 +351,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
 extern "C" void reann_destroy(reann_t *h) {
     if (!h) return;
     if (h->stream) cudaStreamSynchronize(h->stream); else cudaDeviceSynchronize();
-    DevBuf *bufs[] = {&h->w_all, &h->w_tab, &h->rcen, &h->alpha, &h->c0, &h->qtab, &h->species_caller, &h->tiles,
+    DevBuf *bufs[] = {&h->w_all, &h->w_tab, &h->wt_all, &h->wt_tab, &h->rcen, &h->alpha, &h->c0, &h->qtab, &h->species_caller, &h->tiles,
                       &h->pos_build, &h->wshift, &h->perm, &h->inv_perm, &h->xrec, &h->img_index, &h->cell_start,
                       &h->cell_rank, &h->row_ptr, &h->col, &h->rev, &h->sp_list, &h->scratch_a, &h->scratch_b,
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
@@ -356,7 +425,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->bbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.NB));
         CU(h, cudaMemsetAsync(h->bbar.p, 0, h->bbar.bytes, h->stream));       // padded rows stay 0
         RC(dev_ensure(h, h->cbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.nphip));
-        RC(dev_ensure(h, h->Qbuf, sizeof(float) * ((size_t)std::max<int64_t>(N, 1) + DENSE_TM * 2) * md.nqp));
+        RC(dev_ensure(h, h->Qbuf, sizeof(float) * ((size_t)std::max<int64_t>(N, 1) + DENSE_TC_TM * 2) * md.nqp));
         RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
@@ -470,6 +539,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
     const size_t cstride = (size_t)h->n_ext * md.nphip, bstride = (size_t)N * md.NB, zstride = (size_t)N * h->zs;
     float *c_ext = (float *)h->c_ext.p, *b = (float *)h->b.p, *zst = (float *)h->z_stash.p;
     const DenseW *wtab = (const DenseW *)h->w_tab.p;
+    const DenseWT *wttab = (const DenseWT *)h->wt_tab.p;
     for (int t = 0; t < md.T; ++t) {
         mk.mark(2);
         int rcode = launch_edge_fwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
@@ -480,9 +550,13 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         const bool last = t == md.T - 1;
         launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, (const int32_t *)h->qtab.p, b + t * bstride,
                         (float *)h->Qbuf.p);
-        rcode = launch_dense_fwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                 (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
-                                 last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip);
+        rcode = h->dense_tc
+                    ? launch_dense_tc_fwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                          (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
+                                          last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip)
+                    : launch_dense_fwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                       (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
+                                       last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip);
         if (rcode) return set_err(h, rcode, "dense forward: unsupported MLP shape or shared-memory size");
         if (!last) {
             mk.mark(4);
@@ -497,9 +571,13 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
     for (int t = md.T - 1; t >= 0; --t) {
         mk.mark(5);
         const bool last = t == md.T - 1;
-        int rcode = launch_dense_bwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                     (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
-                                     last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);
+        int rcode = h->dense_tc
+                        ? launch_dense_tc_bwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                              (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
+                                              last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p)
+                        : launch_dense_bwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                           (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
+                                           last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);
         if (rcode) return set_err(h, rcode, "dense backward: unsupported MLP shape or shared-memory size");
         launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, b + t * bstride, (const float *)h->Qbuf.p,
                         (float *)h->bbar.p);

@@ -55,6 +55,13 @@ struct DenseW {
     const float *b3;  // [noutp]
 };
 
+// Tensor-core path (dense_tc.cu): pre-split (hi | lo) TF32 weight chunk images, see dense_tc.cu.
+struct DenseWT {
+    const float *g1, *g2, *g3; // forward:  U^T chunks [K1/32], W2^T chunks [H1p/32], W3^T chunks [H2p/32] (N = 16)
+    const float *r1, *r2, *r3; // reverse:  W3 chunk (K = 32), W2 chunks [H2p/32], U blocks of <= 128 rows x [H1p/32]
+    const float *b1, *b2, *b3; // biases (FP32)
+};
+
 struct LayerDims {
     int H1p, H2p, nout, noutp;
 };
@@ -62,6 +69,7 @@ struct LayerDims {
 struct ModelDims {
     int S, T, L, nphi, nphip, Na, NB, norb;
     int npairs, NPp, nqp; // pairs n<=n' per l; padded to 16; (L+1)*NPp
+    int K1;               // nqp rounded up to 32 (K extent of the tensor-core GEMM over Q)
     double rc, skin;
 };
 
@@ -139,4 +147,13 @@ int launch_dense_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims 
                      const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *z_stash, int zs,
                      const float *outbar /* cbar rows or NULL for the energy layer */, int outbar_stride,
                      float *Qbar /* [N][nqp], tile order */);
-#define DENSE_TM 64 // atoms per dense tile
+#define DENSE_TM 64 // atoms per dense tile (SIMT path)
+
+// ---- dense_tc.cu (tcgen05 path; same contracts as the SIMT launchers, 128-atom tiles) ----
+#define DENSE_TC_TM 128
+int launch_dense_tc_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
+                        const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash,
+                        int zs, float *out, int out_stride);
+int launch_dense_tc_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
+                        const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *z_stash, int zs,
+                        const float *outbar, int outbar_stride, float *Qbar);

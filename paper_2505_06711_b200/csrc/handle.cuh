@@ -13,14 +13,16 @@ struct reann {
     // ---- model (device, FP32) ----
     DevBuf w_all;                 // every dense weight, one allocation
     DevBuf w_tab;                 // DenseW[T][S]
+    DevBuf wt_all, wt_tab;        // tensor-core weight images, DenseWT[T][S]
+    bool dense_tc = true;         // REANN_DENSE=simt selects the FP32 SIMT GEMM chain instead
     DevBuf rcen, alpha, c0;       // [T][S][nphip] (alpha pre-multiplied by log2(e)), [S][nphip]
     DevBuf qtab;                  // int32 [nqp] radial-pair table (dense.cu)
     std::vector<DenseW> h_wtab;   // host copy of the table (device pointers inside)
 
     // ---- atoms (device) ----
     DevBuf species_caller;        // int32 [N]
-    DevBuf tiles;                 // DenseTile[n_tiles]
-    int n_tiles = 0;
+    DevBuf tiles;                 // DenseTile[n_tiles]  (tiles of DENSE_TM or DENSE_TC_TM atoms)
+    int n_tiles = 0, tile_rows = 0;
     std::vector<int64_t> species_count;
 
     // ---- neighbour list, rebuilt on demand ----
