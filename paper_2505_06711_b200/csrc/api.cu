@@ -311,17 +311,6 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
             CRC(dev_ensure(h, h->wt_tab, sizeof(DenseWT) * wt.size()));
             CCU(cudaMemcpy(h->wt_tab.p, wt.data(), sizeof(DenseWT) * wt.size(), cudaMemcpyHostToDevice));
         }
-        // radial-pair table
-        std::vector<int32_t> qtab((size_t)md.nqp, 0);
-        for (int l = 0; l <= L; ++l) {
-            const int a0 = l * (l + 1) * (l + 2) / 6, ac = (l + 1) * (l + 2) / 2;
-            int pp = 0;
-            for (int n = 0; n < md.nphi; ++n)
-                for (int n2 = n; n2 < md.nphi; ++n2, ++pp)
-                    qtab[(size_t)l * md.NPp + pp] = n | (n2 << 8) | (a0 << 16) | (ac << 24);
-        }
-        CRC(dev_ensure(h, h->qtab, qtab.size() * 4));
-        CCU(cudaMemcpy(h->qtab.p, qtab.data(), qtab.size() * 4, cudaMemcpyHostToDevice));
     }
     // ---- atoms: species, dense tiles ----
     CRC(dev_ensure(h, h->species_caller, sizeof(int32_t) * (size_t)std::max<int64_t>(n_atoms, 1)));
@@ -351,7 +340,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
 extern "C" void reann_destroy(reann_t *h) {
     if (!h) return;
     if (h->stream) cudaStreamSynchronize(h->stream); else cudaDeviceSynchronize();
-    DevBuf *bufs[] = {&h->w_all, &h->w_tab, &h->wt_all, &h->wt_tab, &h->rcen, &h->alpha, &h->c0, &h->qtab, &h->species_caller, &h->tiles,
+    DevBuf *bufs[] = {&h->w_all, &h->w_tab, &h->wt_all, &h->wt_tab, &h->rcen, &h->alpha, &h->c0, &h->species_caller, &h->tiles,
                       &h->pos_build, &h->wshift, &h->perm, &h->inv_perm, &h->xrec, &h->img_index, &h->cell_start,
                       &h->cell_rank, &h->row_ptr, &h->col, &h->rev, &h->sp_list, &h->scratch_a, &h->scratch_b,
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
@@ -548,7 +537,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
         mk.mark(3);
         const bool last = t == md.T - 1;
-        launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, (const int32_t *)h->qtab.p, b + t * bstride,
+        launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, b + t * bstride,
                         (float *)h->Qbuf.p);
         rcode = h->dense_tc
                     ? launch_dense_tc_fwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,

@@ -132,12 +132,12 @@ void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, con
 void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
                    double dt, double acc_unit, int drift);
 
-// ---- dense.cu ----
+// ---- gram.cu / dense.cu ----
 struct DenseTile {
     int32_t species, start, count; // atoms sp_list[start .. start+count) all of `species`
 };
-int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const int32_t *qtab,
-                    const float *b, float *Q /* [N][nqp], rows in sp_list (tile) order */);
+int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
+                    float *Q /* [N][nqp], rows in sp_list (tile) order */);
 int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
                     const float *Qbar, float *bbar);
 int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w /*[S]*/,

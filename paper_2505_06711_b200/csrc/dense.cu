@@ -1,6 +1,6 @@
 // dense.cu -- rows A6+A7 (contraction, density, per-species MLP) and A9 (their reverse pass) of
-// gram kernels (b <-> radial-pair products Q) and FP32 SIMT GEMM-chain tile
-// kernels (64 atoms of one species per CTA; the tcgen05 version of the chain lives in dense_tc.cu).
+// FP32 SIMT GEMM-chain tile kernels (64 atoms of one species per CTA). The
+// gram kernels (b <-> radial-pair products Q) live in gram.cu, the tcgen05 chain in dense_tc.cu.
 //
 // Eq. 1 with the learned contraction (reading A-1):
 //     d[a,m] = sum_n Wc[l(a)][n][m] b[n,a],   rho[m] = sum_a mu_a d[a,m]^2
@@ -23,7 +23,6 @@ constexpr int DT = 256;      // threads per CTA: 16 (row groups of 4 atoms) x 16
 constexpr int KC = 32;       // K-chunk of the B operand staged in shared memory
 static_assert(TM == DENSE_TM, "tile size");
 
-__constant__ float c_mu[20] = {1, 1, 1, 1, 1, 2, 2, 1, 2, 1, 1, 3, 3, 3, 6, 3, 1, 3, 3, 1};
 
 __device__ __forceinline__ float silu_f(float z) { return z / (1.0f + __expf(-z)); }
 __device__ __forceinline__ float dsilu_f(float z) {
@@ -96,67 +95,6 @@ __device__ __forceinline__ void gemm_smemA(float (&acc)[4][NC], const float *__r
     }
 }
 
-
-// ============================================================================ gram kernels
-// Q[p][q] = sum_{|a|=l} mu_a b[n,a] b[n',a]  for q = (l, n <= n'), row p = position in sp_list (tile order).
-constexpr int GW = 4; // warps per block (warp per atom)
-
-__global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *__restrict__ sp_list,
-                                                      const int32_t *__restrict__ qtab, const float *__restrict__ b,
-                                                      float *__restrict__ Q, int NB, int Na, int nphip, int nqp) {
-    extern __shared__ __align__(16) float sm[];
-    const int NAP = Na | 1;                       // odd row stride: conflict-free over n'
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *bs = sm + (size_t)warp * nphip * NAP;
-    const int64_t p = (int64_t)blockIdx.x * GW + warp;
-    if (p >= N) return;
-    const int64_t atom = sp_list[p];
-    const float *bi = b + atom * NB;
-    for (int f = lane; f < NB; f += 32) bs[(f / Na) * NAP + (f % Na)] = __ldg(bi + f);
-    __syncwarp();
-    float *qo = Q + p * nqp;
-    for (int q = lane; q < nqp; q += 32) {
-        const int32_t e = __ldg(qtab + q);
-        const int n = e & 255, n2 = (e >> 8) & 255, a0 = (e >> 16) & 255, ac = (e >> 24) & 255;
-        const float *p1 = bs + n * NAP + a0, *p2 = bs + n2 * NAP + a0;
-        float qv = 0.f;
-        for (int a = 0; a < ac; ++a) qv = fmaf(c_mu[a0 + a] * p1[a], p2[a], qv);
-        qo[q] = qv;
-    }
-}
-
-// bbar[n,a] = mu_a sum_n' G_l(a)[n,n'] b[n',a],  G_l[n,n'] = Qbar[l, min, max] (1 + delta_nn')
-__global__ void __launch_bounds__(GW * 32) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
-                                                      const float *__restrict__ b, const float *__restrict__ Qbar,
-                                                      float *__restrict__ bbar, int NB, int Na, int nphi, int nphip,
-                                                      int NPp, int nqp) {
-    extern __shared__ __align__(16) float sm[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *bs = sm + (size_t)warp * (NB + nqp), *qs = bs + NB;
-    const int64_t p = (int64_t)blockIdx.x * GW + warp;
-    if (p >= N) return;
-    const int64_t atom = sp_list[p];
-    const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
-    const float4 *qi = reinterpret_cast<const float4 *>(Qbar + p * nqp);
-    for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
-    for (int f = lane; f < nqp / 4; f += 32) reinterpret_cast<float4 *>(qs)[f] = __ldg(qi + f);
-    __syncwarp();
-    float *bo = bbar + atom * NB;
-    for (int o = lane; o < nphi * Na; o += 32) {
-        const int n = o / Na, a = o % Na;
-        const int l = (a >= 10) ? 3 : (a >= 4) ? 2 : (a >= 1) ? 1 : 0;
-        const float *ql = qs + l * NPp;
-        float s = 0.f;
-        for (int n2 = 0; n2 < nphi; ++n2) {
-            const int lo = min(n, n2), hi = max(n, n2);
-            float gq = ql[lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo)];
-            if (n == n2) gq *= 2.0f;
-            s = fmaf(gq, bs[n2 * Na + a], s);
-        }
-        bo[o] = c_mu[a] * s;
-    }
-    // rows n in [nphi, nphip) of bbar stay zero (buffer zero-initialised once)
-}
 
 // ============================================================================ GEMM-chain tile kernels (SIMT)
 struct FwdArgs {
@@ -373,23 +311,6 @@ int run_bwd(const LaunchCtx &ctx, const BwdArgs &A, int n_tiles, size_t smem) {
     }
 
 } // namespace
-
-int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const int32_t *qtab,
-                    const float *b, float *Q) {
-    if (N <= 0) return REANN_OK;
-    const size_t smem = sizeof(float) * GW * md.nphip * (md.Na | 1);
-    LAUNCH(ctx, k_gram_fwd, div_up(N, GW), GW * 32, smem, N, sp_list, qtab, b, Q, md.NB, md.Na, md.nphip, md.nqp);
-    return REANN_OK;
-}
-
-int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
-                    const float *Qbar, float *bbar) {
-    if (N <= 0) return REANN_OK;
-    const size_t smem = sizeof(float) * GW * (md.NB + md.nqp);
-    LAUNCH(ctx, k_gram_bwd, div_up(N, GW), GW * 32, smem, N, sp_list, b, Qbar, bbar, md.NB, md.Na, md.nphi, md.nphip,
-           md.NPp, md.nqp);
-    return REANN_OK;
-}
 
 int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w,
                      const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash, int zs,

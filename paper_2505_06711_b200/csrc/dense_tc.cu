@@ -54,6 +54,18 @@ constexpr uint32_t COL_CORR = 128, COL_BUF = 256;
 // barrier slots (8 bytes each) in the barrier area
 enum { BAR_BFULL = 0, BAR_AFULL = 3, BAR_MMA = 6, BAR_ARES = 9, BAR_DFULL = 10, BAR_DEMPTY = 12, BAR_COUNT = 14 };
 
+// Optional timeline trace of one CTA (development aid, compiled only with -DREANN_TC_TRACE):
+// role 0 = control thread, 1 = row thread 0, 2 = first producer thread; slot k = clock64().
+#ifdef REANN_TC_TRACE
+__device__ long long g_tc_trace[3 * 128];
+#define TC_TRACE(role, k)                                                                             \
+    do {                                                                                              \
+        if (blockIdx.x == 200 && (k) < 128 && (threadIdx.x & 31) == 0) g_tc_trace[(role) * 128 + (k)] = clock64(); \
+    } while (0)
+#else
+#define TC_TRACE(role, k) ((void)0)
+#endif
+
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -231,6 +243,7 @@ __device__ __forceinline__ void drain_group(float *acc, uint32_t bar0, uint32_t 
     const int d = gg & 1;
     mbar_wait(bar0 + 8 * (BAR_DFULL + d), (uint32_t)((gg >> 1) & 1));
     tc_fence_after();
+    if (threadIdx.x == 0) TC_TRACE(1, 2 * gg);
 #pragma unroll
     for (int c = 0; c < NCH; ++c) {
         uint32_t vm[32], vc[32];
@@ -241,6 +254,7 @@ __device__ __forceinline__ void drain_group(float *acc, uint32_t bar0, uint32_t 
     }
     tc_fence_before();
     mbar_arrive(bar0 + 8 * (BAR_DEMPTY + d));
+    if (threadIdx.x == 0) TC_TRACE(1, 2 * gg + 1);
 }
 __device__ __forceinline__ void drain_group16(float *acc, uint32_t bar0, uint32_t tl, int gg) {
     const int d = gg & 1;
@@ -304,6 +318,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
     const DenseWT W = A.w[tile.species];
     const uint32_t bar0 = smem_u32(smem + SM_BAR);
     const uint32_t tmem = tc_prologue(smem, &tmem_base_s, FWD_CTL);
+    if (tid == 0) TC_TRACE(1, 103);
     const int n1 = A.K1 / KC, total = n1 + NCH1 + NCH2;
     const int ng1 = cdiv(n1, GK_Q);
     constexpr int ng2 = cdiv(NCH1, GK_H), ng3 = cdiv(NCH2, GK_H);
@@ -323,6 +338,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 if (i + 1 < total) { src = src_of(i + 1, nr); c.copy_b(i + 1, src, nr); }
                 const int s = i % NSTAGE;
                 mbar_wait(c.bar(BAR_AFULL + s), (uint32_t)((i / NSTAGE) & 1));
+                TC_TRACE(0, 2 * i);
                 if (i < n1) {
                     c.mma_chunk(i, s, H1p, i / GK_Q, i % GK_Q == 0, i % GK_Q == GK_Q - 1 || i == n1 - 1);
                 } else if (i < n1 + NCH1) {
@@ -332,6 +348,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                     const int kc = i - n1 - NCH1;
                     c.mma_chunk(i, s, 16, ng1 + ng2 + kc / GK_H, kc % GK_H == 0, kc % GK_H == GK_H - 1 || kc == NCH2 - 1);
                 }
+                TC_TRACE(0, 2 * i + 1);
             }
         }
     } else if (warp >= 4) {
@@ -351,7 +368,9 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                                         ? __ldg(reinterpret_cast<const float4 *>(Qt + (size_t)row * A.nqp + kg))
                                         : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
+            if (tid == 128) TC_TRACE(2, 3 * i);
             wait_stage_free(bar0, i);
+            if (tid == 128) TC_TRACE(2, 3 * i + 1);
 #pragma unroll
             for (int rb = 0; rb < 4; ++rb)
 #pragma unroll
@@ -361,6 +380,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 }
             fence_async_smem();
             mbar_arrive(bar0 + 8 * (BAR_AFULL + s));
+            if (tid == 128) TC_TRACE(2, 3 * i + 2);
         }
     } else {
         // ---- row threads ----
@@ -376,6 +396,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
 #pragma unroll 1
             for (int g = 0; g < ng1; ++g) drain_group<NCH1>(z1, bar0, tl, g);
             fwd_activate<NCH1>(z1, W.b1, zrow, valid, a_base, bar0, n1, m);
+            if (tid == 0) TC_TRACE(1, 100);
         }
         {
             float z2[H2p];
@@ -384,6 +405,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
 #pragma unroll 1
             for (int g = 0; g < ng2; ++g) drain_group<NCH2>(z2, bar0, tl, ng1 + g);
             fwd_activate<NCH2>(z2, W.b2, zrow + H1p, valid, a_base, bar0, n1 + NCH1, m);
+            if (tid == 0) TC_TRACE(1, 101);
         }
         float o[16];
 #pragma unroll
@@ -397,6 +419,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 if (c < A.nout) dst[c] = o[c] + __ldg(W.b3 + c);
         }
     }
+    if (tid == 0) TC_TRACE(1, 102);
     tc_epilogue(tmem, FWD_CTL);
 }
 
@@ -588,6 +611,12 @@ int run_tc_bwd(const LaunchCtx &ctx, const TcBwdArgs &A, int n_tiles) {
     }
 
 } // namespace
+
+#ifdef REANN_TC_TRACE
+extern "C" int reann_debug_tc_trace(long long *out) {
+    return (int)cudaMemcpyFromSymbol(out, g_tc_trace, sizeof(g_tc_trace));
+}
+#endif
 
 int launch_dense_tc_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
                         const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash,

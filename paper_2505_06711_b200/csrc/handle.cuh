@@ -16,7 +16,6 @@ struct reann {
     DevBuf wt_all, wt_tab;        // tensor-core weight images, DenseWT[T][S]
     bool dense_tc = true;         // REANN_DENSE=simt selects the FP32 SIMT GEMM chain instead
     DevBuf rcen, alpha, c0;       // [T][S][nphip] (alpha pre-multiplied by log2(e)), [S][nphip]
-    DevBuf qtab;                  // int32 [nqp] radial-pair table (dense.cu)
     std::vector<DenseW> h_wtab;   // host copy of the table (device pointers inside)
 
     // ---- atoms (device) ----
