@@ -217,7 +217,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
     {
         std::vector<float> all;
         auto reserve = [&](size_t n) { size_t o = all.size(); all.resize(o + ((n + 3) & ~(size_t)3), 0.f); return o; };
-        struct Off { size_t U, UT, b1, W2, W2T, b2, W3, W3T, b3; };
+        struct Off { size_t U, UT, b1, W2, W2T, b2, W3, W3T, b3, W3p, W3c0; };
         std::vector<Off> offs((size_t)T * md.S);
         std::vector<double> Vq((size_t)v.norb);
         for (int t = 0; t < T; ++t) {
@@ -231,6 +231,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
                 o.b1 = reserve(H1p); o.W2 = reserve((size_t)H1p * H2p); o.W2T = reserve((size_t)H2p * H1p);
                 o.b2 = reserve(H2p); o.W3 = reserve((size_t)H2p * nout); o.W3T = reserve((size_t)nout * H2p);
                 o.b3 = reserve(nout);
+                o.W3p = reserve((size_t)H2p * 16); o.W3c0 = reserve(H2p);   // tensor-core path: ALU GEMM over W3
                 offs[(size_t)k] = o;
                 const double *W1 = v.W1[(size_t)k];
                 for (int l = 0; l <= L; ++l) {
@@ -262,6 +263,8 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
                         const float w = (float)v.W3[(size_t)k][(size_t)b * nout + c];
                         all[o.W3 + (size_t)b * nout + c] = w;
                         all[o.W3T + (size_t)c * H2p + b] = w;
+                        if (c < 16) all[o.W3p + (size_t)b * 16 + c] = w;
+                        if (c == 0) all[o.W3c0 + b] = w;
                     }
                 for (int c = 0; c < nout; ++c) all[o.b3 + c] = (float)v.b3[(size_t)k][c];
             }
@@ -280,7 +283,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         // tensor-core chunk images (dense_tc.cu): pre-split hi | lo TF32 operands
         {
             std::vector<float> img;
-            struct OffT { size_t g1, g2, g3, r1, r2, r3; };
+            struct OffT { size_t g1, g2, r2, r3; };
             std::vector<OffT> ot(offs.size());
             for (int t = 0; t < T; ++t) {
                 const int H1p = h->ld[t].H1p, H2p = h->ld[t].H2p, nout = h->ld[t].nout;
@@ -291,8 +294,6 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
                     auto Uqh = [&](int qq, int hh) { return qq < md.nqp ? A[o.U + (size_t)qq * H1p + hh] : 0.f; };
                     q.g1 = push_images(img, H1p, md.K1, [&](int n, int k) { return Uqh(k, n); });
                     q.g2 = push_images(img, H2p, H1p, [&](int n, int k) { return A[o.W2 + (size_t)k * H2p + n]; });
-                    q.g3 = push_images(img, 16, H2p, [&](int n, int k) { return n < nout ? A[o.W3 + (size_t)k * nout + n] : 0.f; });
-                    q.r1 = push_images(img, H2p, 32, [&](int n, int k) { return k < nout ? A[o.W3 + (size_t)n * nout + k] : 0.f; });
                     q.r2 = push_images(img, H1p, H2p, [&](int n, int k) { return A[o.W2 + (size_t)n * H2p + k]; });
                     q.r3 = img.size();
                     for (int nb = 0; nb * 128 < md.K1; ++nb) {
@@ -306,8 +307,8 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
             const float *ib = (const float *)h->wt_all.p;
             std::vector<DenseWT> wt(offs.size());
             for (size_t k = 0; k < offs.size(); ++k)
-                wt[k] = DenseWT{ib + ot[k].g1, ib + ot[k].g2, ib + ot[k].g3, ib + ot[k].r1, ib + ot[k].r2, ib + ot[k].r3,
-                                base + offs[k].b1, base + offs[k].b2, base + offs[k].b3};
+                wt[k] = DenseWT{ib + ot[k].g1, ib + ot[k].g2, ib + ot[k].r2, ib + ot[k].r3,
+                                base + offs[k].b1, base + offs[k].b2, base + offs[k].b3, base + offs[k].W3p, base + offs[k].W3c0};
             CRC(dev_ensure(h, h->wt_tab, sizeof(DenseWT) * wt.size()));
             CCU(cudaMemcpy(h->wt_tab.p, wt.data(), sizeof(DenseWT) * wt.size(), cudaMemcpyHostToDevice));
         }
@@ -410,11 +411,14 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
     }
     if (!h->b.p) {
         RC(dev_ensure(h, h->b, sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(N, 1) * md.NB));
-        RC(dev_ensure(h, h->z_stash, sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(N, 1) * h->zs));
+        // dense rows: tensor-core path = 128-row tiles (tile-quad layout, dense_tc.cu), SIMT path = sp_list rows
+        const size_t rows = h->dense_tc ? (size_t)std::max(h->n_tiles, 1) * DENSE_TC_TM : (size_t)std::max<int64_t>(N, 1);
+        RC(dev_ensure(h, h->z_stash, sizeof(float) * (size_t)md.T * rows * h->zs));
         RC(dev_ensure(h, h->bbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.NB));
         CU(h, cudaMemsetAsync(h->bbar.p, 0, h->bbar.bytes, h->stream));       // padded rows stay 0
         RC(dev_ensure(h, h->cbar, sizeof(float) * (size_t)std::max<int64_t>(N, 1) * md.nphip));
-        RC(dev_ensure(h, h->Qbuf, sizeof(float) * ((size_t)std::max<int64_t>(N, 1) + DENSE_TC_TM * 2) * md.nqp));
+        RC(dev_ensure(h, h->Qbuf, sizeof(float) * rows * md.K1));
+        CU(h, cudaMemsetAsync(h->Qbuf.p, 0, h->Qbuf.bytes, h->stream));       // padding rows of ragged tiles stay finite
         RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
@@ -525,10 +529,11 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
                        (const int64_t *)h->rc_ptr.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
 
     // ---- forward: T layers (Eq. 1, Eq. 2) ----
-    const size_t cstride = (size_t)h->n_ext * md.nphip, bstride = (size_t)N * md.NB, zstride = (size_t)N * h->zs;
+    const size_t cstride = (size_t)h->n_ext * md.nphip, bstride = (size_t)N * md.NB, zstride = (h->dense_tc ? (size_t)h->n_tiles * DENSE_TC_TM : (size_t)N) * h->zs;
     float *c_ext = (float *)h->c_ext.p, *b = (float *)h->b.p, *zst = (float *)h->z_stash.p;
     const DenseW *wtab = (const DenseW *)h->w_tab.p;
     const DenseWT *wttab = (const DenseWT *)h->wt_tab.p;
+    const DenseTile *gram_tiles = h->dense_tc ? (const DenseTile *)h->tiles.p : nullptr;
     for (int t = 0; t < md.T; ++t) {
         mk.mark(2);
         int rcode = launch_edge_fwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
@@ -537,7 +542,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
         mk.mark(3);
         const bool last = t == md.T - 1;
-        launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, b + t * bstride,
+        launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, gram_tiles, h->n_tiles, b + t * bstride,
                         (float *)h->Qbuf.p);
         rcode = h->dense_tc
                     ? launch_dense_tc_fwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
@@ -568,7 +573,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
                                            (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
                                            last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);
         if (rcode) return set_err(h, rcode, "dense backward: unsupported MLP shape or shared-memory size");
-        launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, b + t * bstride, (const float *)h->Qbuf.p,
+        launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, gram_tiles, h->n_tiles, b + t * bstride, (const float *)h->Qbuf.p,
                         (float *)h->bbar.p);
         mk.mark(6);
         rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,

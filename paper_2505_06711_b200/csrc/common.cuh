@@ -57,9 +57,11 @@ struct DenseW {
 
 // Tensor-core path (dense_tc.cu): pre-split (hi | lo) TF32 weight chunk images, see dense_tc.cu.
 struct DenseWT {
-    const float *g1, *g2, *g3; // forward:  U^T chunks [K1/32], W2^T chunks [H1p/32], W3^T chunks [H2p/32] (N = 16)
-    const float *r1, *r2, *r3; // reverse:  W3 chunk (K = 32), W2 chunks [H2p/32], U blocks of <= 128 rows x [H1p/32]
+    const float *g1, *g2;      // forward:  U^T chunks [K1/32], W2^T chunks [H1p/32]
+    const float *r2, *r3;      // reverse:  W2 chunks [H2p/32], U blocks of <= 128 rows x [H1p/32]
     const float *b1, *b2, *b3; // biases (FP32)
+    const float *w3p;          // FP32 [H2p][16]: W3 rows zero-padded to 16 outputs (ALU GEMM with n_out <= 16)
+    const float *w3c0;         // FP32 [H2p]: first column of W3 (energy layer, n_out = 1)
 };
 
 struct LayerDims {
@@ -136,10 +138,12 @@ void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, co
 struct DenseTile {
     int32_t species, start, count; // atoms sp_list[start .. start+count) all of `species`
 };
-int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
-                    float *Q /* [N][nqp], rows in sp_list (tile) order */);
-int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
-                    const float *Qbar, float *bbar);
+// tiles != nullptr: Q / Qbar in the tile-quad layout of dense_tc.cu (K1 columns, 128-row tiles);
+// tiles == nullptr: row-major [N][nqp] rows in sp_list order (SIMT path)
+int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const DenseTile *tiles,
+                    int n_tiles, const float *b, float *Q);
+int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const DenseTile *tiles,
+                    int n_tiles, const float *b, const float *Qbar, float *bbar);
 int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseW *d_w /*[S]*/,
                      const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash,
                      int zs, float *out /* c_ext[t+1] rows (stride nphip) or Ei (stride 1) */, int out_stride);

@@ -2,16 +2,18 @@
 // of Eq. 1 in its radial-pair form (see dense.cu for the algebra)
 //     forward   Q[l, n<=n'] = sum_{|a|=l} mu_a b[n,a] b[n',a]
 //     reverse   bbar[n,a]   = mu_a sum_n' G_l(a)[n,n'] b[n',a],   G_l[n,n'] = Qbar[l,min,max] (1 + delta_nn')
-// Both are HBM-bound streaming kernels: a warp owns one atom at a time (grid-stride), stages its
-// b row (and Qbar row) in shared memory with coalesced float4 loads and writes coalesced rows.
-// Q / Qbar rows are in tile order (row p belongs to atom sp_list[p]), row stride nqp,
-// column l * NPp + pair(n, n'), pair(n, n') = n nphi - n (n - 1) / 2 + (n' - n).
+// Both are HBM-bound streaming kernels: a block owns 8 consecutive rows of Q / Qbar, one warp per
+// row (= atom); b rows are staged with coalesced float4 loads and Q rows go through shared memory so
+// that the block reads / writes them in full 128-byte lines in either of the two layouts:
+//   tile-quad (tensor-core path, see dense_tc.cu): [tile][q/4][128 rows][4], KQ = K1 columns;
+//   row-major (SIMT path, dense.cu):               [p][KQ = nqp], row p belongs to atom sp_list[p].
+// Column q = l * NPp + pair(n, n'), pair(n, n') = n nphi - n (n - 1) / 2 + (n' - n); columns that
+// are padding are written as zeros.
 #include "common.cuh"
 
 namespace {
 
-constexpr int GW = 8;           // warps per block
-constexpr int GRID_PER_SM = 6;  // resident blocks per SM the grid is sized for
+constexpr int GW = 8;           // warps (= rows) per block
 
 __host__ __device__ constexpr float mu_of(int a) { // l! / (lx! ly! lz!) in the graded monomial order of edge.cu
     return (a == 5 || a == 6 || a == 8) ? 2.f
@@ -41,48 +43,82 @@ __device__ __forceinline__ void load_row(const float *__restrict__ src, float *x
     }
 }
 
+// row of this warp: tile-quad mode (tiles != nullptr): block = (tile, group of 8 rows); else p = 8 block + warp
+struct RowId {
+    int64_t p;      // position in sp_list, -1 if the row is padding
+    int tile, r0;   // tile-quad mode: tile index, first row of the block's group
+};
+__device__ __forceinline__ RowId row_of_block(const DenseTile *__restrict__ tiles, int64_t N, int warp) {
+    RowId r;
+    if (tiles) {
+        r.tile = blockIdx.x >> 4; r.r0 = (blockIdx.x & 15) * 8;
+        const DenseTile t = tiles[r.tile];
+        r.p = (r.r0 + warp < t.count) ? (int64_t)t.start + r.r0 + warp : -1;
+    } else {
+        r.tile = 0; r.r0 = 0;
+        r.p = (int64_t)blockIdx.x * GW + warp;
+        if (r.p >= N) r.p = -1;
+    }
+    return r;
+}
+// float4 index in global memory of (row r8 of this block, column quad q4)
+__device__ __forceinline__ int64_t quad_index(const DenseTile *tiles, const RowId &r, int r8, int q4, int KQ) {
+    if (tiles) return ((int64_t)r.tile * (KQ >> 2) + q4) * DENSE_TC_TM + r.r0 + r8;
+    return ((int64_t)blockIdx.x * GW + r8) * (KQ >> 2) + q4;
+}
+
 // ---------------------------------------------------------------------------------------- forward
 template <int NPHIP, int NA>
 __global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *__restrict__ sp_list,
+                                                      const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, float *__restrict__ Q, int nphi,
-                                                      int npairs, int NPp, int nqp) {
+                                                      int npairs, int NPp, int KQ) {
     constexpr int NB = NPHIP * NA, JMAX = (NPHIP * (NPHIP + 1) / 2 + 31) / 32, LMAX = l_of(NA - 1);
-    __shared__ __align__(16) float bs_all[GW][NB];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *bs = bs_all[warp];
-    // this lane's pairs: pair index lane + 32 j -> (n, n') with n <= n'
-    int pn[JMAX], pn2[JMAX];
-#pragma unroll
-    for (int j = 0; j < JMAX; ++j) {
-        int pi = lane + 32 * j, lo = 0;
-        while (lo < nphi && pi >= nphi - lo) { pi -= nphi - lo; ++lo; }
-        pn[j] = lo; pn2[j] = lo + pi;           // lo == nphi: beyond the last pair (padding column)
-    }
-    for (int64_t p = (int64_t)blockIdx.x * GW + warp; p < N; p += (int64_t)gridDim.x * GW) {
-        const float4 *bi = reinterpret_cast<const float4 *>(b + (int64_t)sp_list[p] * NB);
+    extern __shared__ __align__(16) float sm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, QS = KQ + 4;
+    float *bs = sm + warp * NB, *qs = sm + GW * NB + warp * QS;
+    const RowId row = row_of_block(tiles, N, warp);
+    for (int f = lane; f < KQ / 4; f += 32) reinterpret_cast<float4 *>(qs)[f] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (row.p >= 0) {
+        const float4 *bi = reinterpret_cast<const float4 *>(b + (int64_t)sp_list[row.p] * NB);
 #pragma unroll
         for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
         __syncwarp();
-        float *qo = Q + p * nqp;
 #pragma unroll
         for (int j = 0; j < JMAX; ++j) {
-            const int pi = lane + 32 * j;
-            if (pi < NPp) {
-                float s[LMAX + 1];
+            int pi = lane + 32 * j;
+            if (pi < npairs) {
+                // pair index -> (n, n') with n <= n'
+                int lo = 0, rem = pi;
+                while (rem >= nphi - lo) { rem -= nphi - lo; ++lo; }
+                float x[NA], y[NA], s[LMAX + 1];
+                load_row<NA>(bs + lo * NA, x);
+                load_row<NA>(bs + (lo + rem) * NA, y);
 #pragma unroll
                 for (int l = 0; l <= LMAX; ++l) s[l] = 0.f;
-                if (pi < npairs) {
-                    float x[NA], y[NA];
-                    load_row<NA>(bs + pn[j] * NA, x);
-                    load_row<NA>(bs + pn2[j] * NA, y);
 #pragma unroll
-                    for (int a = 0; a < NA; ++a) s[l_of(a)] = fmaf(mu_of(a) * x[a], y[a], s[l_of(a)]);
-                }
+                for (int a = 0; a < NA; ++a) s[l_of(a)] = fmaf(mu_of(a) * x[a], y[a], s[l_of(a)]);
 #pragma unroll
-                for (int l = 0; l <= LMAX; ++l) qo[l * NPp + pi] = s[l];
+                for (int l = 0; l <= LMAX; ++l) qs[l * NPp + pi] = s[l];
             }
         }
-        __syncwarp();
+    }
+    __syncthreads();
+    if (!tiles && (int64_t)blockIdx.x * GW >= N) return;
+    const float *q0 = sm + GW * NB;
+    float4 *Q4 = reinterpret_cast<float4 *>(Q);
+    const int nq4 = KQ >> 2;
+    if (tiles) {
+        for (int idx = threadIdx.x; idx < GW * nq4; idx += GW * 32) {
+            const int q4 = idx >> 3, r8 = idx & 7;
+            Q4[quad_index(tiles, row, r8, q4, KQ)] = *reinterpret_cast<const float4 *>(q0 + r8 * QS + q4 * 4);
+        }
+    } else {
+        for (int idx = threadIdx.x; idx < GW * nq4; idx += GW * 32) {
+            const int r8 = idx / nq4, q4 = idx - r8 * nq4;
+            if ((int64_t)blockIdx.x * GW + r8 < N)
+                Q4[quad_index(tiles, row, r8, q4, KQ)] = *reinterpret_cast<const float4 *>(q0 + r8 * QS + q4 * 4);
+        }
     }
 }
 
@@ -92,34 +128,42 @@ struct BwdCfg {
     static constexpr int PARTS = NPHIP == 4 ? 8 : NPHIP == 8 ? 4 : 2; // lanes per row n
     static constexpr int CNT = (NA + PARTS - 1) / PARTS;              // monomials per lane
     static constexpr int TS = NPHIP + 4;                              // row stride of the transposed b
+    static constexpr int PER_WARP = NA * TS + NPHIP * NA;             // floats: bT | outs
 };
 
 template <int NPHIP, int NA>
 __global__ void __launch_bounds__(GW * 32) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
+                                                      const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, const float *__restrict__ Qbar,
-                                                      float *__restrict__ bbar, int nphi, int NPp, int nqp) {
+                                                      float *__restrict__ bbar, int nphi, int NPp, int KQ) {
     using C = BwdCfg<NPHIP, NA>;
     constexpr int NB = NPHIP * NA;
     extern __shared__ __align__(16) float sm[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int per_warp = NA * C::TS + NB + nqp;
-    float *bT = sm + (size_t)warp * per_warp, *outs = bT + NA * C::TS, *qs = outs + NB;
-    const int n = lane / C::PARTS, a0 = (lane % C::PARTS) * C::CNT;
-    const bool row_ok = n < nphi;
-    // triangular offsets of G[n, k] and the (1 + delta) factor; 0 for padded rows / columns
-    int idx[NPHIP];
-    float fac[NPHIP];
-#pragma unroll
-    for (int k = 0; k < NPHIP; ++k) {
-        const int lo = min(n, k), hi = max(n, k);
-        const bool ok = row_ok && k < nphi;
-        idx[k] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
-        fac[k] = ok ? (k == n ? 2.0f : 1.0f) : 0.0f;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, QS = KQ + 4;
+    float *bT = sm + warp * C::PER_WARP, *outs = bT + NA * C::TS, *q0 = sm + GW * C::PER_WARP, *qs = q0 + warp * QS;
+    const RowId row = row_of_block(tiles, N, warp);
+    if (!tiles && (int64_t)blockIdx.x * GW >= N) return;
+    // ---- block: the 8 Qbar rows, full lines ----
+    {
+        const float4 *Q4 = reinterpret_cast<const float4 *>(Qbar);
+        const int nq4 = KQ >> 2;
+        if (tiles) {
+            for (int idx = threadIdx.x; idx < GW * nq4; idx += GW * 32) {
+                const int q4 = idx >> 3, r8 = idx & 7;
+                *reinterpret_cast<float4 *>(q0 + r8 * QS + q4 * 4) = __ldg(Q4 + quad_index(tiles, row, r8, q4, KQ));
+            }
+        } else {
+            for (int idx = threadIdx.x; idx < GW * nq4; idx += GW * 32) {
+                const int r8 = idx / nq4, q4 = idx - r8 * nq4;
+                if ((int64_t)blockIdx.x * GW + r8 < N)
+                    *reinterpret_cast<float4 *>(q0 + r8 * QS + q4 * 4) = __ldg(Q4 + quad_index(tiles, row, r8, q4, KQ));
+            }
+        }
     }
-    for (int64_t p = (int64_t)blockIdx.x * GW + warp; p < N; p += (int64_t)gridDim.x * GW) {
-        const int64_t atom = sp_list[p];
+    int64_t atom = 0;
+    if (row.p >= 0) {
+        atom = sp_list[row.p];
         const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
-        const float4 *qi = reinterpret_cast<const float4 *>(Qbar + p * nqp);
 #pragma unroll
         for (int f = lane; f < NB / 4; f += 32) {
             const float4 v = __ldg(bi + f);
@@ -130,68 +174,84 @@ __global__ void __launch_bounds__(GW * 32) k_gram_bwd(int64_t N, const int32_t *
                 bT[(e % NA) * C::TS + e / NA] = va[u];
             }
         }
-        for (int f = lane; f < nqp / 4; f += 32) reinterpret_cast<float4 *>(qs)[f] = __ldg(qi + f);
-        __syncwarp();
-        if (n < NPHIP) {
-            float G[NPHIP];
-            int lcur = -1;
+    }
+    __syncthreads();
+    if (row.p < 0) return;
+    const int n = lane / C::PARTS, a0 = (lane % C::PARTS) * C::CNT;
+    if (n < NPHIP) {
+        // triangular offsets of G[n, k] and the (1 + delta) factor; 0 for padded rows / columns
+        int idx[NPHIP];
+        float fac[NPHIP];
 #pragma unroll
-            for (int ai = 0; ai < C::CNT; ++ai) {
-                const int a = a0 + ai;
-                if (a < NA) {
-                    const int l = l_of(a);
-                    if (l != lcur) {
-                        const float *ql = qs + l * NPp;
+        for (int k = 0; k < NPHIP; ++k) {
+            const int lo = min(n, k), hi = max(n, k);
+            const bool ok = n < nphi && k < nphi;
+            idx[k] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
+            fac[k] = ok ? (k == n ? 2.0f : 1.0f) : 0.0f;
+        }
+        float G[NPHIP];
+        int lcur = -1;
 #pragma unroll
-                        for (int k = 0; k < NPHIP; ++k) G[k] = ql[idx[k]] * fac[k];
-                        lcur = l;
-                    }
-                    float s = 0.f;
+        for (int ai = 0; ai < C::CNT; ++ai) {
+            const int a = a0 + ai;
+            if (a < NA) {
+                const int l = l_of(a);
+                if (l != lcur) {
+                    const float *ql = qs + l * NPp;
 #pragma unroll
-                    for (int k4 = 0; k4 < NPHIP / 4; ++k4) {
-                        const float4 v = *reinterpret_cast<const float4 *>(bT + a * C::TS + 4 * k4);
-                        s = fmaf(G[4 * k4], v.x, s); s = fmaf(G[4 * k4 + 1], v.y, s);
-                        s = fmaf(G[4 * k4 + 2], v.z, s); s = fmaf(G[4 * k4 + 3], v.w, s);
-                    }
-                    outs[n * NA + a] = c_mu[a] * s;
+                    for (int k = 0; k < NPHIP; ++k) G[k] = ql[idx[k]] * fac[k];
+                    lcur = l;
                 }
+                float s = 0.f;
+#pragma unroll
+                for (int k4 = 0; k4 < NPHIP / 4; ++k4) {
+                    const float4 v = *reinterpret_cast<const float4 *>(bT + a * C::TS + 4 * k4);
+                    s = fmaf(G[4 * k4], v.x, s); s = fmaf(G[4 * k4 + 1], v.y, s);
+                    s = fmaf(G[4 * k4 + 2], v.z, s); s = fmaf(G[4 * k4 + 3], v.w, s);
+                }
+                outs[n * NA + a] = c_mu[a] * s;
             }
         }
-        __syncwarp();
-        float4 *bo = reinterpret_cast<float4 *>(bbar + atom * NB);
-#pragma unroll
-        for (int f = lane; f < NB / 4; f += 32) bo[f] = reinterpret_cast<const float4 *>(outs)[f];
-        __syncwarp();
     }
+    __syncwarp();
+    float4 *bo = reinterpret_cast<float4 *>(bbar + atom * NB);
+#pragma unroll
+    for (int f = lane; f < NB / 4; f += 32) bo[f] = reinterpret_cast<const float4 *>(outs)[f];
 }
 
-int gram_grid(int64_t N) {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int64_t want = (N + GW - 1) / GW, cap = (int64_t)sms * GRID_PER_SM;
-    return (int)(want < cap ? want : cap);
-}
-
-template <int NPHIP, int NA>
-int run_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b, float *Q) {
-    LAUNCH(ctx, (k_gram_fwd<NPHIP, NA>), gram_grid(N), GW * 32, 0, N, sp_list, b, Q, md.nphi, md.npairs, md.NPp, md.nqp);
-    return REANN_OK;
-}
-template <int NPHIP, int NA>
-int run_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
-                 const float *Qbar, float *bbar) {
-    using C = BwdCfg<NPHIP, NA>;
-    const size_t smem = sizeof(float) * GW * (size_t)(NA * C::TS + NPHIP * NA + md.nqp);
-    static size_t attr = 48 * 1024;
+template <class K>
+int set_smem(K kernel, size_t smem, size_t &attr) {
     if (smem > attr) {
-        if (cudaFuncSetAttribute(k_gram_bwd<NPHIP, NA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
             cudaGetLastError();
             return REANN_ERR_UNSUPPORTED;
         }
         attr = smem;
     }
-    LAUNCH(ctx, (k_gram_bwd<NPHIP, NA>), gram_grid(N), GW * 32, smem, N, sp_list, b, Qbar, bbar, md.nphi, md.NPp, md.nqp);
+    return REANN_OK;
+}
+
+template <int NPHIP, int NA>
+int run_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const DenseTile *tiles,
+                 int n_tiles, const float *b, float *Q) {
+    const int KQ = tiles ? md.K1 : md.nqp;
+    const size_t smem = sizeof(float) * GW * (size_t)(NPHIP * NA + KQ + 4);
+    static size_t attr = 48 * 1024;
+    if (int rc = set_smem(k_gram_fwd<NPHIP, NA>, smem, attr)) return rc;
+    const unsigned grid = tiles ? (unsigned)n_tiles * 16u : div_up(N, GW);
+    LAUNCH(ctx, (k_gram_fwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Q, md.nphi, md.npairs, md.NPp, KQ);
+    return REANN_OK;
+}
+template <int NPHIP, int NA>
+int run_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const DenseTile *tiles,
+                 int n_tiles, const float *b, const float *Qbar, float *bbar) {
+    using C = BwdCfg<NPHIP, NA>;
+    const int KQ = tiles ? md.K1 : md.nqp;
+    const size_t smem = sizeof(float) * GW * (size_t)(C::PER_WARP + KQ + 4);
+    static size_t attr = 48 * 1024;
+    if (int rc = set_smem(k_gram_bwd<NPHIP, NA>, smem, attr)) return rc;
+    const unsigned grid = tiles ? (unsigned)n_tiles * 16u : div_up(N, GW);
+    LAUNCH(ctx, (k_gram_bwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Qbar, bbar, md.nphi, md.NPp, KQ);
     return REANN_OK;
 }
 
@@ -210,14 +270,14 @@ int run_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int
 
 } // namespace
 
-int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
-                    float *Q) {
+int launch_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const DenseTile *tiles,
+                    int n_tiles, const float *b, float *Q) {
     if (N <= 0) return REANN_OK;
-    GRAM_DISPATCH(run_gram_fwd, ctx, md, N, sp_list, b, Q)
+    GRAM_DISPATCH(run_gram_fwd, ctx, md, N, sp_list, tiles, n_tiles, b, Q)
 }
 
-int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const float *b,
-                    const float *Qbar, float *bbar) {
+int launch_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int32_t *sp_list, const DenseTile *tiles,
+                    int n_tiles, const float *b, const float *Qbar, float *bbar) {
     if (N <= 0) return REANN_OK;
-    GRAM_DISPATCH(run_gram_bwd, ctx, md, N, sp_list, b, Qbar, bbar)
+    GRAM_DISPATCH(run_gram_bwd, ctx, md, N, sp_list, tiles, n_tiles, b, Qbar, bbar)
 }
