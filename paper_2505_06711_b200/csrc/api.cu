@@ -579,7 +579,8 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
                                 (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
                                 (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
-                                (float4 *)h->gst.p, (double *)h->Fc.p, (double *)h->vir_part.p, h->n_vir_blocks);
+                                (float4 *)h->gst.p, (double *)h->Fc.p, virial ? (double *)h->vir_part.p : nullptr,
+                                h->n_vir_blocks);
         if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
         mk.mark(7);
         launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,

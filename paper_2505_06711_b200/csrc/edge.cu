@@ -12,6 +12,8 @@
 //   g_e = (sum_n c_j[n] R'_n S_n) r_hat + sum_a P_a grad A_a;   kappa_e[n] = R_n S_n  (t >= 1)
 //   cbar_k[n] = sum_{e in row(k)} kappa_{rev(e)}[n];   F_k = sum_{e in row(k)} (g_e - g_{rev(e)})
 // No floating-point atomics anywhere: the neighbour-side sums are gathers through rev[].
+#include <stdlib.h>
+
 #include "common.cuh"
 
 namespace {
@@ -165,7 +167,7 @@ struct RadialTab { // per layer: [S][NPHIP]; alpha pre-multiplied by log2(e)
 template <int NPHIP, int NA, int PN, int PA>
 struct FwdCfg {
     static constexpr int NG = NPHIP / PN, AG = (NA + PA - 1) / PA, LPA = NG * AG, APW = 32 / LPA;
-    static constexpr int AST = (PA <= 4) ? 4 : 8;       // floats reserved per a-group (16-B aligned)
+    static constexpr int AST = (PA <= 4) ? 4 : (PA <= 8) ? 8 : 12;       // floats reserved per a-group (16-B aligned)
     static constexpr int ROW = NPHIP + AG * AST + 4;     // +4: de-phase rows across banks
     static constexpr int SMEM = EW * APW * 32 * ROW * 4;
     static_assert(NPHIP % PN == 0 && 32 % LPA == 0 && NPHIP % 4 == 0, "bad edge-forward tiling");
@@ -283,33 +285,48 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
 // Warp per atom, one edge per lane; bbar_i is broadcast from shared memory, S_n and P_a stay in the
 // lane's registers, so there is no cross-lane reduction per edge. Orbitals are recomputed (nothing
 // per-edge is kept from the forward pass). Writes the per-edge stash g_e (float4) and kappa_e.
-template <int NPHIP, int NA>
-__global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
+// The radial tables sit in shared memory; c_j and the next pass's edge record are prefetched one
+// step ahead so that no global-load latency is exposed inside the FMA loop. VIR: accumulate the
+// virial (only when the caller asked for it).
+template <int NPHIP, int NA, bool VIR>
+__global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                       const uint32_t *__restrict__ col_rc,
                                                       const float4 *__restrict__ geom,
-                                                      const float *__restrict__ c_ext, RadialTab rt,
+                                                      const float *__restrict__ c_ext, RadialTab rt, int S,
                                                       const float *__restrict__ bbar, int want_kappa,
                                                       float *__restrict__ kappa, float4 *__restrict__ gst,
                                                       double *__restrict__ Fc, double *__restrict__ vir_part) {
     constexpr int NB = NPHIP * NA;
     __shared__ __align__(16) float bb_s[EW][NB];
-    __shared__ double vir_s[EW][9];
+    __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
+    __shared__ float vir_s[VIR ? EW : 1][9];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t i = (int64_t)blockIdx.x * EW + warp;
-    float aF[3] = {0.f, 0.f, 0.f}, aV[9];
+    for (int k = threadIdx.x; k < S * NPHIP; k += EW * 32) { tab_s[0][k] = rt.rcen[k]; tab_s[1][k] = rt.alpha2[k]; }
+    float aF[3] = {0.f, 0.f, 0.f}, aV[VIR ? 9 : 1];
 #pragma unroll
-    for (int k = 0; k < 9; ++k) aV[k] = 0.f;
+    for (int k = 0; k < (VIR ? 9 : 1); ++k) aV[k] = 0.f;
     if (i < N) {
         const float4 *src = reinterpret_cast<const float4 *>(bbar + i * (int64_t)NB);
         for (int k = lane; k < NB / 4; k += 32) reinterpret_cast<float4 *>(bb_s[warp])[k] = src[k];
-        __syncwarp();
+    }
+    __syncthreads();
+    if (i < N) {
         const int64_t beg = rc_ptr[i], end = rc_ptr[i + 1];
         const float pi_rc = 3.14159265358979f * rt.inv_rc;
-        for (int64_t e = beg + lane; e < end; e += 32) {
-            const float4 g = geom[e];
-            const uint32_t cj = col_rc[e];
+        int64_t e = beg + lane;
+        float4 g = make_float4(0.f, 0.f, 0.f, 1.f);
+        uint32_t cj = 0;
+        if (e < end) { g = geom[e]; cj = col_rc[e]; }
+        while (e < end) {
             const int sj = cj >> COL_SPECIES_SHIFT;
             const float4 *cptr = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
+            float4 cv = cptr[0];
+            // next pass's edge record
+            const int64_t e_next = e + 32;
+            float4 g_next = g;
+            uint32_t cj_next = cj;
+            if (e_next < end) { g_next = geom[e_next]; cj_next = col_rc[e_next]; }
             float sn, cs;
             sincospif(g.w * rt.inv_rc, &sn, &cs);
             const float fc = 0.5f + 0.5f * cs, dfc = -0.5f * pi_rc * sn;
@@ -323,12 +340,12 @@ __global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd(int64_t N, const int64_
             float4 *kp = reinterpret_cast<float4 *>(kappa + e * (int64_t)NPHIP);
 #pragma unroll 1
             for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
-                const float4 cv = cptr[n4];
-                const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[n4];
-                const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[n4];
+                const float4 cvn = cptr[n4 + 1 < NPHIP / 4 ? n4 + 1 : n4];
+                const float4 rc4 = reinterpret_cast<const float4 *>(tab_s[0] + sj * NPHIP)[n4];
+                const float4 al4 = reinterpret_cast<const float4 *>(tab_s[1] + sj * NPHIP)[n4];
                 const float cva[4] = {cv.x, cv.y, cv.z, cv.w}, rca[4] = {rc4.x, rc4.y, rc4.z, rc4.w},
                             ala[4] = {al4.x, al4.y, al4.z, al4.w};
-                float Rn[4], xn[4], yn[4], S[4];
+                float Rn[4], xn[4], yn[4], Sn[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const float d = g.w - rca[u];
@@ -337,7 +354,7 @@ __global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd(int64_t N, const int64_
                     Rn[u] = ex * fc;
                     xn[u] = cva[u] * Rn[u];
                     yn[u] = cva[u] * ((-1.3862943611198906f * ala[u] * d * fc + dfc) * ex);
-                    S[u] = 0.f;
+                    Sn[u] = 0.f;
                 }
                 const float4 *bb4 = reinterpret_cast<const float4 *>(bb_s[warp] + n4 * 4 * NA);
 #pragma unroll
@@ -347,49 +364,52 @@ __global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd(int64_t N, const int64_
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const int f = f4 * 4 + u, nl = f / NA, a = f % NA;
-                        S[nl] = fmaf(va[u], A[a], S[nl]);
+                        Sn[nl] = fmaf(va[u], A[a], Sn[nl]);
                         P[a] = fmaf(va[u], xn[nl], P[a]);
                     }
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u) radial = fmaf(yn[u], S[u], radial);
-                if (want_kappa) kp[n4] = make_float4(Rn[0] * S[0], Rn[1] * S[1], Rn[2] * S[2], Rn[3] * S[3]);
+                for (int u = 0; u < 4; ++u) radial = fmaf(yn[u], Sn[u], radial);
+                if (want_kappa) kp[n4] = make_float4(Rn[0] * Sn[0], Rn[1] * Sn[1], Rn[2] * Sn[2], Rn[3] * Sn[3]);
+                cv = cvn;
             }
             float gx, gy, gz;
             monomial_vjp<NA>(A, P, gx, gy, gz);
-            const float rr = radial / g.w;
+            const float rr = __fdividef(radial, g.w);
             gx = fmaf(rr, g.x, gx); gy = fmaf(rr, g.y, gy); gz = fmaf(rr, g.z, gz);
             gst[e] = make_float4(gx, gy, gz, 0.f);
             aF[0] += gx; aF[1] += gy; aF[2] += gz;
-            aV[0] -= g.x * gx; aV[1] -= g.x * gy; aV[2] -= g.x * gz;
-            aV[3] -= g.y * gx; aV[4] -= g.y * gy; aV[5] -= g.y * gz;
-            aV[6] -= g.z * gx; aV[7] -= g.z * gy; aV[8] -= g.z * gz;
+            if constexpr (VIR) {
+                aV[0] -= g.x * gx; aV[1] -= g.x * gy; aV[2] -= g.x * gz;
+                aV[3] -= g.y * gx; aV[4] -= g.y * gy; aV[5] -= g.y * gz;
+                aV[6] -= g.z * gx; aV[7] -= g.z * gy; aV[8] -= g.z * gz;
+            }
+            e = e_next; g = g_next; cj = cj_next;
         }
     }
-    // fixed-order reductions: lanes (butterfly), then warps, then one slot per block
-    double dF[3], dV[9];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) dF[k] = (double)aF[k];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) dV[k] = (double)aV[k];
+    // fixed-order reductions: lanes (butterfly, FP32), then FP64 accumulation across layers / warps
 #pragma unroll
     for (int d = 16; d >= 1; d >>= 1) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) dF[k] += __shfl_xor_sync(0xffffffffu, dF[k], d);
+        for (int k = 0; k < 3; ++k) aF[k] += __shfl_xor_sync(0xffffffffu, aF[k], d);
+        if constexpr (VIR) {
 #pragma unroll
-        for (int k = 0; k < 9; ++k) dV[k] += __shfl_xor_sync(0xffffffffu, dV[k], d);
+            for (int k = 0; k < 9; ++k) aV[k] += __shfl_xor_sync(0xffffffffu, aV[k], d);
+        }
     }
-    if (lane == 0) {
-        if (i < N) { Fc[3 * i] += dF[0]; Fc[3 * i + 1] += dF[1]; Fc[3 * i + 2] += dF[2]; }
+    if (lane == 0 && i < N) { Fc[3 * i] += (double)aF[0]; Fc[3 * i + 1] += (double)aF[1]; Fc[3 * i + 2] += (double)aF[2]; }
+    if constexpr (VIR) {
+        if (lane == 0) {
 #pragma unroll
-        for (int k = 0; k < 9; ++k) vir_s[warp][k] = dV[k];
-    }
-    __syncthreads();
-    if (threadIdx.x < 9) {
-        double s = 0.0;
+            for (int k = 0; k < 9; ++k) vir_s[warp][k] = aV[k];
+        }
+        __syncthreads();
+        if (threadIdx.x < 9) {
+            double s = 0.0;
 #pragma unroll
-        for (int w = 0; w < EW; ++w) s += vir_s[w][threadIdx.x];
-        vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x] += s;
+            for (int w = 0; w < EW; ++w) s += (double)vir_s[w][threadIdx.x];
+            vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x] += s;
+        }
     }
 }
 
@@ -552,6 +572,13 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
     if (N <= 0) return REANN_OK;
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
 #define M(NP, NA_, PN_, PA_) return run_edge_fwd<NP, NA_, PN_, PA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    if (md.nphip == 16 && md.Na == 20) {   // EXPERIMENT
+        static int v = -1;
+        if (v < 0) { const char *e = getenv("REANN_FWD_TILE"); v = e ? atoi(e) : 0; }
+        if (v == 1) M(16, 20, 4, 5)
+        if (v == 2) M(16, 20, 8, 5)
+        if (v == 3) M(16, 20, 4, 10)
+    }
     EDGE_DISPATCH(M)
 #undef M
 }
@@ -566,9 +593,13 @@ int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
     (void)n_vir_blocks;
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
     const int want_kappa = t >= 1;
-#define M(NP, NA_, PN_, PA_)                                                                                  \
-    LAUNCH(ctx, (k_edge_bwd<NP, NA_>), div_up(N, EW), EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt, bbar,   \
-           want_kappa, kappa, gst, Fc, vir_part);                                                             \
+#define M(NP, NA_, PN_, PA_)                                                                                      \
+    if (vir_part)                                                                                                 \
+        LAUNCH(ctx, (k_edge_bwd<NP, NA_, true>), div_up(N, EW), EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,   \
+               md.S, bbar, want_kappa, kappa, gst, Fc, vir_part);                                                 \
+    else                                                                                                          \
+        LAUNCH(ctx, (k_edge_bwd<NP, NA_, false>), div_up(N, EW), EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,  \
+               md.S, bbar, want_kappa, kappa, gst, Fc, vir_part);                                                 \
     return REANN_OK;
     EDGE_DISPATCH(M)
 #undef M
