@@ -12,8 +12,6 @@
 //   g_e = (sum_n c_j[n] R'_n S_n) r_hat + sum_a P_a grad A_a;   kappa_e[n] = R_n S_n  (t >= 1)
 //   cbar_k[n] = sum_{e in row(k)} kappa_{rev(e)}[n];   F_k = sum_{e in row(k)} (g_e - g_{rev(e)})
 // No floating-point atomics anywhere: the neighbour-side sums are gathers through rev[].
-#include <stdlib.h>
-
 #include "common.cuh"
 
 namespace {
@@ -160,16 +158,22 @@ struct RadialTab { // per layer: [S][NPHIP]; alpha pre-multiplied by log2(e)
 };
 
 // ------------------------------------------------------------------------------------------ A5
-// Warp-autonomous: a warp owns APW = 32/LPA atoms. Per chunk of 32 edges of one atom the lanes
-// first work one-edge-per-lane (radial functions x_e[n], monomials A_a -> shared memory), then
-// every lane accumulates its PN x PA block of b_i[n,a] over the staged edges (operands read as
-// broadcast vectors from shared memory, accumulators in registers, no atomics).
+// Warp-autonomous: a warp owns APW = 32/LPA atoms; lane group `sub` (LPA lanes) owns atom `sub` and
+// every lane of it a PN x PA block of b_i[n,a] in registers. Per round the warp stages 32 edges,
+// EPA = 32/APW of each of its atoms (staged row = lane):
+//   1a  one edge per lane: edge record, cutoff function, monomials A_a -> shared memory;
+//   1b  NPHIP/4 lanes per edge: each gathers one float4 of c_j (a load instruction then touches
+//       whole 64-byte rows) and stores its four x_e[n];
+//   2   every lane accumulates its block over the staged edges of its atom (operands read as
+//       vectors from shared memory, no atomics).
+// Shared memory delivers 128 B per clock to the lanes whether or not they read the same word, so
+// what counts is operand floats per FMA: (PN + PA) / (PN PA) -- hence the large register blocks.
 template <int NPHIP, int NA, int PN, int PA>
 struct FwdCfg {
-    static constexpr int NG = NPHIP / PN, AG = (NA + PA - 1) / PA, LPA = NG * AG, APW = 32 / LPA;
-    static constexpr int AST = (PA <= 4) ? 4 : (PA <= 8) ? 8 : 12;       // floats reserved per a-group (16-B aligned)
+    static constexpr int NG = NPHIP / PN, AG = (NA + PA - 1) / PA, LPA = NG * AG, APW = 32 / LPA, EPA = 32 / APW;
+    static constexpr int AST = (PA + 3) & ~3;            // floats reserved per a-group (16-B aligned)
     static constexpr int ROW = NPHIP + AG * AST + 4;     // +4: de-phase rows across banks
-    static constexpr int SMEM = EW * APW * 32 * ROW * 4;
+    static constexpr int SMEM = EW * 32 * ROW * 4;
     static_assert(NPHIP % PN == 0 && 32 % LPA == 0 && NPHIP % 4 == 0, "bad edge-forward tiling");
 };
 
@@ -182,7 +186,7 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
     using C = FwdCfg<NPHIP, NA, PN, PA>;
     extern __shared__ __align__(16) float smem_f[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *stage = smem_f + (size_t)warp * C::APW * 32 * C::ROW;
+    float *stage = smem_f + (size_t)warp * 32 * C::ROW;
     const int sub = lane / C::LPA, sl = lane % C::LPA, p = sl % C::NG, q = sl / C::NG;
     const int64_t atom0 = ((int64_t)blockIdx.x * EW + warp) * C::APW;
     if (atom0 >= N) return;
@@ -192,61 +196,80 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
     int64_t maxlen = my_end - my_beg;
 #pragma unroll
     for (int d = 16; d >= 1; d >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, d));
+    // phase 1a: lane -> (atom slot, edge within the round); EPA == LPA, so slot == sub
+    const int le = lane % C::EPA;
     float acc[PN][PA];
 #pragma unroll
     for (int a = 0; a < PN; ++a)
 #pragma unroll
         for (int c = 0; c < PA; ++c) acc[a][c] = 0.0f;
 
-    for (int64_t c0 = 0; c0 < maxlen; c0 += 32) {
-        // ---- phase 1: one edge per lane ----
+    for (int64_t c0 = 0; c0 < maxlen; c0 += C::EPA) {
+        // ---- phase 1a ----
+        const int64_t e = my_beg + c0 + le;
+        float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+        uint32_t cj = 0;
+        float fc = 0.f;
+        const bool have = e < my_end;
+        if (have) {
+            g = geom[e];
+            cj = col_rc[e];
+            fc = 0.5f + 0.5f * cospif(g.w * rt.inv_rc);
+            float *row = stage + (size_t)lane * C::ROW;
+            float A[C::AG * C::AST];
 #pragma unroll
-        for (int s = 0; s < C::APW; ++s) {
-            const int64_t beg = __shfl_sync(0xffffffffu, my_beg, s * C::LPA);
-            const int64_t end = __shfl_sync(0xffffffffu, my_end, s * C::LPA);
-            const int64_t e = beg + c0 + lane;
-            if (e < end) {
-                const float4 g = geom[e];
-                const uint32_t cj = col_rc[e];
-                const int sj = cj >> COL_SPECIES_SHIFT;
-                const float4 *cptr = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
-                const float fc = 0.5f + 0.5f * cospif(g.w * rt.inv_rc);
-                float *row = stage + (size_t)(s * 32 + lane) * C::ROW;
+            for (int a = 0; a < C::AG * C::AST; ++a) A[a] = 0.0f;
+            float Am[NA];
+            monomials<NA>(g.x, g.y, g.z, Am);
 #pragma unroll
-                for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
-                    const float4 cv = cptr[n4];
-                    const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[n4];
-                    const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[n4];
+            for (int a = 0; a < NA; ++a) A[(a / PA) * C::AST + a % PA] = Am[a];
+#pragma unroll
+            for (int v4 = 0; v4 < C::AG * C::AST / 4; ++v4)
+                reinterpret_cast<float4 *>(row + NPHIP)[v4] = make_float4(A[4 * v4], A[4 * v4 + 1], A[4 * v4 + 2], A[4 * v4 + 3]);
+        }
+        // ---- phase 1b ----
+        {
+            constexpr int PARTS = NPHIP / 4, EPI = 32 / PARTS, ROUNDS = (32 + EPI - 1) / EPI;
+            const int part = lane % PARTS;
+#pragma unroll
+            for (int r = 0; r < ROUNDS; ++r) {
+                const int rr = r * EPI + lane / PARTS;            // staged row = lane that holds its record
+                const bool mine = lane < EPI * PARTS && rr < 32;
+                const int src = mine ? rr : 0;
+                const uint32_t cje = __shfl_sync(0xffffffffu, cj, src);
+                const float we = __shfl_sync(0xffffffffu, g.w, src);
+                const float fce = __shfl_sync(0xffffffffu, fc, src);
+                const int ok = __shfl_sync(0xffffffffu, (int)have, src);
+                if (mine && ok) {
+                    const int sj = cje >> COL_SPECIES_SHIFT;
+                    const float4 cv = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cje & COL_IDX_MASK) * NPHIP)[part];
+                    const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[part];
+                    const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[part];
                     float4 xv;
                     float d;
-                    d = g.w - rc4.x; xv.x = cv.x * (exp2f(-al4.x * d * d) * fc);
-                    d = g.w - rc4.y; xv.y = cv.y * (exp2f(-al4.y * d * d) * fc);
-                    d = g.w - rc4.z; xv.z = cv.z * (exp2f(-al4.z * d * d) * fc);
-                    d = g.w - rc4.w; xv.w = cv.w * (exp2f(-al4.w * d * d) * fc);
-                    reinterpret_cast<float4 *>(row)[n4] = xv;
+                    d = we - rc4.x; xv.x = cv.x * (exp2f(-al4.x * d * d) * fce);
+                    d = we - rc4.y; xv.y = cv.y * (exp2f(-al4.y * d * d) * fce);
+                    d = we - rc4.z; xv.z = cv.z * (exp2f(-al4.z * d * d) * fce);
+                    d = we - rc4.w; xv.w = cv.w * (exp2f(-al4.w * d * d) * fce);
+                    reinterpret_cast<float4 *>(stage + (size_t)rr * C::ROW)[part] = xv;
                 }
-                float A[C::AG * PA];
-#pragma unroll
-                for (int a = NA; a < C::AG * PA; ++a) A[a] = 0.0f;
-                monomials<NA>(g.x, g.y, g.z, A);
-#pragma unroll
-                for (int ag = 0; ag < C::AG; ++ag)
-#pragma unroll
-                    for (int pa = 0; pa < PA; ++pa) row[NPHIP + ag * C::AST + pa] = A[ag * PA + pa];
             }
         }
         __syncwarp();
         // ---- phase 2: register-tiled accumulation over the staged edges of my atom ----
         int64_t cnt64 = my_end - (my_beg + c0);
-        const int cnt = cnt64 > 32 ? 32 : (cnt64 < 0 ? 0 : (int)cnt64);
-        const float *rowb = stage + (size_t)(sub * 32) * C::ROW;
+        const int cnt = cnt64 > C::EPA ? C::EPA : (cnt64 < 0 ? 0 : (int)cnt64);
+        const float *rowb = stage + (size_t)(sub * C::EPA) * C::ROW;
 #pragma unroll 4
         for (int k = 0; k < cnt; ++k) {
             const float *row = rowb + (size_t)k * C::ROW;
             float xv[PN], av[PA];
-            if constexpr (PN == 4) {
-                const float4 v = *reinterpret_cast<const float4 *>(row + p * 4);
-                xv[0] = v.x; xv[1] = v.y; xv[2] = v.z; xv[3] = v.w;
+            if constexpr (PN % 4 == 0) {
+#pragma unroll
+                for (int a4 = 0; a4 < PN / 4; ++a4) {
+                    const float4 v = *reinterpret_cast<const float4 *>(row + p * PN + a4 * 4);
+                    xv[a4 * 4] = v.x; xv[a4 * 4 + 1] = v.y; xv[a4 * 4 + 2] = v.z; xv[a4 * 4 + 3] = v.w;
+                }
             } else if constexpr (PN == 2) {
                 const float2 v = *reinterpret_cast<const float2 *>(row + p * 2);
                 xv[0] = v.x; xv[1] = v.y;
@@ -255,15 +278,16 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
                 for (int a = 0; a < PN; ++a) xv[a] = row[p * PN + a];
             }
             const float *ar = row + NPHIP + q * C::AST;
-            if constexpr (PA >= 4) {
-                const float4 v = *reinterpret_cast<const float4 *>(ar);
-                av[0] = v.x; av[1] = v.y; av[2] = v.z; av[3] = v.w;
 #pragma unroll
-                for (int c = 4; c < PA; ++c) av[c] = ar[c];
-            } else {
-#pragma unroll
-                for (int c = 0; c < PA; ++c) av[c] = ar[c];
+            for (int c4 = 0; c4 < PA / 4; ++c4) {
+                const float4 v = *reinterpret_cast<const float4 *>(ar + c4 * 4);
+                av[c4 * 4] = v.x; av[c4 * 4 + 1] = v.y; av[c4 * 4 + 2] = v.z; av[c4 * 4 + 3] = v.w;
             }
+            if constexpr (PA % 4 >= 2) {
+                const float2 v = *reinterpret_cast<const float2 *>(ar + (PA / 4) * 4);
+                av[(PA / 4) * 4] = v.x; av[(PA / 4) * 4 + 1] = v.y;
+            }
+            if constexpr (PA % 2 == 1) av[PA - 1] = ar[PA - 1];
 #pragma unroll
             for (int a = 0; a < PN; ++a)
 #pragma unroll
@@ -562,7 +586,7 @@ static int run_edge_fwd(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, 
         case 401: M(4, 1, 1, 1) case 404: M(4, 4, 1, 4) case 410: M(4, 10, 1, 5) case 420: M(4, 20, 1, 5)      \
         case 801: M(8, 1, 2, 1) case 804: M(8, 4, 2, 4) case 810: M(8, 10, 2, 5) case 820: M(8, 20, 2, 5)      \
         case 1201: M(12, 1, 3, 1) case 1204: M(12, 4, 3, 4) case 1210: M(12, 10, 3, 5) case 1220: M(12, 20, 3, 5) \
-        case 1601: M(16, 1, 2, 1) case 1604: M(16, 4, 2, 4) case 1610: M(16, 10, 2, 5) case 1620: M(16, 20, 2, 5) \
+        case 1601: M(16, 1, 2, 1) case 1604: M(16, 4, 2, 4) case 1610: M(16, 10, 2, 5) case 1620: M(16, 20, 4, 5) \
         default: return REANN_ERR_UNSUPPORTED;                                                           \
     }
 
@@ -572,13 +596,6 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
     if (N <= 0) return REANN_OK;
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
 #define M(NP, NA_, PN_, PA_) return run_edge_fwd<NP, NA_, PN_, PA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
-    if (md.nphip == 16 && md.Na == 20) {   // EXPERIMENT
-        static int v = -1;
-        if (v < 0) { const char *e = getenv("REANN_FWD_TILE"); v = e ? atoi(e) : 0; }
-        if (v == 1) M(16, 20, 4, 5)
-        if (v == 2) M(16, 20, 8, 5)
-        if (v == 3) M(16, 20, 4, 10)
-    }
     EDGE_DISPATCH(M)
 #undef M
 }
