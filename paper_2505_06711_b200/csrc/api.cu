@@ -283,7 +283,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         // tensor-core chunk images (dense_tc.cu): pre-split hi | lo TF32 operands
         {
             std::vector<float> img;
-            struct OffT { size_t g1, g2, r2, r3; };
+            struct OffT { size_t g1, g2, r1, r2, r3; };
             std::vector<OffT> ot(offs.size());
             for (int t = 0; t < T; ++t) {
                 const int H1p = h->ld[t].H1p, H2p = h->ld[t].H2p, nout = h->ld[t].nout;
@@ -294,6 +294,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
                     auto Uqh = [&](int qq, int hh) { return qq < md.nqp ? A[o.U + (size_t)qq * H1p + hh] : 0.f; };
                     q.g1 = push_images(img, H1p, md.K1, [&](int n, int k) { return Uqh(k, n); });
                     q.g2 = push_images(img, H2p, H1p, [&](int n, int k) { return A[o.W2 + (size_t)k * H2p + n]; });
+                    q.r1 = push_images(img, H2p, 32, [&](int n, int k) { return k < nout ? A[o.W3 + (size_t)n * nout + k] : 0.f; });
                     q.r2 = push_images(img, H1p, H2p, [&](int n, int k) { return A[o.W2 + (size_t)n * H2p + k]; });
                     q.r3 = img.size();
                     for (int nb = 0; nb * 128 < md.K1; ++nb) {
@@ -307,7 +308,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
             const float *ib = (const float *)h->wt_all.p;
             std::vector<DenseWT> wt(offs.size());
             for (size_t k = 0; k < offs.size(); ++k)
-                wt[k] = DenseWT{ib + ot[k].g1, ib + ot[k].g2, ib + ot[k].r2, ib + ot[k].r3,
+                wt[k] = DenseWT{ib + ot[k].g1, ib + ot[k].g2, ib + ot[k].r1, ib + ot[k].r2, ib + ot[k].r3,
                                 base + offs[k].b1, base + offs[k].b2, base + offs[k].b3, base + offs[k].W3p, base + offs[k].W3c0};
             CRC(dev_ensure(h, h->wt_tab, sizeof(DenseWT) * wt.size()));
             CCU(cudaMemcpy(h->wt_tab.p, wt.data(), sizeof(DenseWT) * wt.size(), cudaMemcpyHostToDevice));

@@ -58,7 +58,7 @@ struct DenseW {
 // Tensor-core path (dense_tc.cu): pre-split (hi | lo) TF32 weight chunk images, see dense_tc.cu.
 struct DenseWT {
     const float *g1, *g2;      // forward:  U^T chunks [K1/32], W2^T chunks [H1p/32]
-    const float *r2, *r3;      // reverse:  W2 chunks [H2p/32], U blocks of <= 128 rows x [H1p/32]
+    const float *r1, *r2, *r3; // reverse:  W3 chunk (K = n_out padded to 32), W2 chunks [H2p/32], U blocks of <= 128 rows x [H1p/32]
     const float *b1, *b2, *b3; // biases (FP32)
     const float *w3p;          // FP32 [H2p][16]: W3 rows zero-padded to 16 outputs (ALU GEMM with n_out <= 16)
     const float *w3c0;         // FP32 [H2p]: first column of W3 (energy layer, n_out = 1)

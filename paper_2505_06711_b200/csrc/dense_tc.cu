@@ -482,28 +482,35 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
     const DenseWT W = A.w[tile.species];
     const uint32_t bar0 = smem_u32(smem + SM_BAR);
     const uint32_t tmem = tc_prologue(smem, &tmem_base_s, CW2 >= 32 ? 128u : 256u);
-    const int nblk = (A.K1 + 127) / 128, total = NCH2 + nblk * NCH1;
+    // steps: [R1 (only when outbar is given: K = n_out padded to 32)] NCH2 x R2, nblk x NCH1 x R3
+    const int o1 = A.outbar ? 1 : 0, i3 = o1 + NCH2;
+    const int nblk = (A.K1 + 127) / 128, total = i3 + nblk * NCH1;
 
     if (warp == CTL_WARP) {
         if (lane == 0) {
             Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem};
-            auto rows_of = [&](int i) { return i < NCH2 ? H1p : min(128, A.K1 - ((i - NCH2) / NCH1) * 128); };
+            auto rows_of = [&](int i) { return i < o1 ? H2p : i < i3 ? H1p : min(128, A.K1 - ((i - i3) / NCH1) * 128); };
             auto copy_b = [&](int i) {
-                if (i < NCH2) { c.copy_b(i, W.r2 + (size_t)i * (2 * H1p * KC), H1p); return; }
-                const int nb = (i - NCH2) / NCH1, kc = (i - NCH2) % NCH1, nr = rows_of(i);
+                if (i < o1) { c.copy_b(i, W.r1, H2p); return; }
+                if (i < i3) { c.copy_b(i, W.r2 + (size_t)(i - o1) * (2 * H1p * KC), H1p); return; }
+                const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1, nr = rows_of(i);
                 c.copy_b(i, W.r3 + (size_t)nb * NCH1 * (2 * 128 * KC) + (size_t)kc * (2 * nr * KC), nr);
             };
             copy_b(0);
             if (total > 1) copy_b(1);
             for (int i = 0; i < total; ++i) {
-                if (i < NCH2) {
-                    mbar_wait(c.bar(BAR_AH + i), 0);
+                if (i < o1) {
+                    mbar_wait(c.bar(BAR_AFULL), 0);
                     TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, i, H1p);
+                    c.mma_chunk(i, 0, H2p);
+                } else if (i < i3) {
+                    mbar_wait(c.bar(BAR_AH + (i - o1)), 0);
+                    TC_TRACE(1, 0, 2 * i);
+                    c.mma_chunk(i, i - o1, H1p);
                 } else {
-                    if (i == NCH2) mbar_wait(c.bar(BAR_ARES), 0);
+                    if (i == i3) mbar_wait(c.bar(BAR_ARES), 0);
                     TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, (i - NCH2) % NCH1, rows_of(i));
+                    c.mma_chunk(i, (i - i3) % NCH1, rows_of(i));
                 }
                 TC_TRACE(1, 0, 2 * i + 1);
                 if (i + 2 < total) copy_b(i + 2);
@@ -516,67 +523,76 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
         unsigned char *a_base = smem + SM_A;
         const float *zt = A.z_stash + (size_t)blockIdx.x * A.zs * TM + m * 4;
         if (tid == 0) TC_TRACE(1, 1, 100);
-        // ---- h2bar = outbar W3^T (FP32, own column half); z2bar = h2bar SiLU'(z2) -> A operand of GEMM R2 ----
+        // ---- h2bar = outbar W3^T: tensor core (K = n_out padded to 32) or, for the energy layer, W3's column;
+        //      z2bar = h2bar SiLU'(z2) -> A operand of GEMM R2. The z stash is read ahead of the drains. ----
         {
-            float ob[16];
-#pragma unroll
-            for (int c = 0; c < 16; ++c) ob[c] = 0.f;
-            if (valid && A.outbar) {
-                const float4 *src =
-                    reinterpret_cast<const float4 *>(A.outbar + (size_t)A.sp_list[tile.start + m] * A.outbar_stride);
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (q * 4 < A.nout) {
-                        const float4 t = __ldg(src + q);
-                        ob[q * 4] = t.x; ob[q * 4 + 1] = t.y; ob[q * 4 + 2] = t.z; ob[q * 4 + 3] = t.w;
-                    }
-#pragma unroll
-                for (int c = 0; c < 16; ++c)
-                    if (c >= A.nout) ob[c] = 0.f;
-            }
-            float x[CW2];
+            float4 z2[CW2 / 4];
 #pragma unroll
             for (int k4 = 0; k4 < CW2 / 4; ++k4) {
-                const int col = hf * CW2 + k4 * 4;
-                float hb[4];
-                if (A.outbar == nullptr) {
-                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + col));
-                    hb[0] = w4.x; hb[1] = w4.y; hb[2] = w4.z; hb[3] = w4.w;
-                } else {
+                z2[k4] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (valid) z2[k4] = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((H1p + hf * CW2 + k4 * 4) >> 2) * (TM * 4)));
+            }
+            float x[CW2];
+            if (o1) {
+                // operand: row m of outbar in columns 0..15 (column half 0), zeros in 16..31 (half 1)
+                float ob[16];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const float4 *wr = reinterpret_cast<const float4 *>(W.w3p + (size_t)(col + u) * 16);
-                        float sacc = 0.f;
+                for (int c = 0; c < 16; ++c) ob[c] = 0.f;
+                if (valid && hf == 0) {
+                    const float4 *src =
+                        reinterpret_cast<const float4 *>(A.outbar + (size_t)A.sp_list[tile.start + m] * A.outbar_stride);
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const float4 w4 = __ldg(wr + q);
-                            sacc = fmaf(ob[q * 4], w4.x, sacc); sacc = fmaf(ob[q * 4 + 1], w4.y, sacc);
-                            sacc = fmaf(ob[q * 4 + 2], w4.z, sacc); sacc = fmaf(ob[q * 4 + 3], w4.w, sacc);
+                    for (int q = 0; q < 4; ++q)
+                        if (q * 4 < A.nout) {
+                            const float4 t = __ldg(src + q);
+                            ob[q * 4] = t.x; ob[q * 4 + 1] = t.y; ob[q * 4 + 2] = t.z; ob[q * 4 + 3] = t.w;
                         }
-                        hb[u] = sacc;
-                    }
+#pragma unroll
+                    for (int c = 0; c < 16; ++c)
+                        if (c >= A.nout) ob[c] = 0.f;
                 }
-                float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (valid) z = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((H1p + col) >> 2) * (TM * 4)));
-                x[k4 * 4] = valid ? hb[0] * dsilu_f(z.x) : 0.f; x[k4 * 4 + 1] = valid ? hb[1] * dsilu_f(z.y) : 0.f;
-                x[k4 * 4 + 2] = valid ? hb[2] * dsilu_f(z.z) : 0.f; x[k4 * 4 + 3] = valid ? hb[3] * dsilu_f(z.w) : 0.f;
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) store_split4(a_base, hf * 4 + k4, m, ob + k4 * 4);
+                fence_async_smem();
+                mbar_arrive(bar0 + 8 * BAR_AFULL);
+#pragma unroll
+                for (int c = 0; c < CW2; ++c) x[c] = 0.f;
+                drain_group<CW2>(x, bar0, tl, 0, hf * CW2, true);   // the R1 MMAs have completed: slot 0 is free again
+            } else {
+#pragma unroll
+                for (int k4 = 0; k4 < CW2 / 4; ++k4) {
+                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + hf * CW2 + k4 * 4));
+                    x[k4 * 4] = w4.x; x[k4 * 4 + 1] = w4.y; x[k4 * 4 + 2] = w4.z; x[k4 * 4 + 3] = w4.w;
+                }
+            }
+#pragma unroll
+            for (int k4 = 0; k4 < CW2 / 4; ++k4) {
+                x[k4 * 4] = valid ? x[k4 * 4] * dsilu_f(z2[k4].x) : 0.f;
+                x[k4 * 4 + 1] = valid ? x[k4 * 4 + 1] * dsilu_f(z2[k4].y) : 0.f;
+                x[k4 * 4 + 2] = valid ? x[k4 * 4 + 2] * dsilu_f(z2[k4].z) : 0.f;
+                x[k4 * 4 + 3] = valid ? x[k4 * 4 + 3] * dsilu_f(z2[k4].w) : 0.f;
             }
             store_operand<CW2>(x, a_base, bar0, hf * CW2, m);
         }
         if (tid == 0) TC_TRACE(1, 1, 101);
         // ---- GEMM R2: h1bar = z2bar W2^T; z1bar = h1bar SiLU'(z1) -> resident A operand of GEMM R3 ----
         {
+            float4 z1[CW1 / 4];
+#pragma unroll
+            for (int k4 = 0; k4 < CW1 / 4; ++k4) {
+                z1[k4] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (valid) z1[k4] = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((hf * CW1 + k4 * 4) >> 2) * (TM * 4)));
+            }
             float h1b[CW1];
 #pragma unroll
             for (int c = 0; c < CW1; ++c) h1b[c] = 0.f;
 #pragma unroll 1
-            for (int kc = 0; kc < NCH2; ++kc) drain_group<CW1>(h1b, bar0, tl, kc, hf * CW1, true);
+            for (int kc = 0; kc < NCH2; ++kc) drain_group<CW1>(h1b, bar0, tl, o1 + kc, hf * CW1, true);
             // all MMAs of R2 have completed: the A slots may be overwritten
 #pragma unroll
             for (int k4 = 0; k4 < CW1 / 4; ++k4) {
                 const int col = hf * CW1 + k4 * 4;
-                float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (valid) z = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)(col >> 2) * (TM * 4)));
+                const float4 z = z1[k4];
                 const float xv[4] = {valid ? h1b[k4 * 4] * dsilu_f(z.x) : 0.f, valid ? h1b[k4 * 4 + 1] * dsilu_f(z.y) : 0.f,
                                      valid ? h1b[k4 * 4 + 2] * dsilu_f(z.z) : 0.f, valid ? h1b[k4 * 4 + 3] * dsilu_f(z.w) : 0.f};
                 store_split4(a_base + (col >> 5) * A_SLOT, (col & 31) >> 2, m, xv);
@@ -596,7 +612,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
             for (int c = 0; c < 64; ++c) q[c] = 0.f;
 #pragma unroll 1
             for (int kc = 0; kc < NCH1; ++kc) {
-                const int g = NCH2 + nb * NCH1 + kc;
+                const int g = i3 + nb * NCH1 + kc;
                 if (ncols - hf * 64 >= 64) drain_group<64>(q, bar0, tl, g, hf * 64, true);
                 else if (ncols - hf * 64 >= 32) drain_group<32>(q, bar0, tl, g, hf * 64, true);
                 else drain_group<32>(q, bar0, tl, g, hf * 64, false);
