@@ -44,6 +44,22 @@ def load_peaks():
             "_source": "fallback"}
 
 
+def load_traffic(k: int) -> dict:
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture) of
+    the kernel groups, from the committed profile summary; only valid for the config it was captured on."""
+    p = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    out = {}
+    if os.path.exists(p):
+        with open(p) as f:
+            for line in f:
+                if line.startswith("#") or not line.strip():
+                    continue
+                group, cfg, nbytes = line.strip().split(",")[:3]
+                if group != "group" and int(cfg) == k:
+                    out[group] = float(nbytes)
+    return out
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -60,6 +76,11 @@ class ClockSampler:
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
             self.proc = None
+
+    def wait_first(self, timeout_s: float):
+        t0 = time.time()
+        while self.proc is not None and not self.rows and time.time() - t0 < timeout_s:
+            time.sleep(0.02)
 
     def _read(self):
         for line in self.proc.stdout:
@@ -174,17 +195,24 @@ def main():
         m.energy_forces(pos, box, E, F)
         m.verlet(pos, vel, F, inv_m, dt_fs, acc, False)
 
+    # nvidia-smi takes a few hundred ms to attach to the driver and holds up CUDA calls while it does: start it
+    # before the warm-up and wait for its first sample, so that only its periodic queries fall in the timed region
+    sampler = ClockSampler(local_rank)
+    sampler.start()
     m.build_neighbors(pos, box)
     m.energy_forces(pos, box, E, F)
     for _ in range(W):
         md_step()
     torch.cuda.synchronize()
+    sampler.wait_first(5.0)
+    for _ in range(2):
+        md_step()
+    torch.cuda.synchronize()
+    sampler.rows.clear()
 
     # ---------------- device-resident timed region ----------------
     m.set_profiling(True)
     s0 = m.stats()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -240,20 +268,36 @@ def main():
         E_rc = s1["n_edges_rc"]
         H1, H2 = cfg["H"]
         n_q = gen.n_orb_default(nphi, L)
-        # algorithmic flops per launch (one layer): 1 FMA = 2 flop
-        flops = {"ms_edge_fwd": 2.0 * E_rc * nphi * Na, "ms_edge_bwd": 4.0 * E_rc * nphi * Na,
-                 "ms_dense_fwd": 2.0 * n * (n_q * H1 + H1 * H2 + H2 * nphi),
-                 "ms_dense_bwd": 2.0 * n * (n_q * H1 + H1 * H2 + H2 * nphi)}
-        dom = max(flops, key=lambda g: groups[g])
+        # algorithmic work per launch (one layer), SURVEY.md 8(d) / DESIGN.md section 6: 1 FMA = 2 flop.
+        # dense groups = gram kernel + tensor-core chain; n_out is N_phi for the T-1 coefficient layers, 1 for the last
+        nout_avg = ((T - 1) * nphi + 1) / T
+        dense_flops = 2.0 * n * (n_q * H1 + H1 * H2 + H2 * nout_avg)
+        work = {"ms_edge_fwd": ("alu", 2.0 * E_rc * nphi * Na), "ms_edge_bwd": ("alu", 4.0 * E_rc * nphi * Na),
+                "ms_dense_fwd": ("tensor", dense_flops), "ms_dense_bwd": ("tensor", dense_flops),
+                "ms_rev_gather": ("hbm", float(E_rc) * (4 * nphi + 16 + 4) + n * (4 * nphi + 24))}
         sm_max = peaks.get("sm_max_mhz", 1965.0)
         alu_peak = N_SM * FP32_FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-        per_launch_ms = groups[dom] / T
-        achieved = flops[dom] / (per_launch_ms * 1e-3) / 1e12 if per_launch_ms > 0 else 0.0
-        roofline = {"bound": "alu", "kernel": dom.replace("ms_", ""), "achieved": achieved, "peak": alu_peak,
-                    "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": None,
-                    "peak_source": f"148 SM x 128 FP32 FMA lanes x 2 x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
-                    "ms_per_launch": per_launch_ms, "launches_per_step": T,
-                    "ms_per_step_by_group": {k.replace("ms_", ""): v for k, v in groups.items()}}
+        # TF32 peak = measured BF16 dense peak x the guide's nominal TF32/BF16 ratio (1.13 / 2.25 PFLOP/s);
+        # the sustained figure, because the kernel is timed inside a long step
+        tf32_peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * 0.5
+        peak_of = {"alu": (alu_peak, "TFLOP/s", f"148 SM x 128 FP32 FMA lanes x 2 x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)"),
+                   "tensor": (tf32_peak, "TFLOP/s", f"0.5 x {peaks['_source']} sustained BF16 cuBLAS peak (TF32 nominal ratio)"),
+                   "hbm": (peaks["hbm_gbs"], "GB/s", f"{peaks['_source']} HBM copy bandwidth")}
+        traffic = load_traffic(args.config)
+
+        def roof(g):
+            bound, amount = work[g]
+            ms = groups[g] / T
+            peak, unit, src = peak_of[bound]
+            ach = amount / (ms * 1e-3) / (1e9 if bound == "hbm" else 1e12) if ms > 0 else 0.0
+            return {"bound": bound, "kernel": g.replace("ms_", ""), "achieved": ach, "peak": peak, "unit": unit,
+                    "frac": ach / peak, "traffic": traffic.get(g.replace("ms_", "")), "peak_source": src,
+                    "ms_per_launch": ms, "launches_per_step": T}
+
+        dom = max(work, key=lambda g: groups[g])
+        roofline = roof(dom)
+        roofline["ms_per_step_by_group"] = {k.replace("ms_", ""): v for k, v in groups.items()}
+        roofline["other_kernels"] = [roof(g) for g in work if g != dom]
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
