@@ -44,6 +44,24 @@ def load_peaks():
             "_source": "fallback"}
 
 
+def max_over_ranks(value: float, device: str = "cuda") -> float:
+    """Replicas only: the one cross-rank step of the bench is the max of the per-rank
+    device times, so that `value` = (units all ranks processed) / (slowest rank's time)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(n_units_per_rank: int, steps: int, ms_total_local: float, world: int, device: str = "cuda"):
+    """(whole-job units/s, ms per step) from each rank's locally timed region."""
+    ms = max_over_ranks(ms_total_local, device)
+    return world * n_units_per_rank * steps / (ms * 1e-3), ms / steps
+
+
 def load_traffic(k: int) -> dict:
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture) of
     the kernel groups, from the committed profile summary; only valid for the config it was captured on."""
@@ -223,15 +241,13 @@ def main():
     ev1.record(stream)
     torch.cuda.synchronize()
     ms_total = ev0.elapsed_time(ev1)
+    value, ms_step = aggregate_throughput(n, K, ms_total, world)
     if world > 1:
-        tmax = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
         dist.barrier()
-        ms_total = float(tmax.item())
+    ms_total = ms_step * K
     clocks = sampler.stop()
     s1 = m.stats()
     m.set_profiling(False)
-    value = world * n * K / (ms_total * 1e-3)
 
     # ---------------- end-to-end leg: host buffers through the C ABI ----------------
     # replay: positions of an MD trajectory advanced on the host side of the boundary (pinned memory);
@@ -251,10 +267,7 @@ def main():
         m.energy_forces(pos_np, box, E_np, F_np)              # H2D pos, kernels, D2H E/F, stream sync
         vel_h += 0.5 * dt_fs * acc * inv_m_h * F_np
     t_e2e = time.perf_counter() - t0
-    if world > 1:
-        tt = torch.tensor([t_e2e], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_e2e = float(tt.item())
+    t_e2e = max_over_ranks(t_e2e)
     e2e = {"value": world * n * Ke / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(n * 24),
            "d2h_bytes_per_step": int(n * 24 + 8), "steps": Ke}
 
@@ -306,7 +319,8 @@ def main():
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "working set (compact edge list + stash, >300 MB) exceeds the 126 MB L2; no flush needed",
                            "rebuilds_in_timed_region": s1["n_rebuilds"] - s0["n_rebuilds"],
-                           "n_edges_rc": E_rc, "n_edges_list": s1["n_edges_list"], "n_ext": s1["n_ext"]},
+                           "n_edges_rc": E_rc, "n_edges_list": s1["n_edges_list"], "n_ext": s1["n_ext"],
+                           "device_bytes": s1["bytes_device"]},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": s1["n_launches"] - s0["n_launches"],
                 "roofline": roofline}
         if not args.no_cpu_baseline:

@@ -517,12 +517,36 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
     h->E_rc = n_rc;
     if (n_rc > h->cap_rc) {
         const int64_t cap = n_rc + n_rc / 16 + 1024;
+        dev_free(h, h->kappa);
         RC(dev_ensure(h, h->col_rc, sizeof(uint32_t) * (size_t)cap));
         RC(dev_ensure(h, h->rev_rc, sizeof(uint32_t) * (size_t)cap));
         RC(dev_ensure(h, h->geom, sizeof(float4) * (size_t)cap));
         RC(dev_ensure(h, h->gst, sizeof(float4) * (size_t)cap));
-        RC(dev_ensure(h, h->kappa, sizeof(float) * (size_t)cap * md.nphip));
+        // kappa stash (4 N_phi bytes per edge, one layer live): whole if it fits into what is left of the device
+        // memory, else in chunks of atoms -- k_edge_bwd / k_rev_gather then run once per chunk (config 5)
+        const size_t whole = sizeof(float) * (size_t)cap * md.nphip;
+        size_t free_b = 0, total_b = 0;
+        CU(h, cudaMemGetInfo(&free_b, &total_b));
+        const size_t budget = free_b > ((size_t)3 << 30) ? free_b - ((size_t)3 << 30) : free_b / 2;
+        int C = 1;
+        if (const char *e = getenv("REANN_STASH_CHUNKS")) C = std::max(1, atoi(e));
+        else while (C < 64 && (C == 1 ? whole : whole / C + whole / (8 * C)) > budget) ++C;
+        h->stash_chunks = C;
+        RC(dev_ensure(h, h->kappa, C == 1 ? whole : whole / C + whole / (8 * C)));
         h->cap_rc = cap;
+    }
+    // atom / edge ranges of the stash chunks
+    const int C = (N > 0) ? h->stash_chunks : 1;
+    std::vector<int64_t> ch_atom((size_t)C + 1, 0), ch_edge((size_t)C + 1, 0);
+    ch_atom[(size_t)C] = N; ch_edge[(size_t)C] = n_rc;
+    if (C > 1) {
+        for (int c = 1; c < C; ++c) ch_atom[(size_t)c] = ((N * c / C) + 3) & ~(int64_t)3;
+        for (int c = 1; c < C; ++c)
+            CU(h, cudaMemcpyAsync(&ch_edge[(size_t)c], (const int64_t *)h->rc_ptr.p + ch_atom[(size_t)c], 8, cudaMemcpyDeviceToHost, h->stream));
+        CU(h, cudaStreamSynchronize(h->stream));
+        int64_t widest = 0;
+        for (int c = 0; c < C; ++c) widest = std::max(widest, ch_edge[(size_t)c + 1] - ch_edge[(size_t)c]);
+        RC(dev_ensure(h, h->kappa, sizeof(float) * (size_t)widest * md.nphip));
     }
     const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
     launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
@@ -577,15 +601,21 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, gram_tiles, h->n_tiles, b + t * bstride, (const float *)h->Qbuf.p,
                         (float *)h->bbar.p);
         mk.mark(6);
-        rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
-                                (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
-                                (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
-                                (float4 *)h->gst.p, (double *)h->Fc.p, virial ? (double *)h->vir_part.p : nullptr,
-                                h->n_vir_blocks);
-        if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
-        mk.mark(7);
-        launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
-                          (const float4 *)h->gst.p, md.nphip, t >= 1, (float *)h->cbar.p, (double *)h->Fc.p);
+        for (int c = 0; c < C; ++c) {
+            if (c > 0) mk.mark(6);
+            rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
+                                    (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
+                                    (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
+                                    (float4 *)h->gst.p, (double *)h->Fc.p, virial ? (double *)h->vir_part.p : nullptr,
+                                    ch_atom[(size_t)c], ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
+            if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
+            mk.mark(7);
+            // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after
+            if (t >= 1 || c == C - 1)
+                launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
+                                  (const float4 *)h->gst.p, md.nphip, t >= 1, (float *)h->cbar.p, (double *)h->Fc.p,
+                                  ch_edge[(size_t)c], ch_edge[(size_t)c + 1], c == C - 1, c > 0);
+        }
     }
     // ---- outputs (A12) ----
     mk.mark(8);

@@ -124,10 +124,11 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
                     const float *alpha, const float *bbar, float *kappa, float4 *gst, double *Fc, double *vir_part,
-                    int n_vir_blocks);
+                    int64_t a0, int64_t a1, int64_t e_lo /* atoms [a0, a1), a0 % 4 == 0; kappa holds edges from e_lo on */);
 int edge_bwd_blocks(int64_t N);
 void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *rev_rc,
-                       const float *kappa, const float4 *gst, int nphip, int want_cbar, float *cbar, double *Fc);
+                       const float *kappa, const float4 *gst, int nphip, int want_cbar, float *cbar, double *Fc,
+                       int64_t e_lo, int64_t e_hi, int do_forces, int accumulate /* kappa holds edges [e_lo, e_hi) */);
 void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, const double *Fc, const float *Ei,
                    const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
                    double *Ei_sorted, double *scratch);

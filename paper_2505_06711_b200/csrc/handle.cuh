@@ -49,6 +49,7 @@ struct reann {
     DevBuf rc_ptr;                // int64 [N+1]
     DevBuf col_rc, geom, rev_rc;  // uint32 / float4 / uint32 [cap_rc]
     int64_t cap_rc = 0, E_rc = 0;
+    int stash_chunks = 1;         // kappa stash held for 1/stash_chunks of the atoms at a time (memory-limited systems)
     DevBuf c_ext;                 // float [T][n_ext][nphip]
     DevBuf b;                     // float [T][N][NB]
     DevBuf z_stash;               // float [T][N][zs]  (z1 | z2 pre-activations)

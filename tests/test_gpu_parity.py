@@ -255,3 +255,42 @@ def test_full_size_config3_sampled(R):
     assert np.abs(Ei[sel][in_e] - ref["Ei"][in_e]).max() <= 4e-6 * max(1.0, np.abs(ref["Ei"][in_e]).max())
     assert np.abs(F[sel][in_f] - ref["F"][in_f]).max() <= F_TOL
     m.close()
+
+
+def test_mma_edge_backward_variant_parity():
+    """REANN_EDGE=mma (mma.sync 3xTF32 version of the edge backward kernel; the switch is read once per
+    process, hence the subprocess): same parity gates as the default FP32 ALU kernel."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import sys; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+        "import gen, oracle\nimport paper_2505_06711_b200 as R\nfrom gpu_util import check_parity\n"
+        "for k, kw in ((3, dict(n_mol=700)), (2, dict(n_mol=300))):\n"
+        "    cfg = gen.make_config(k, **kw)\n"
+        "    m = R.Reann.from_config(cfg); m.build_neighbors(cfg['pos'], cfg['box'])\n"
+        "    out = m.energy_forces(cfg['pos'], cfg['box'])\n"
+        "    ref = oracle.energy_forces(cfg['blob'], cfg['species'], cfg['pos'], cfg['box'])\n"
+        "    check_parity(out, ref, m.n, 'mma cfg%%d' %% k); m.close()\n" % (root, os.path.join(root, "tests")))
+    r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, REANN_EDGE="mma"), capture_output=True,
+                       text=True, timeout=600)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("[parity] mma") == 2
+
+
+def test_stash_chunks_memory_limited_path(R, monkeypatch):
+    """Config 5 needs the kappa stash in chunks of atoms to fit 180 GB; REANN_STASH_CHUNKS forces the same code
+    path on a small system: parity with the oracle, and the same result as the unchunked run up to the
+    summation order of cbar."""
+    cfg = gen.make_config(5, n_mol=900)
+    m1, (E1, F1, V1) = run(R, cfg)
+    m1.close()
+    monkeypatch.setenv("REANN_STASH_CHUNKS", "3")
+    m3, out3 = run(R, cfg)
+    ref = oracle.energy_forces(cfg["blob"], cfg["species"], cfg["pos"], cfg["box"])
+    check_parity(out3, ref, m3.n, "stash chunks = 3")
+    E3, F3, V3 = out3
+    assert abs(E3 - E1) <= 1e-9 * max(1.0, abs(E1)) * m3.n
+    assert np.abs(F3 - F1).max() <= 2e-5 and np.abs(V3 - V1).max() <= 1e-5 * max(1.0, np.abs(V1).max())
+    E3b, F3b, _ = m3.energy_forces(cfg["pos"], cfg["box"])       # deterministic for a fixed chunk count
+    assert E3b == E3 and (F3b == F3).all()
+    m3.close()
