@@ -315,6 +315,132 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
     }
 }
 
+// ---- warp-level tensor-core helpers (mma.sync TF32, 3xTF32 splitting) ----
+__device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void split_bits(float x, uint32_t &hi, uint32_t &lo) {
+    // hi rounded to nearest TF32, lo = x - hi exact (<= 13 significant bits, of which the MMA reads the top 11):
+    // |x - hi - lo_read| <= 2^-22 |x|
+    hi = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;
+    lo = __float_as_uint(x - __uint_as_float(hi));
+}
+
+// ------------------------------------------------------------------------------------------ A5 (MMA)
+// Edge forward with the neighbour sum on the tensor cores: b_i[n,a] = sum_e X[e,n] A[e,a] is a
+// (N_phi x edges) x (edges x N_a) product with K = the edges of atom i. Warp per atom, rounds of 32 edges:
+// phase 1 as in k_edge_fwd (edge record / monomials one edge per lane, x_e[n] by N_phi/4 lanes per edge)
+// but staged transposed, XT[n][e] | AT[a][e] with a row stride of 36 floats, so that both the scalar
+// stores and the mma.sync fragment loads are conflict-free; phase 2: four K = 8 steps of
+// mma.sync.m16n8k8 TF32 (3xTF32: lo.hi + hi.lo + hi.hi into a fresh accumulator per step, summed in FP32
+// registers). Needs N_phi = 16.
+template <int NA>
+struct FwdMma {
+    static constexpr int NAP = (NA + 7) & ~7, AT = NAP / 8, TS = 36;
+    static constexpr int ROWS = 16 + NAP, SMEM = EW * ROWS * TS * 4;
+};
+
+template <int NA>
+__global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64_t *__restrict__ rc_ptr,
+                                                          const uint32_t *__restrict__ col_rc,
+                                                          const float4 *__restrict__ geom,
+                                                          const float *__restrict__ c_ext, RadialTab rt,
+                                                          float *__restrict__ b) {
+    using C = FwdMma<NA>;
+    constexpr int NPHIP = 16, NAP = C::NAP, AT = C::AT, TS = C::TS;
+    extern __shared__ __align__(16) float smem_f[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g8 = lane >> 2, t4 = lane & 3;
+    float *XT = smem_f + (size_t)warp * C::ROWS * TS, *AT_s = XT + 16 * TS;
+    const int64_t i = (int64_t)blockIdx.x * EW + warp;
+    if (i >= N) return;
+    const int64_t beg = rc_ptr[i], end = rc_ptr[i + 1];
+    float acc[AT][4];
+#pragma unroll
+    for (int at = 0; at < AT; ++at) acc[at][0] = acc[at][1] = acc[at][2] = acc[at][3] = 0.f;
+    float4 g_nx = make_float4(0.f, 0.f, 0.f, 0.f);
+    uint32_t cj_nx = 0;
+    if (beg + lane < end) { g_nx = geom[beg + lane]; cj_nx = col_rc[beg + lane]; }
+    for (int64_t e0 = beg; e0 < end; e0 += 32) {
+        // ---- phase 1a: one edge per lane (the next round's record is fetched one round ahead) ----
+        const int64_t e = e0 + lane;
+        const bool have = e < end;
+        const float4 g = g_nx;
+        const uint32_t cj = cj_nx;
+        if (e + 32 < end) { g_nx = geom[e + 32]; cj_nx = col_rc[e + 32]; }
+        float fc = 0.f;
+        {
+            float A[NAP];
+#pragma unroll
+            for (int a = 0; a < NAP; ++a) A[a] = 0.f;
+            if (have) {
+                fc = 0.5f + 0.5f * cospif(g.w * rt.inv_rc);
+                monomials<NA>(g.x, g.y, g.z, A);
+            }
+#pragma unroll
+            for (int a = 0; a < NAP; ++a) AT_s[a * TS + lane] = A[a];       // zeros for the lanes past the row's end
+        }
+        // ---- phase 1b: four lanes per edge, one float4 of c_j each ----
+        {
+            const int part = lane & 3;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int rr = r * 8 + (lane >> 2);
+                const uint32_t cje = __shfl_sync(0xffffffffu, cj, rr);
+                const float we = __shfl_sync(0xffffffffu, g.w, rr);
+                const float fce = __shfl_sync(0xffffffffu, fc, rr);
+                float4 xv = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (e0 + rr < end) {
+                    const int sj = cje >> COL_SPECIES_SHIFT;
+                    const float4 cv = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cje & COL_IDX_MASK) * NPHIP)[part];
+                    const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[part];
+                    const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[part];
+                    float d;
+                    d = we - rc4.x; xv.x = cv.x * (exp2f(-al4.x * d * d) * fce);
+                    d = we - rc4.y; xv.y = cv.y * (exp2f(-al4.y * d * d) * fce);
+                    d = we - rc4.z; xv.z = cv.z * (exp2f(-al4.z * d * d) * fce);
+                    d = we - rc4.w; xv.w = cv.w * (exp2f(-al4.w * d * d) * fce);
+                }
+                float *dst = XT + (part * 4) * TS + rr;
+                dst[0] = xv.x; dst[TS] = xv.y; dst[2 * TS] = xv.z; dst[3 * TS] = xv.w;
+            }
+        }
+        __syncwarp();
+        // ---- phase 2: K = 8 edges per step ----
+        const int nks = (int)((end - e0 + 7) >> 3) < 4 ? (int)((end - e0 + 7) >> 3) : 4;
+#pragma unroll 1
+        for (int ks = 0; ks < nks; ++ks) {
+            const float *xa = XT + g8 * TS + ks * 8 + t4;
+            uint32_t ah[4], al[4];
+            split_bits(xa[0], ah[0], al[0]); split_bits(xa[8 * TS], ah[1], al[1]);
+            split_bits(xa[4], ah[2], al[2]); split_bits(xa[8 * TS + 4], ah[3], al[3]);
+#pragma unroll
+            for (int at = 0; at < AT; ++at) {
+                const float *ba = AT_s + (at * 8 + g8) * TS + ks * 8 + t4;
+                uint32_t bh0, bl0, bh1, bl1;
+                split_bits(ba[0], bh0, bl0); split_bits(ba[4], bh1, bl1);
+                float d[4] = {0.f, 0.f, 0.f, 0.f};
+                mma_tf32(d, al, bh0, bh1);
+                mma_tf32(d, ah, bl0, bl1);
+                mma_tf32(d, ah, bh0, bh1);
+                acc[at][0] += d[0]; acc[at][1] += d[1]; acc[at][2] += d[2]; acc[at][3] += d[3];
+            }
+        }
+        __syncwarp();
+    }
+    // C fragment: rows n = g, g + 8; columns a = at*8 + 2t, +1
+    float *bi = b + i * (int64_t)(NPHIP * NA);
+#pragma unroll
+    for (int at = 0; at < AT; ++at) {
+        const int a = at * 8 + 2 * t4;
+        if (a < NA) {
+            *reinterpret_cast<float2 *>(bi + g8 * NA + a) = make_float2(acc[at][0], acc[at][1]);
+            *reinterpret_cast<float2 *>(bi + (g8 + 8) * NA + a) = make_float2(acc[at][2], acc[at][3]);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------ A10
 // Warp per atom, one edge per lane; bbar_i is broadcast from shared memory, S_n and P_a stay in the
 // lane's registers, so there is no cross-lane reduction per edge. Orbitals are recomputed (nothing
@@ -459,16 +585,6 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
 // Warp per atom, rounds of 32 edges: (1) one edge per lane: radial functions, monomials -> shared memory
 // rows (X | A); (2) two M = 16 edge tiles through the MMAs, S | P back to shared memory; (3) one edge
 // per lane again (R_n, y_n kept in registers): radial part, kappa_e, sum_a P_a grad A_a, g_e.
-__device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void split_bits(float x, uint32_t &hi, uint32_t &lo) {
-    hi = __float_as_uint(x) & 0xFFFFE000u;
-    lo = __float_as_uint(x - __uint_as_float(hi));   // exact; the MMA reads its top 19 bits
-}
-
 template <int NPHIP, int NA>
 struct BwdMma {
     static constexpr int NAP = (NA + 7) & ~7, NT = NPHIP / 8, AT = NAP / 8;
@@ -834,6 +950,21 @@ void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, i
     if (work > 0) LAUNCH(ctx, k_ghost_gather, div_up(work, 256), 256, 0, c_ext, xrec, N, n_ext, nphip);
 }
 
+// REANN_EDGE_FWD=simt keeps the FP32 ALU forward kernel where the mma.sync one applies (N_phi = 16, L >= 2)
+static bool edge_fwd_mma_enabled() {
+    static int v = -1;
+    if (v < 0) { const char *e = getenv("REANN_EDGE_FWD"); v = (e && strcmp(e, "simt") == 0) ? 0 : 1; }
+    return v == 1;
+}
+
+template <int NA>
+static int run_edge_fwd_mma(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
+                            const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
+    using C = FwdMma<NA>;
+    LAUNCH(ctx, (k_edge_fwd_mma<NA>), div_up(N, EW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    return REANN_OK;
+}
+
 template <int NPHIP, int NA, int PN, int PA>
 static int run_edge_fwd(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
                         const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
@@ -862,6 +993,9 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
                     const float *alpha, float *b) {
     if (N <= 0) return REANN_OK;
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
+    if (md.nphip == 16 && md.Na >= 10 && edge_fwd_mma_enabled())
+        return md.Na == 20 ? run_edge_fwd_mma<20>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b)
+                           : run_edge_fwd_mma<10>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
 #define M(NP, NA_, PN_, PA_) return run_edge_fwd<NP, NA_, PN_, PA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
     EDGE_DISPATCH(M)
 #undef M

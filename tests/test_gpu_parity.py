@@ -258,8 +258,9 @@ def test_full_size_config3_sampled(R):
 
 
 def test_mma_edge_backward_variant_parity():
-    """REANN_EDGE=mma (mma.sync 3xTF32 version of the edge backward kernel; the switch is read once per
-    process, hence the subprocess): same parity gates as the default FP32 ALU kernel."""
+    """The non-default edge kernels: REANN_EDGE=mma (mma.sync 3xTF32 version of the edge backward kernel) together
+    with REANN_EDGE_FWD=simt (FP32 ALU forward kernel where the mma.sync one is the default). The switches are
+    read once per process, hence the subprocess. Same parity gates as the default pair."""
     import os, subprocess, sys
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     code = (
@@ -271,7 +272,8 @@ def test_mma_edge_backward_variant_parity():
         "    out = m.energy_forces(cfg['pos'], cfg['box'])\n"
         "    ref = oracle.energy_forces(cfg['blob'], cfg['species'], cfg['pos'], cfg['box'])\n"
         "    check_parity(out, ref, m.n, 'mma cfg%%d' %% k); m.close()\n" % (root, os.path.join(root, "tests")))
-    r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, REANN_EDGE="mma"), capture_output=True,
+    r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, REANN_EDGE="mma", REANN_EDGE_FWD="simt"),
+                       capture_output=True,
                        text=True, timeout=600)
     assert r.returncode == 0, r.stdout + r.stderr
     assert r.stdout.count("[parity] mma") == 2
