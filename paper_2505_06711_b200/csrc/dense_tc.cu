@@ -52,11 +52,13 @@ constexpr int SM_A = 0, SM_B = NASLOT * A_SLOT, SM_BAR = SM_B + NSTAGE * B_SLOT;
 constexpr int SM_TOTAL = SM_BAR + 256;
 constexpr uint32_t A_LBO = TM * 16;
 constexpr int NCOMPUTE = 256, NTHREADS = NCOMPUTE + 32, CTL_WARP = 8;
-constexpr uint32_t COL_BUF = 128;      // TMEM columns per group buffer (two buffers)
+constexpr uint32_t COL_BUF = 128;      // TMEM columns per group buffer
+constexpr int NBUF = 3;                // group buffers: one filling, one complete, one being drained
+constexpr uint32_t TMEM_COLS = 512;    // allocation (power of two >= NBUF * COL_BUF)
 
 // barrier slots (8 bytes each) in the barrier area
 enum { BAR_BFULL = 0, BAR_MMA = 3, BAR_AFULL = 6, BAR_AH = 9, BAR_QFULL = 13, BAR_QEMPTY = 15, BAR_DFULL = 17,
-       BAR_DEMPTY = 19, BAR_ARES = 21, BAR_COUNT = 22 };
+       BAR_DEMPTY = 20, BAR_ARES = 23, BAR_COUNT = 24 };
 
 // Optional timeline trace of one CTA (development aid, compiled only with -DREANN_TC_TRACE):
 // role 0 = control thread, 1 = compute thread 0; slot k = clock64().
@@ -181,6 +183,8 @@ __device__ __forceinline__ uint32_t tc_prologue(unsigned char *smem, uint32_t *t
         for (int d = 0; d < 2; ++d) {
             mbar_init(bar0 + 8 * (BAR_QFULL + d), 1);
             mbar_init(bar0 + 8 * (BAR_QEMPTY + d), NCOMPUTE);
+        }
+        for (int d = 0; d < NBUF; ++d) {
             mbar_init(bar0 + 8 * (BAR_DFULL + d), 1);
             mbar_init(bar0 + 8 * (BAR_DEMPTY + d), NCOMPUTE);
         }
@@ -188,7 +192,7 @@ __device__ __forceinline__ uint32_t tc_prologue(unsigned char *smem, uint32_t *t
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == CTL_WARP) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_s)), "r"(256u)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_s)), "r"(TMEM_COLS)
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -201,7 +205,7 @@ __device__ __forceinline__ void tc_epilogue(uint32_t tmem) {
     tc_fence_before();
     __syncthreads();
     if ((int)(threadIdx.x >> 5) == CTL_WARP)
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(256u) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(TMEM_COLS) : "memory");
 }
 
 // ---- control-thread helpers ----
@@ -216,11 +220,11 @@ struct Ctl {
         mbar_expect_tx(bar(BAR_BFULL + s), bytes);
         bulk_g2s(b0 + (uint32_t)s * B_SLOT, src, bytes, bar(BAR_BFULL + s));
     }
-    // One K chunk = one accumulation group (step i, group buffer i & 1):
+    // One K chunk = one accumulation group (step i, group buffer i % NBUF):
     //   D[:, 0:n) = A_lo B_hi^T + A_hi B_lo^T  (4 x K = 8),  then  D += A_hi B_hi^T  (4 x K = 8)
     __device__ __forceinline__ void mma_chunk(int i, int a_slot, int n_rows) const {
-        const int s = i % NSTAGE, d = i & 1;
-        if (i >= 2) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((i >> 1) - 1) & 1));
+        const int s = i % NSTAGE, d = i % NBUF;
+        if (i >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((i / NBUF) - 1) & 1));
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t idesc = make_idesc(n_rows);
@@ -250,8 +254,8 @@ struct Ctl {
 // acc[0..CW) += group buffer of step g, columns [col0, col0 + CW) of this thread's TMEM lane
 template <int CW>
 __device__ __forceinline__ void drain_group(float *acc, uint32_t bar0, uint32_t tl, int g, int col0, bool read) {
-    const int d = g & 1;
-    mbar_wait(bar0 + 8 * (BAR_DFULL + d), (uint32_t)((g >> 1) & 1));
+    const int d = g % NBUF;
+    mbar_wait(bar0 + 8 * (BAR_DFULL + d), (uint32_t)((g / NBUF) & 1));
     tc_fence_after();
     if (read) {
         const uint32_t ta = tl + COL_BUF * (uint32_t)d + (uint32_t)col0;

@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *
                                                       const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, float *__restrict__ Q, int nphi,
                                                       int npairs, int NPp, int KQ) {
-    constexpr int NB = NPHIP * NA, JMAX = (NPHIP * (NPHIP + 1) / 2 + 31) / 32, LMAX = l_of(NA - 1);
+    constexpr int NB = NPHIP * NA, LMAX = l_of(NA - 1);
     extern __shared__ __align__(16) float sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, QS = KQ + 4;
     float *bs = sm + warp * NB, *qs = sm + GW * NB + warp * QS;
@@ -84,22 +84,39 @@ __global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *
 #pragma unroll
         for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
         __syncwarp();
+        // 2 x 2 blocks of row pairs: block (I <= J) = rows {2I, 2I+1} x {2J, 2J+1}; four rows loaded for (up to)
+        // four products -- half the shared-memory operand traffic of one pair per lane
+        constexpr int NBK = NPHIP / 2, NBLOCKS = NBK * (NBK + 1) / 2;
 #pragma unroll
-        for (int j = 0; j < JMAX; ++j) {
-            int pi = lane + 32 * j;
-            if (pi < npairs) {
-                // pair index -> (n, n') with n <= n'
-                int lo = 0, rem = pi;
-                while (rem >= nphi - lo) { rem -= nphi - lo; ++lo; }
-                float x[NA], y[NA], s[LMAX + 1];
-                load_row<NA>(bs + lo * NA, x);
-                load_row<NA>(bs + (lo + rem) * NA, y);
+        for (int j = 0; j < (NBLOCKS + 31) / 32; ++j) {
+            const int bi = lane + 32 * j;
+            if (bi < NBLOCKS) {
+                int I = 0, rem = bi;
+                while (rem >= NBK - I) { rem -= NBK - I; ++I; }
+                const int J = I + rem, n0 = 2 * I, m0 = 2 * J;
+                float s[4][LMAX + 1];                       // (n0,m0) (n0,m1) (n1,m0) (n1,m1)
 #pragma unroll
-                for (int l = 0; l <= LMAX; ++l) s[l] = 0.f;
+                for (int k = 0; k < 4; ++k)
 #pragma unroll
-                for (int a = 0; a < NA; ++a) s[l_of(a)] = fmaf(mu_of(a) * x[a], y[a], s[l_of(a)]);
+                    for (int l = 0; l <= LMAX; ++l) s[k][l] = 0.f;
+                float x0[NA], x1[NA], y0[NA], y1[NA];
+                load_row<NA>(bs + n0 * NA, x0); load_row<NA>(bs + (n0 + 1) * NA, x1);
+                load_row<NA>(bs + m0 * NA, y0); load_row<NA>(bs + (m0 + 1) * NA, y1);
 #pragma unroll
-                for (int l = 0; l <= LMAX; ++l) qs[l * NPp + pi] = s[l];
+                for (int a = 0; a < NA; ++a) {
+                    const float u0 = mu_of(a) * x0[a], u1 = mu_of(a) * x1[a];
+                    s[0][l_of(a)] = fmaf(u0, y0[a], s[0][l_of(a)]); s[1][l_of(a)] = fmaf(u0, y1[a], s[1][l_of(a)]);
+                    s[2][l_of(a)] = fmaf(u1, y0[a], s[2][l_of(a)]); s[3][l_of(a)] = fmaf(u1, y1[a], s[3][l_of(a)]);
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int n = n0 + (k >> 1), m = m0 + (k & 1);
+                    if (n <= m && m < nphi) {                // diagonal block: (n1, m0) is the mirror of (n0, m1)
+                        const int pi = n * nphi - (n * (n - 1)) / 2 + (m - n);
+#pragma unroll
+                        for (int l = 0; l <= LMAX; ++l) qs[l * NPp + pi] = s[k][l];
+                    }
+                }
             }
         }
     }
@@ -132,7 +149,7 @@ struct BwdCfg {
 };
 
 template <int NPHIP, int NA>
-__global__ void __launch_bounds__(GW * 32) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
+__global__ void __launch_bounds__(GW * 32, 4) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
                                                       const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, const float *__restrict__ Qbar,
                                                       float *__restrict__ bbar, int nphi, int NPp, int KQ) {
