@@ -98,17 +98,39 @@ __global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict_
     if (i >= N) return;
     const XRec me = xrec[i];
     const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1], c0 = rc_ptr[i];
-    for (int64_t e = r0 + lane; e < r1; e += 32) {
-        const uint16_t rk = rank16[e];
-        if (rk == 0xFFFF) continue;
-        const int32_t j = col[e];
-        const XRec o = xrec[j];
-        double dx, dy, dz;
-        const double d2 = edge_d2(me, o, Lx, Ly, Lz, &dx, &dy, &dz);
-        const int64_t ce = c0 + rk;
-        col_rc[ce] = (uint32_t)j | ((uint32_t)o.species << COL_SPECIES_SHIFT);
-        geom[ce] = make_float4((float)dx, (float)dy, (float)dz, (float)sqrt(d2));
-        rev_rc[ce] = (uint32_t)(rc_ptr[o.owner] + rank16[rev[e]]);
+    // four list entries per lane and iteration: their (dependent) gathers are all in flight together
+    constexpr int U = 4;
+    for (int64_t eb = r0 + lane; eb < r1; eb += 32 * U) {
+        uint16_t rk[U];
+        int32_t j[U];
+        uint32_t rv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t e = eb + 32 * u;
+            rk[u] = e < r1 ? rank16[e] : (uint16_t)0xFFFF;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (rk[u] != 0xFFFF) { j[u] = col[eb + 32 * u]; rv[u] = rev[eb + 32 * u]; }
+        XRec o[U];
+        uint16_t rrk[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (rk[u] != 0xFFFF) { o[u] = xrec[j[u]]; rrk[u] = rank16[rv[u]]; }
+        int64_t base[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (rk[u] != 0xFFFF) base[u] = rc_ptr[o[u].owner];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (rk[u] != 0xFFFF) {
+                double dx, dy, dz;
+                const double d2 = edge_d2(me, o[u], Lx, Ly, Lz, &dx, &dy, &dz);
+                const int64_t ce = c0 + rk[u];
+                col_rc[ce] = (uint32_t)j[u] | ((uint32_t)o[u].species << COL_SPECIES_SHIFT);
+                geom[ce] = make_float4((float)dx, (float)dy, (float)dz, (float)sqrt(d2));
+                rev_rc[ce] = (uint32_t)(base[u] + rrk[u]);
+            }
     }
 }
 
