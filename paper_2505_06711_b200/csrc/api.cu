@@ -175,7 +175,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
     ModelDims &md = h->md;
     md.S = v.S; md.T = T; md.L = L; md.nphi = n_gauss; md.nphip = (n_gauss + 3) & ~3;
     md.Na = (L + 1) * (L + 2) * (L + 3) / 6; md.NB = md.nphip * md.Na; md.norb = v.norb;
-    md.npairs = n_gauss * (n_gauss + 1) / 2; md.NPp = (md.npairs + 15) & ~15; md.nqp = (L + 1) * md.NPp;
+    md.npairs = n_gauss * (n_gauss + 1) / 2; md.NPp = md.npairs; md.nqp = ((L + 1) * md.NPp + 15) & ~15;
     md.K1 = (md.nqp + 31) & ~31;
     {
         const char *e = getenv("REANN_DENSE");

@@ -70,7 +70,7 @@ struct LayerDims {
 
 struct ModelDims {
     int S, T, L, nphi, nphip, Na, NB, norb;
-    int npairs, NPp, nqp; // pairs n<=n' per l; padded to 16; (L+1)*NPp
+    int npairs, NPp, nqp; // pairs n<=n' per l; stride of an l block in Q (= npairs); (L+1)*NPp rounded up to 16
     int K1;               // nqp rounded up to 32 (K extent of the tensor-core GEMM over Q)
     double rc, skin;
 };
