@@ -357,7 +357,8 @@ __device__ __forceinline__ void split_bits(float x, uint32_t &hi, uint32_t &lo) 
 // but staged transposed, XT[n][e] | AT[a][e] with a row stride of 36 floats, so that both the scalar
 // stores and the mma.sync fragment loads are conflict-free; phase 2: four K = 8 steps of
 // mma.sync.m16n8k8 TF32 (3xTF32: lo.hi + hi.lo + hi.hi into a fresh accumulator per step, summed in FP32
-// registers). Needs N_phi = 16.
+// registers: accumulating the ~36 steps of an atom inside the MMA truncates like tcgen05 does and was measured
+// to cost 1.4e-6 eV/atom on config 2, above the 1e-6 gate). Needs N_phi = 16.
 template <int NA>
 struct FwdMma {
     static constexpr int NAP = (NA + 7) & ~7, AT = NAP / 8, TS = 36;
