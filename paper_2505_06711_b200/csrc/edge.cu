@@ -69,16 +69,23 @@ __global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict
     const XRec me = xrec[i];
     const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1];
     int cnt = 0;
-    for (int64_t eb = r0; eb < r1; eb += 32) {
-        const int64_t e = eb + lane;
-        bool in = false;
-        if (e < r1) {
-            double dx, dy, dz;
-            in = edge_d2(me, xrec[col[e]], Lx, Ly, Lz, &dx, &dy, &dz) < rc2;
-        }
-        const unsigned m = __ballot_sync(0xffffffffu, in);
-        if (e < r1) rank16[e] = in ? (uint16_t)(cnt + __popc(m & ((1u << lane) - 1))) : (uint16_t)0xFFFF;
-        cnt += __popc(m);
+    // two batches of 32 list entries per iteration: both gathers are in flight together
+    for (int64_t eb = r0; eb < r1; eb += 64) {
+        const int64_t e0 = eb + lane, e1 = e0 + 32;
+        int32_t j0 = 0, j1 = 0;
+        if (e0 < r1) j0 = col[e0];
+        if (e1 < r1) j1 = col[e1];
+        XRec o0 = me, o1 = me;
+        if (e0 < r1) o0 = xrec[j0];
+        if (e1 < r1) o1 = xrec[j1];
+        double dx, dy, dz;
+        const bool in0 = e0 < r1 && edge_d2(me, o0, Lx, Ly, Lz, &dx, &dy, &dz) < rc2;
+        const bool in1 = e1 < r1 && edge_d2(me, o1, Lx, Ly, Lz, &dx, &dy, &dz) < rc2;
+        const unsigned m0 = __ballot_sync(0xffffffffu, in0), m1 = __ballot_sync(0xffffffffu, in1);
+        if (e0 < r1) rank16[e0] = in0 ? (uint16_t)(cnt + __popc(m0 & ((1u << lane) - 1))) : (uint16_t)0xFFFF;
+        cnt += __popc(m0);
+        if (e1 < r1) rank16[e1] = in1 ? (uint16_t)(cnt + __popc(m1 & ((1u << lane) - 1))) : (uint16_t)0xFFFF;
+        cnt += __popc(m1);
     }
     if (lane == 0) rc_cnt[i] = cnt;
 }
