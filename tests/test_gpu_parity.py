@@ -257,6 +257,34 @@ def test_full_size_config3_sampled(R):
     m.close()
 
 
+def test_full_size_config4_sampled(R):
+    """Config 4 at full size (4 000 000 fcc atoms, T = 3 of the sweep): sampled E_i / F_k against the oracle on an
+    open cluster (receptive field T*rc), the per-atom neighbour count of the perturbed lattice,
+    and global invariants."""
+    cfg = gen.make_config(4, T=3)
+    m, (E, F, vir) = run(R, cfg)
+    n = m.n
+    assert n == 4_000_000
+    Ei = m.atomic_energies()
+    assert abs(Ei.sum() - E) <= 1e-9 * max(1.0, abs(E))
+    assert np.abs(F.sum(0)).max() <= 1e-6 * n
+    st = m.stats()
+    assert 77.5 * n < st["n_edges_list"] < 78.5 * n              # shells 12+6+24+12+24 within rc+skin = 6 A
+    assert 42 * n < st["n_edges_rc"] < 48 * n
+    T, rc = cfg["T"], cfg["rc"]
+    k0 = 2_345_678
+    centre = cfg["pos"][k0]
+    r_f, r_e = 3.0, 3.0 + T * rc
+    sel, cpos, cbox = open_cluster(cfg["pos"], cfg["species"], cfg["box"], centre, r_f + 2 * T * rc + 0.5)
+    ref = oracle.energy_forces(cfg["blob"], cfg["species"][sel], cpos, cbox)
+    d = np.linalg.norm(cpos - cpos[np.nonzero(sel == k0)[0][0]], axis=1)
+    in_e, in_f = d < r_e, d < r_f
+    assert in_f.sum() >= 10 and in_e.sum() >= 1000
+    assert np.abs(Ei[sel][in_e] - ref["Ei"][in_e]).max() <= 4e-6 * max(1.0, np.abs(ref["Ei"][in_e]).max())
+    assert np.abs(F[sel][in_f] - ref["F"][in_f]).max() <= F_TOL
+    m.close()
+
+
 def test_mma_edge_backward_variant_parity():
     """The non-default edge kernels: REANN_EDGE=mma (mma.sync 3xTF32 version of the edge backward kernel) together
     with REANN_EDGE_FWD=simt (FP32 ALU forward kernel where the mma.sync one is the default). The switches are
