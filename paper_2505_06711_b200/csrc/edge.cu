@@ -184,6 +184,17 @@ __device__ __forceinline__ void monomial_vjp(const float *A, const float *P, flo
     }
 }
 
+// Packed FP32 pairs: Blackwell's fma.rn.f32x2 (SASS FFMA2) does two FP32 FMAs per issue slot at the same FLOP
+// rate (measured 74 TFLOP/s either way), which halves the instruction count of the FMA loops below.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ void ffma2(f32x2 &c, f32x2 a, f32x2 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
+
 struct StashChunk { // reverse gather: kappa holds the edges [e_lo, e_hi); forces once; cbar = or +=
     int64_t e_lo, e_hi;
     int do_forces, accumulate;
@@ -522,10 +533,17 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
             float sn, cs;
             sincospif(g.w * rt.inv_rc, &sn, &cs);
             const float fc = 0.5f + 0.5f * cs, dfc = -0.5f * pi_rc * sn;
+            constexpr bool PAIRS = NA % 2 == 0;                   // (a, a+1) pairs never straddle a row of bbar_i
+            constexpr int NP2 = PAIRS ? NA / 2 : 1;
             float A[NA], P[NA];
             monomials<NA>(g.x, g.y, g.z, A);
 #pragma unroll
             for (int a = 0; a < NA; ++a) P[a] = 0.f;
+            f32x2 A2[NP2], P2[NP2];
+            if constexpr (PAIRS) {
+#pragma unroll
+                for (int a2 = 0; a2 < NP2; ++a2) { A2[a2] = pack2(A[2 * a2], A[2 * a2 + 1]); P2[a2] = pack2(0.f, 0.f); }
+            }
             // four rows n of bbar_i per outer iteration (one float4 of c_j / r_n / alpha_n / kappa);
             // the outer loop is kept rolled so that the shared-memory loads are not all hoisted.
             float radial = 0.f;
@@ -549,21 +567,44 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
                     Sn[u] = 0.f;
                 }
                 const float4 *bb4 = reinterpret_cast<const float4 *>(bb_s[warp] + n4 * 4 * NA);
+                if constexpr (PAIRS) {
+                    f32x2 S2[4], x2[4];
 #pragma unroll
-                for (int f4 = 0; f4 < NA; ++f4) { // 4 rows x NA values = NA float4
-                    const float4 v = bb4[f4];
-                    const float va[4] = {v.x, v.y, v.z, v.w};
+                    for (int u = 0; u < 4; ++u) { S2[u] = pack2(0.f, 0.f); x2[u] = pack2(xn[u], xn[u]); }
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const int f = f4 * 4 + u, nl = f / NA, a = f % NA;
-                        Sn[nl] = fmaf(va[u], A[a], Sn[nl]);
-                        P[a] = fmaf(va[u], xn[nl], P[a]);
+                    for (int f4 = 0; f4 < NA; ++f4) { // 4 rows x NA values = NA float4 = 2 NA pairs
+                        const float4 v = bb4[f4];
+                        const f32x2 v2[2] = {pack2(v.x, v.y), pack2(v.z, v.w)};
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const int f = f4 * 4 + 2 * h, nl = f / NA, a2 = (f % NA) / 2;
+                            ffma2(S2[nl], v2[h], A2[a2]);
+                            ffma2(P2[a2], v2[h], x2[nl]);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { float lo, hi; unpack2(S2[u], lo, hi); Sn[u] = lo + hi; }
+                } else {
+#pragma unroll
+                    for (int f4 = 0; f4 < NA; ++f4) {
+                        const float4 v = bb4[f4];
+                        const float va[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const int f = f4 * 4 + u, nl = f / NA, a = f % NA;
+                            Sn[nl] = fmaf(va[u], A[a], Sn[nl]);
+                            P[a] = fmaf(va[u], xn[nl], P[a]);
+                        }
                     }
                 }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) radial = fmaf(yn[u], Sn[u], radial);
                 if (want_kappa) kp[n4] = make_float4(Rn[0] * Sn[0], Rn[1] * Sn[1], Rn[2] * Sn[2], Rn[3] * Sn[3]);
                 cv = cvn;
+            }
+            if constexpr (PAIRS) {
+#pragma unroll
+                for (int a2 = 0; a2 < NP2; ++a2) unpack2(P2[a2], P[2 * a2], P[2 * a2 + 1]);
             }
             float gx, gy, gz;
             monomial_vjp<NA>(A, P, gx, gy, gz);
