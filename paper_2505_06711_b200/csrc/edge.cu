@@ -194,6 +194,8 @@ __device__ __forceinline__ f32x2 pack2(float lo, float hi) {
 }
 __device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ void ffma2(f32x2 &c, f32x2 a, f32x2 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
+__device__ __forceinline__ f32x2 fmadd2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 
 struct StashChunk { // reverse gather: kappa holds the edges [e_lo, e_hi); forces once; cbar = or +=
     int64_t e_lo, e_hi;
@@ -556,15 +558,22 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
                 const float cva[4] = {cv.x, cv.y, cv.z, cv.w}, rca[4] = {rc4.x, rc4.y, rc4.z, rc4.w},
                             ala[4] = {al4.x, al4.y, al4.z, al4.w};
                 float Rn[4], xn[4], yn[4], Sn[4];
+                // alpha2 = alpha*log2(e): d/dr exp(-alpha d^2) = -2 ln2 alpha2 d ex; two n per packed operation
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const float d = g.w - rca[u];
-                    const float ex = exp2f(-ala[u] * d * d);
-                    // alpha2 = alpha*log2(e): d/dr exp(-alpha d^2) = -2 ln2 alpha2 d ex
-                    Rn[u] = ex * fc;
-                    xn[u] = cva[u] * Rn[u];
-                    yn[u] = cva[u] * ((-1.3862943611198906f * ala[u] * d * fc + dfc) * ex);
-                    Sn[u] = 0.f;
+                for (int h = 0; h < 2; ++h) {
+                    const f32x2 al2 = pack2(ala[2 * h], ala[2 * h + 1]), c2 = pack2(cva[2 * h], cva[2 * h + 1]);
+                    const f32x2 d2 = fmadd2(pack2(rca[2 * h], rca[2 * h + 1]), pack2(-1.f, -1.f), pack2(g.w, g.w));
+                    const f32x2 ad2 = fmul2(al2, d2);
+                    float a0, a1;
+                    unpack2(fmul2(ad2, d2), a0, a1);
+                    const f32x2 ex2 = pack2(exp2f(-a0), exp2f(-a1));
+                    const f32x2 R2 = fmul2(ex2, pack2(fc, fc));
+                    const f32x2 y2 = fmul2(c2, fmul2(fmadd2(ad2, pack2(-1.3862943611198906f * fc, -1.3862943611198906f * fc),
+                                                            pack2(dfc, dfc)), ex2));
+                    unpack2(R2, Rn[2 * h], Rn[2 * h + 1]);
+                    unpack2(fmul2(c2, R2), xn[2 * h], xn[2 * h + 1]);
+                    unpack2(y2, yn[2 * h], yn[2 * h + 1]);
+                    Sn[2 * h] = Sn[2 * h + 1] = 0.f;
                 }
                 const float4 *bb4 = reinterpret_cast<const float4 *>(bb_s[warp] + n4 * 4 * NA);
                 if constexpr (PAIRS) {
