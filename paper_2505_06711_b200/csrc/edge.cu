@@ -197,6 +197,8 @@ __device__ __forceinline__ void ffma2(f32x2 &c, f32x2 a, f32x2 b) { asm("fma.rn.
 __device__ __forceinline__ f32x2 fmadd2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 __device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
 struct StashChunk { // reverse gather: kappa holds the edges [e_lo, e_hi); forces once; cbar = or +=
     int64_t e_lo, e_hi;
     int do_forces, accumulate;
@@ -439,11 +441,14 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
                     const float4 cv = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cje & COL_IDX_MASK) * NPHIP)[part];
                     const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[part];
                     const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[part];
-                    float d;
-                    d = we - rc4.x; xv.x = cv.x * (exp2f(-al4.x * d * d) * fce);
-                    d = we - rc4.y; xv.y = cv.y * (exp2f(-al4.y * d * d) * fce);
-                    d = we - rc4.z; xv.z = cv.z * (exp2f(-al4.z * d * d) * fce);
-                    d = we - rc4.w; xv.w = cv.w * (exp2f(-al4.w * d * d) * fce);
+                    // x_n = c_j[n] exp2(-alpha2 (r - r_n)^2) f_c(r), two n per packed operation
+                    const f32x2 w2 = pack2(we, we), m1 = pack2(-1.f, -1.f), f2 = pack2(fce, fce);
+                    const f32x2 da = fmadd2(pack2(rc4.x, rc4.y), m1, w2), db = fmadd2(pack2(rc4.z, rc4.w), m1, w2);
+                    float a0, a1, a2, a3;
+                    unpack2(fmul2(fmul2(pack2(al4.x, al4.y), da), da), a0, a1);
+                    unpack2(fmul2(fmul2(pack2(al4.z, al4.w), db), db), a2, a3);
+                    unpack2(fmul2(pack2(cv.x, cv.y), fmul2(pack2(exp2f(-a0), exp2f(-a1)), f2)), xv.x, xv.y);
+                    unpack2(fmul2(pack2(cv.z, cv.w), fmul2(pack2(exp2f(-a2), exp2f(-a3)), f2)), xv.z, xv.w);
                 }
                 float *dst = XT + (part * 4) * TS + rr;
                 dst[0] = xv.x; dst[TS] = xv.y; dst[2 * TS] = xv.z; dst[3 * TS] = xv.w;
