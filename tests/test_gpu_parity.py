@@ -285,10 +285,12 @@ def test_full_size_config4_sampled(R):
     m.close()
 
 
-def test_mma_edge_backward_variant_parity():
-    """The non-default edge kernels: REANN_EDGE=mma (mma.sync 3xTF32 version of the edge backward kernel) together
-    with REANN_EDGE_FWD=simt (FP32 ALU forward kernel where the mma.sync one is the default). The switches are
-    read once per process, hence the subprocess. Same parity gates as the default pair."""
+@pytest.mark.parametrize("env", [{"REANN_EDGE": "mma", "REANN_EDGE_FWD": "simt"}, {"REANN_DENSE": "simt"}],
+                         ids=["edge_bwd_mma+edge_fwd_simt", "dense_simt"])
+def test_non_default_kernel_variants_parity(env):
+    """The kernels behind the library's environment switches: REANN_EDGE=mma (mma.sync 3xTF32 edge
+    backward) with REANN_EDGE_FWD=simt (FP32 ALU edge forward), and REANN_DENSE=simt (FP32 ALU GEMM chain). The
+    switches are read once per process, hence the subprocess. Same parity gates as the default kernels."""
     import os, subprocess, sys
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     code = (
@@ -299,12 +301,11 @@ def test_mma_edge_backward_variant_parity():
         "    m = R.Reann.from_config(cfg); m.build_neighbors(cfg['pos'], cfg['box'])\n"
         "    out = m.energy_forces(cfg['pos'], cfg['box'])\n"
         "    ref = oracle.energy_forces(cfg['blob'], cfg['species'], cfg['pos'], cfg['box'])\n"
-        "    check_parity(out, ref, m.n, 'mma cfg%%d' %% k); m.close()\n" % (root, os.path.join(root, "tests")))
-    r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, REANN_EDGE="mma", REANN_EDGE_FWD="simt"),
-                       capture_output=True,
-                       text=True, timeout=600)
+        "    check_parity(out, ref, m.n, 'variant cfg%%d' %% k); m.close()\n" % (root, os.path.join(root, "tests")))
+    r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, **env), capture_output=True, text=True,
+                       timeout=600)
     assert r.returncode == 0, r.stdout + r.stderr
-    assert r.stdout.count("[parity] mma") == 2
+    assert r.stdout.count("[parity] variant") == 2
 
 
 def test_stash_chunks_memory_limited_path(R, monkeypatch):
