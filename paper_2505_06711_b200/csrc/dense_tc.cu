@@ -9,8 +9,9 @@
 // followed by  A_hi B_hi;  the dropped A_lo B_lo term is 2^-22 relative.
 // The tensor core adds into its FP32 accumulator with truncation (measured on B200: one
 // accumulator over K = 576 carries a -6e-6 relative bias, 10x the error of an FP32 FMA loop), so
-// K is cut into groups of 32: every group accumulates into a fresh TMEM buffer (double-buffered)
-// which the compute threads then add into FP32 registers with round-to-nearest.
+// K is cut into groups of 32 (64 in the last reverse GEMM, whose result only feeds the forces): every group
+// accumulates into a fresh TMEM buffer (three buffers in rotation) which the compute threads then add into
+// FP32 registers with round-to-nearest.
 //
 // One CTA = one tile of 128 atoms of one species (UMMA M = 128, cta_group::1):
 //   forward   z1 = Q U + b1;  h1 = SiLU(z1);  z2 = h1 W2 + b2;  h2 = SiLU(z2);  out = h2 W3 + b3
@@ -222,31 +223,50 @@ struct Ctl {
     }
     // One K chunk = one accumulation group (step i, group buffer i % NBUF):
     //   D[:, 0:n) = A_lo B_hi^T + A_hi B_lo^T  (4 x K = 8),  then  D += A_hi B_hi^T  (4 x K = 8)
-    __device__ __forceinline__ void mma_chunk(int i, int a_slot, int n_rows) const {
-        const int s = i % NSTAGE, d = i % NBUF;
-        if (i >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((i / NBUF) - 1) & 1));
+    __device__ __forceinline__ void mma_chunk(int i, int a_slot, int n_rows, int g) const {
+        const int s = i % NSTAGE, d = g % NBUF;
+        if (g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
+        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
+        issue(i, a_slot, n_rows, dm, true, false, true);
+        issue(i, a_slot, n_rows, dm, false, true, false);
+        tc_commit(bar(BAR_MMA + s));
+        tc_commit(bar(BAR_DFULL + d));
+    }
+    // Two K chunks (steps i, i+1) = one accumulation group of K = 64: all corrections first, then hi.hi of both
+    __device__ __forceinline__ void mma_pair(int i, int a_slot0, int a_slot1, int n_rows, int g) const {
+        const int d = g % NBUF;
+        if (g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
+        mbar_wait(bar(BAR_BFULL + i % NSTAGE), (uint32_t)((i / NSTAGE) & 1));
+        mbar_wait(bar(BAR_BFULL + (i + 1) % NSTAGE), (uint32_t)(((i + 1) / NSTAGE) & 1));
+        tc_fence_after();
+        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
+        issue(i, a_slot0, n_rows, dm, true, false, true);
+        issue(i + 1, a_slot1, n_rows, dm, true, false, false);
+        issue(i, a_slot0, n_rows, dm, false, true, false);
+        tc_commit(bar(BAR_MMA + i % NSTAGE));
+        issue(i + 1, a_slot1, n_rows, dm, false, true, false);
+        tc_commit(bar(BAR_MMA + (i + 1) % NSTAGE));
+        tc_commit(bar(BAR_DFULL + d));
+    }
+    // the MMAs of one chunk: corrections (A_lo B_hi + A_hi B_lo) and / or main (A_hi B_hi); fresh: overwrite D first
+    __device__ __forceinline__ void issue(int i, int a_slot, int n_rows, uint32_t dm, bool corr, bool main, bool fresh) const {
+        const int s = i % NSTAGE;
         const uint32_t idesc = make_idesc(n_rows);
         const uint32_t a_hi = a0 + (uint32_t)a_slot * A_SLOT, a_lo = a_hi + A_HALF;
         const uint32_t b_lbo = (uint32_t)n_rows * 16;
         const uint32_t b_hi = b0 + (uint32_t)s * B_SLOT, b_lo = b_hi + (uint32_t)n_rows * KC * 4;
-        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
 #pragma unroll
         for (int kk = 0; kk < KC / 8; ++kk) {
             const uint64_t ah = make_desc(a_hi + kk * 2 * A_LBO, A_LBO), al = make_desc(a_lo + kk * 2 * A_LBO, A_LBO);
             const uint64_t bh = make_desc(b_hi + kk * 2 * b_lbo, b_lbo), bl = make_desc(b_lo + kk * 2 * b_lbo, b_lbo);
-            umma_tf32(dm, al, bh, idesc, kk == 0 ? 0u : 1u);
-            umma_tf32(dm, ah, bl, idesc, 1u);
+            if (corr) {
+                umma_tf32(dm, al, bh, idesc, (fresh && kk == 0) ? 0u : 1u);
+                umma_tf32(dm, ah, bl, idesc, 1u);
+            }
+            if (main) umma_tf32(dm, ah, bh, idesc, 1u);
         }
-#pragma unroll
-        for (int kk = 0; kk < KC / 8; ++kk) {
-            const uint64_t ah = make_desc(a_hi + kk * 2 * A_LBO, A_LBO);
-            const uint64_t bh = make_desc(b_hi + kk * 2 * b_lbo, b_lbo);
-            umma_tf32(dm, ah, bh, idesc, 1u);
-        }
-        tc_commit(bar(BAR_MMA + s));
-        tc_commit(bar(BAR_DFULL + d));
     }
 };
 
@@ -343,11 +363,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                     mbar_wait(c.bar(BAR_AFULL + s), (uint32_t)((i / NSTAGE) & 1));
                     if (i + 2 < n1) issue_q(i + 2);
                     TC_TRACE(0, 0, 2 * i);
-                    c.mma_chunk(i, s, H1p);
+                    c.mma_chunk(i, s, H1p, i);
                 } else {
                     mbar_wait(c.bar(BAR_AH + (i - n1)), 0);
                     TC_TRACE(0, 0, 2 * i);
-                    c.mma_chunk(i, i - n1, H2p);
+                    c.mma_chunk(i, i - n1, H2p, i);
                 }
                 TC_TRACE(0, 0, 2 * i + 1);
                 if (i + 2 < total) copy_b(i + 2);
@@ -487,6 +507,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
     const uint32_t bar0 = smem_u32(smem + SM_BAR);
     const uint32_t tmem = tc_prologue(smem, &tmem_base_s, CW2 >= 32 ? 128u : 256u);
     // steps: [R1 (only when outbar is given: K = n_out padded to 32)] NCH2 x R2, nblk x NCH1 x R3
+    constexpr int GR3 = NCH1 >= 2 ? 2 : 1;         // K chunks per accumulator group of R3
     const int o1 = A.outbar ? 1 : 0, i3 = o1 + NCH2;
     const int nblk = (A.K1 + 127) / 128, total = i3 + nblk * NCH1;
 
@@ -506,15 +527,26 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                 if (i < o1) {
                     mbar_wait(c.bar(BAR_AFULL), 0);
                     TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, 0, H2p);
+                    c.mma_chunk(i, 0, H2p, i);
                 } else if (i < i3) {
                     mbar_wait(c.bar(BAR_AH + (i - o1)), 0);
                     TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, i - o1, H1p);
+                    c.mma_chunk(i, i - o1, H1p, i);
                 } else {
+                    // R3: groups of GR3 chunks (K = 32 GR3 per accumulator); group index continues after R2
                     if (i == i3) mbar_wait(c.bar(BAR_ARES), 0);
+                    const int kc = (i - i3) % NCH1, g = i3 + (i - i3) / GR3;
                     TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, (i - i3) % NCH1, rows_of(i));
+                    if (GR3 == 2) {
+                        if (i + 2 < total) copy_b(i + 2);          // in flight during this group's MMAs
+                        c.mma_pair(i, kc, kc + 1, rows_of(i), g);
+                        if (i + 3 < total) copy_b(i + 3);          // waits for the hi.hi MMAs of chunk i
+                        TC_TRACE(1, 0, 2 * i + 1);
+                        ++i;
+                        continue;
+                    } else {
+                        c.mma_chunk(i, kc, rows_of(i), g);
+                    }
                 }
                 TC_TRACE(1, 0, 2 * i + 1);
                 if (i + 2 < total) copy_b(i + 2);
@@ -615,8 +647,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
 #pragma unroll
             for (int c = 0; c < 64; ++c) q[c] = 0.f;
 #pragma unroll 1
-            for (int kc = 0; kc < NCH1; ++kc) {
-                const int g = i3 + nb * NCH1 + kc;
+            for (int gi = 0; gi < NCH1 / GR3; ++gi) {
+                const int g = i3 + nb * (NCH1 / GR3) + gi;
                 if (ncols - hf * 64 >= 64) drain_group<64>(q, bar0, tl, g, hf * 64, true);
                 else if (ncols - hf * 64 >= 32) drain_group<32>(q, bar0, tl, g, hf * 64, true);
                 else drain_group<32>(q, bar0, tl, g, hf * 64, false);
