@@ -401,7 +401,8 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
     const int64_t N = h->N;
     if (N == 0) { h->G = 0; h->n_ext = 0; h->E_list = 0; h->E_rc_build = 0; }
     // per-evaluation buffers whose size follows the list
-    RC(dev_ensure(h, h->rank16, sizeof(uint16_t) * (size_t)std::max<int64_t>(h->E_list, 1)));
+    if (h->rank16.bytes < sizeof(uint16_t) * (size_t)std::max<int64_t>(h->E_list, 1))
+        RC(dev_ensure(h, h->rank16, sizeof(uint16_t) * ((size_t)std::max<int64_t>(h->E_list, 1) + (size_t)h->E_list / 32 + 1024)));
     RC(dev_ensure(h, h->rc_cnt, sizeof(int32_t) * (size_t)(N + 1)));
     RC(dev_ensure(h, h->rc_ptr, sizeof(int64_t) * (size_t)(N + 1)));
     RC(dev_ensure(h, h->scan_ws, scan_workspace_bytes(N + 1)));

@@ -370,8 +370,11 @@ int neighbor_build(reann *h, const double *d_pos) {
     if (E >= ((int64_t)1 << 32)) return set_err(h, REANN_ERR_UNSUPPORTED, "more than 2^32 list entries");
     h->E_list = E;
     h->E_rc_build = (int64_t)(*(unsigned long long *)(h->h_flags + 4));
-    RC(dev_ensure(h, h->col, sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1)));
-    RC(dev_ensure(h, h->rev, sizeof(uint32_t) * (size_t)std::max<int64_t>(E, 1)));
+    // list-sized buffers get 3 % head-room: the list length fluctuates from rebuild to rebuild, and a
+    // cudaFree + cudaMalloc of a few hundred MB in the middle of an MD run costs tens of milliseconds
+    const size_t e_cap = (size_t)std::max<int64_t>(E, 1) + (size_t)E / 32 + 1024;
+    if (h->col.bytes < sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1)) RC(dev_ensure(h, h->col, sizeof(int32_t) * e_cap));
+    if (h->rev.bytes < sizeof(uint32_t) * (size_t)std::max<int64_t>(E, 1)) RC(dev_ensure(h, h->rev, sizeof(uint32_t) * e_cap));
     LAUNCH(ctx, k_nbr<true>, div_up(N, NB_WARPS), NB_WARPS * 32, 0, (const XRec *)h->xrec.p, N, g,
            (const int32_t *)h->cell_rank.p, (const int64_t *)h->cell_start.p, (const int32_t *)h->img_index.p,
            (int32_t *)nullptr, (unsigned long long *)nullptr, (const int64_t *)h->row_ptr.p, (int32_t *)h->col.p,
