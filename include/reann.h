@@ -22,7 +22,13 @@
  *  - Every function returns a REANN_* code, never throws or aborts; reann_last_error() gives
  *    text for the last failure on that handle.
  *  - Determinism: same inputs give bitwise-identical outputs (no floating-point atomics;
- *    fixed reduction order).
+ *    fixed reduction order) for a given build, kernel selection and stash chunk count.
+ *  - Memory: device buffers grow on demand and are kept; list-sized buffers carry head-room so
+ *    that skin-triggered rebuilds do not allocate. When the per-edge stash of the reverse pass
+ *    (4 n_gauss bytes per edge within rc) does not fit into the free device memory it is held
+ *    for a fraction of the atoms at a time (transparent to the caller).
+ *  - Environment switches read by the library (kernel selection, for testing):
+ *    REANN_DENSE=simt, REANN_EDGE_FWD=simt, REANN_EDGE=mma, REANN_STASH_CHUNKS=n.
  */
 #ifndef REANN_H
 #define REANN_H
