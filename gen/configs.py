@@ -109,8 +109,10 @@ def _calib_table() -> dict:
 
 
 def make_config(k: int, T: int | None = None, n_mol: int | None = None, ncell: int | None = None,
-                geometry_only: bool = False, gains: dict | None = None) -> dict:
+                geometry_only: bool = False, gains: dict | None = None, radial_jitter: float = 0.0) -> dict:
     """Build config k. Overrides (T, n_mol, ncell) give same-density replicas / the T sweep.
+
+    radial_jitter > 0 (tests only): per-(layer, species) radial tables, see make_weights.
 
     Returns dict with pos[N,3] f64, species[N] i32, box[9] f64 (row-major lattice), masses[N],
     hyper-parameters, and (unless geometry_only) the weights blob (bytes)."""
@@ -149,7 +151,8 @@ def make_config(k: int, T: int | None = None, n_mol: int | None = None, ncell: i
         g = gains if gains is not None else _calib_table().get(f"{k}:{r['T']}", {})
         w = make_weights(S=S, T=r["T"], L=r["L"], n_gauss=r["n_gauss"], n_orb=out["n_orb"],
                          H=r["H"], Hc=r.get("Hc", r["H"]), rc=r["rc"], nbar=r["nbar"], seed=seed_w,
-                         e_scale=g.get("e", 1.0), wc_gain=g.get("wc"), c_gain=g.get("c"))
+                         e_scale=g.get("e", 1.0), wc_gain=g.get("wc"), c_gain=g.get("c"),
+                         radial_jitter=radial_jitter)
         out["weights"] = w
         out["blob"] = pack_blob(w)
         out["gains"] = g

@@ -38,18 +38,29 @@ def n_orb_default(n_gauss: int, L: int) -> int:
 
 
 def make_weights(S, T, L, n_gauss, n_orb, H, rc, nbar, seed, Hc=None, e_scale=1.0, wc_gain=None,
-                 c_gain=None) -> dict:
+                 c_gain=None, radial_jitter=0.0) -> dict:
     """Seeded weights: r_n = n rc/(N-1), alpha = 1/(2 Delta^2) with Delta = rc/(N-1);
     c0 ~ N(0,1); Wc[t] ~ wc_gain[t] N(0,1) rc^-l / sqrt(N nbar); MLP Xavier-normal, biases
     N(0, 0.1^2); last layer of coefficient network t multiplied by c_gain[t]; the energy
     network's last layer by e_scale. The gains (gen/calib.json, written by
     oracle/calibrate.py) keep rho^t and c^t of order one in every layer, so that every term
-    of the backward pass carries weight in the parity tests."""
+    of the backward pass carries weight in the parity tests.
+
+    radial_jitter > 0 (tests only; the BASELINE configs keep identical rows, as their recipe says):
+    every (layer t, species s) row of r_center / alpha is scaled by its own seeded factor
+    (1 + j (1 + u))^(+-1), u ~ U[0,1), j = radial_jitter (10-20 % for j = 0.1; drawn from a separate
+    stream so that no other weight changes), so that reading A-3 -- tables indexed by layer and by
+    the NEIGHBOUR's species -- is visible to the pins and the parity tests."""
     rng = np.random.default_rng(seed)
     Hc = H if Hc is None else Hc
     delta = rc / (n_gauss - 1) if n_gauss > 1 else rc
     rcen = np.broadcast_to(np.arange(n_gauss) * delta, (T, S, n_gauss)).copy()
     alpha = np.full((T, S, n_gauss), 1.0 / (2.0 * delta * delta))
+    if radial_jitter > 0:
+        jr = np.random.default_rng(seed + 7777)
+        for arr in (rcen, alpha):
+            f = (1.0 + radial_jitter * (1.0 + jr.random((T, S)))) ** jr.choice([-1.0, 1.0], size=(T, S))
+            arr *= f[:, :, None]
     c0 = rng.standard_normal((S, n_gauss))
     Wc = rng.standard_normal((T, L + 1, n_gauss, n_orb))
     for l in range(L + 1):

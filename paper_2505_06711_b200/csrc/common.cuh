@@ -94,15 +94,6 @@ size_t scan_workspace_bytes(int64_t n);
 void exclusive_scan_i32_to_i64(const LaunchCtx &ctx, const int32_t *in, int64_t *out, int64_t n, void *workspace);
 
 // ---- neighbor.cu ----
-struct NeighborArgs {
-    int64_t N;
-    double Lb[3];
-    int nc[3];
-    int64_t ncell;
-    double R2;      // (rc+skin)^2
-    double R;       // rc+skin
-    double rc2;     // rc^2
-};
 struct reann; // handle (api.cu)
 int neighbor_build(reann *h, const double *d_pos);   // returns REANN_* code
 int neighbor_export(reann *h, int64_t *n_edges, int64_t *row_ptr, int32_t *j, int8_t *shift);

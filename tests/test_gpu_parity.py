@@ -21,10 +21,13 @@ def R():
     return R
 
 
-def small_cfg(S=2, T=3, L=3, n_gauss=5, H=(12, 10), Hc=(9, 11), rc=3.5, skin=0.5, n=60, box=14.0, seed=5):
+def small_cfg(S=2, T=3, L=3, n_gauss=5, H=(12, 10), Hc=(9, 11), rc=3.5, skin=0.5, n=60, box=14.0, seed=5,
+              radial_jitter=0.15):
+    """Radial tables differ per (layer, neighbour species) by 15-30 % (reading A-3 is visible to the parity)."""
     rng = np.random.default_rng(seed)
     w = gen.make_weights(S=S, T=T, L=L, n_gauss=n_gauss, n_orb=gen.n_orb_default(n_gauss, L), H=H, Hc=Hc, rc=rc,
-                         nbar=12.0, seed=seed + 1, wc_gain=[2.0] * T, c_gain=[2.0] * (T - 1), e_scale=3.0)
+                         nbar=12.0, seed=seed + 1, wc_gain=[2.0] * T, c_gain=[2.0] * (T - 1), e_scale=3.0,
+                         radial_jitter=radial_jitter)
     return dict(pos=rng.random((n, 3)) * box, species=rng.integers(0, S, n).astype(np.int32),
                 box=np.diag([box] * 3).reshape(9), rc=rc, skin=skin, T=T, L=L, n_gauss=n_gauss, blob=gen.pack_blob(w),
                 weights=w)
@@ -64,10 +67,15 @@ def test_neighbor_pair_sets_exact(R, case):
 
 
 # ------------------------------------------------------------------ energy / forces / virial
-@pytest.mark.parametrize("case", ["cfg0", "cfg1", "cfg2", "cfg3r", "cfg4r_T1", "cfg4r_T3", "cfg4r_T6", "cfg5r",
-                                  "small_L3", "small_L0", "small_L1_S1", "small_n4", "small_n12"])
+@pytest.mark.parametrize("case", ["cfg0", "cfg0j", "cfg1", "cfg2", "cfg2j", "cfg3r", "cfg3rj", "cfg4r_T1", "cfg4r_T3",
+                                  "cfg4r_T6", "cfg5r", "small_L3", "small_L0", "small_L1_S1", "small_n4", "small_n12"])
 def test_energy_forces_virial_parity(R, case):
+    """`j` cases: radial tables that differ per (layer, neighbour species) -- with identical rows (the BASELINE
+    recipe) an indexing mistake in the edge kernels (s_j -> s_i, t -> 0) would be invisible."""
     if case.startswith("cfg") and case[3:].isdigit(): cfg = gen.make_config(int(case[3:]))
+    elif case == "cfg0j": cfg = gen.make_config(0, radial_jitter=0.15)
+    elif case == "cfg2j": cfg = gen.make_config(2, n_mol=300, radial_jitter=0.1)   # N_phi = 16, L = 2: mma.sync edge forward
+    elif case == "cfg3rj": cfg = gen.make_config(3, n_mol=500, radial_jitter=0.1)  # N_phi = 16, L = 3
     elif case == "cfg3r": cfg = gen.make_config(3, n_mol=700)         # L=3, 16 Gaussians, ragged tiles
     elif case.startswith("cfg4r"): cfg = gen.make_config(4, ncell=7, T=int(case[-1]))
     elif case == "cfg5r": cfg = gen.make_config(5, n_mol=900)

@@ -15,9 +15,11 @@ import np_pairform
 BIG = np.diag([200.0, 200.0, 200.0]).reshape(9)
 
 
-def small_model(S=2, T=3, L=3, n_gauss=5, H=(12, 10), Hc=(9, 11), rc=3.5, seed=77, n_orb=None):
+def small_model(S=2, T=3, L=3, n_gauss=5, H=(12, 10), Hc=(9, 11), rc=3.5, seed=77, n_orb=None, radial_jitter=0.15):
+    """Radial tables differ per (layer, species) by 15-30 % so that their indexing (A-3) is visible."""
     n_orb = gen.n_orb_default(n_gauss, L) if n_orb is None else n_orb
-    w = gen.make_weights(S=S, T=T, L=L, n_gauss=n_gauss, n_orb=n_orb, H=H, Hc=Hc, rc=rc, nbar=12.0, seed=seed)
+    w = gen.make_weights(S=S, T=T, L=L, n_gauss=n_gauss, n_orb=n_orb, H=H, Hc=Hc, rc=rc, nbar=12.0, seed=seed,
+                         radial_jitter=radial_jitter)
     return w, gen.pack_blob(w)
 
 
@@ -70,6 +72,48 @@ def test_dimer_closed_form():
             * 0.5 * (1 + np.cos(np.pi * rr / w["rc"]))
         ang = np.array([dv[0] ** a * dv[1] ** b * dv[2] ** c for a, b, c in lxyz])
         np.testing.assert_allclose(r["b"][0, i], np.outer(rad, ang), rtol=1e-13, atol=1e-15)
+        # A-3 (PAPER.md:35 "G_j ... of the jth neighbor atom", :38): the radial table is the NEIGHBOUR's row.
+        # With the centre's row instead the value is different (the rows differ by >= 15 %), so this pin can fail.
+        rad_i = w["c0"][sp[j]] * np.exp(-w["alpha"][0, sp[i]] * (rr - w["rcen"][0, sp[i]]) ** 2) \
+            * 0.5 * (1 + np.cos(np.pi * rr / w["rc"]))
+        assert np.abs(np.outer(rad_i, ang) - r["b"][0, i]).max() > 1e-3 * np.abs(r["b"][0, i]).max()
+
+
+def test_dimer_second_layer_uses_its_own_tables():
+    """T = 2 dimer: b^1_i[n,a] = c^1_j[n] R_n(r; t=1, s_j) A_a typed by hand from the layer-1 rows of the radial
+    tables and the oracle's own c^1 (the MLP output, pinned by the pair form and the matmul pins). The rows of
+    layer 0 give a different value: the layer index of the tables (A-3) is pinned."""
+    w, blob = small_model(T=2, L=2, n_gauss=6)
+    assert np.abs(w["rcen"][1] / np.where(w["rcen"][0] == 0, 1, w["rcen"][0]) - 1)[:, 1:].min() > 0.02
+    d = np.array([-0.9, 1.3, 0.8])
+    pos = np.array([[100.0, 100.0, 100.0], [100.0, 100.0, 100.0] + d])
+    sp = np.array([1, 0], dtype=np.int32)
+    r = oracle.energy_forces(blob, sp, pos, BIG, forces=False, dumps=True)
+    lxyz, _ = oracle.monomials(2)
+    rr = np.linalg.norm(d)
+    fc = 0.5 * (1 + np.cos(np.pi * rr / w["rc"]))
+    for i, j, dv in ((0, 1, d), (1, 0, -d)):
+        ang = np.array([dv[0] ** a * dv[1] ** b * dv[2] ** c for a, b, c in lxyz])
+        for t_tab, same in ((1, True), (0, False)):
+            rad = r["c"][1, j] * np.exp(-w["alpha"][t_tab, sp[j]] * (rr - w["rcen"][t_tab, sp[j]]) ** 2) * fc
+            ok = np.allclose(r["b"][1, i], np.outer(rad, ang), rtol=1e-12, atol=1e-15)
+            assert ok == same, (i, t_tab)
+
+
+def test_pairform_T2_layer_tables_differ():
+    """Whole-E pin on a model whose layer-0 and layer-1 tables (and species rows) differ: the independent NumPy
+    pair form, which reads alpha[t][s_j] / rcen[t][s_j] as the blob docstring lays them out."""
+    w, blob = small_model(T=2, L=2, n_gauss=6, radial_jitter=0.2)
+    pos, sp = cluster(24, 1.7, 13)
+    r = oracle.energy_forces(blob, sp, pos, BIG, forces=False, dumps=True)
+    E, Ei, rhos, cs = np_pairform.energy(w, sp, pos, BIG, True)
+    np.testing.assert_allclose(r["Ei"], Ei, rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(r["rho"][1], rhos[1], rtol=1e-9, atol=1e-12)
+    # the same weights with every row equal to row (0, 0) give a different energy: the test can see the indexing
+    w2 = dict(w); w2["rcen"] = np.broadcast_to(w["rcen"][0, 0], w["rcen"].shape).copy()
+    w2["alpha"] = np.broadcast_to(w["alpha"][0, 0], w["alpha"].shape).copy()
+    r2 = oracle.energy_forces(gen.pack_blob(w2), sp, pos, BIG, forces=False)
+    assert np.abs(r2["Ei"] - r["Ei"]).max() > 1e-4 * np.abs(r["Ei"]).max()
 
 
 def test_cutoff_function_limits():
