@@ -102,6 +102,8 @@ typedef struct {
            ms_rev_gather, ms_output;
     int64_t n_profiled_calls;        /* calls the ms_* fields (except ms_build) accumulate    */
     size_t bytes_device;             /* device memory currently held by the handle            */
+    double ms_rev_gather_t0;         /* the layer-0 reverse gather (forces only, no cbar); ms_rev_gather = layers t >= 1 */
+    int64_t stash_chunks;            /* atom chunks the per-edge stash is currently held in (1 = whole) */
 } reann_stats_t;
 
 /* Neighbour list in the CALLER's order and frame (for exact pair-set parity):
@@ -110,6 +112,12 @@ typedef struct {
  *   that the edge vector is pos[j] + shift o box - pos[i] for the positions given at build.
  *   All three are HOST pointers. */
 int reann_get_neighbors(reann_t *h, int64_t *n_edges, int64_t *row_ptr, int32_t *j, int8_t *shift);
+
+/* The same for n_sel selected atoms only (caller indices, HOST array): row_ptr[n_sel+1] is always written; j and
+ * shift (both or neither; HOST arrays of row_ptr[n_sel] entries) when given. For sampled exact pair-set parity
+ * on systems whose whole list (up to 2^32 entries) is too large to export. */
+int reann_get_neighbor_rows(reann_t *h, int64_t n_sel, const int64_t *atoms, int64_t *row_ptr, int32_t *j,
+                            int8_t *shift);
 
 int reann_get_stats(reann_t *h, reann_stats_t *out);
 int reann_set_profiling(reann_t *h, int on);            /* CUDA-event timing of kernel groups  */

@@ -36,6 +36,9 @@ def lib():
         L.oracle_neighbors.restype = ctypes.c_int64
         L.oracle_neighbors.argtypes = [c_dp, ctypes.c_int64, c_dp, ctypes.c_double, ctypes.c_int,
                                        c_ip, ctypes.c_int64]
+        L.oracle_neighbor_rows.restype = ctypes.c_int64
+        L.oracle_neighbor_rows.argtypes = [c_dp, ctypes.c_int64, c_dp, ctypes.c_double, ctypes.POINTER(ctypes.c_int64),
+                                           ctypes.c_int64, ctypes.POINTER(ctypes.c_int64), c_ip, ctypes.c_int64]
         L.oracle_energy_forces.restype = ctypes.c_int
         L.oracle_energy_forces.argtypes = [ctypes.c_void_p, ctypes.c_size_t, c_ip, ctypes.c_int64, c_dp,
                                            c_dp, ctypes.c_int, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp,
@@ -74,6 +77,25 @@ def neighbors(pos, box9, R, mode="cell") -> np.ndarray:
     n2 = lib().oracle_neighbors(_dp(pos), N, _dp(box9), float(R), m, _ip(rows), n)
     assert n2 == n
     return rows[:n]
+
+
+def neighbor_rows(pos, box9, R, sel):
+    """Sorted rows (i, j, Sx, Sy, Sz) of the atoms `sel` (strictly ascending) only, and row_ptr[len(sel)+1]:
+    the same pair test as neighbors() over the cell list; for systems whose full list is too large."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    box9 = np.ascontiguousarray(box9, dtype=np.float64).reshape(9)
+    sel = np.ascontiguousarray(sel, dtype=np.int64)
+    i64p = ctypes.POINTER(ctypes.c_int64)
+    row_ptr = np.zeros(len(sel) + 1, dtype=np.int64)
+    n = lib().oracle_neighbor_rows(_dp(pos), pos.shape[0], _dp(box9), float(R), sel.ctypes.data_as(i64p), len(sel),
+                                   row_ptr.ctypes.data_as(i64p), None, 0)
+    if n < 0:
+        raise ValueError(f"oracle_neighbor_rows error {-n}")
+    rows = np.zeros((max(n, 1), 5), dtype=np.int32)
+    n2 = lib().oracle_neighbor_rows(_dp(pos), pos.shape[0], _dp(box9), float(R), sel.ctypes.data_as(i64p), len(sel),
+                                    row_ptr.ctypes.data_as(i64p), _ip(rows), n)
+    assert n2 == n
+    return rows[:n], row_ptr
 
 
 def blob_info(blob: bytes) -> dict:

@@ -151,8 +151,12 @@ static inline int pair_test(const double *xi, const double *xj, const int S[3], 
     return d2 < R2;
 }
 
-/* mode 0: O(N^2 * 27) brute force over S in {-1,0,1}^3; mode 1: cell list. Both need L_d >= R. */
-static int build_edges(const double *pos, int64_t N, const double *box9, double R, int mode, edges_t *E) {
+/* mode 0: O(N^2 * 27) brute force over S in {-1,0,1}^3; mode 1: cell list. Both need L_d >= R.
+ * sel == NULL: rows of all N atoms (row k = atom k); else rows of the n_sel atoms sel[k] only (row k = atom
+ * sel[k]; the same pair test over the same candidates -- used for sampled pair-set parity on systems whose
+ * full list would not fit the host). */
+static int build_edges_sel(const double *pos, int64_t N, const double *box9, double R, int mode, edges_t *E,
+                           const int64_t *sel, int64_t n_sel) {
     memset(E, 0, sizeof(*E));
     double Lb[3];
     int rc_ = box_lengths(box9, Lb);
@@ -161,7 +165,8 @@ static int build_edges(const double *pos, int64_t N, const double *box9, double 
     const double R2 = R * R;
     E->xw = malloc(sizeof(double) * 3 * (size_t)(N > 0 ? N : 1));
     E->w = malloc(sizeof(int32_t) * 3 * (size_t)(N > 0 ? N : 1));
-    E->off = calloc((size_t)N + 1, sizeof(int64_t));
+    const int64_t n_rows = sel ? n_sel : N;
+    E->off = calloc((size_t)n_rows + 1, sizeof(int64_t));
     if (!E->xw || !E->w || !E->off) return ORC_ERR_MEM;
     wrap_all(pos, N, Lb, E->xw, E->w);
     int nc[3]; int64_t ncell = 1;
@@ -196,16 +201,17 @@ static int build_edges(const double *pos, int64_t N, const double *box9, double 
     for (int pass = 0; pass < 2; ++pass) {
         if (pass == 1) {
             int64_t tot = 0;
-            for (int64_t i = 0; i < N; ++i) { int64_t c = E->off[i + 1]; E->off[i + 1] = tot + c; tot += c; }
+            for (int64_t i = 0; i < n_rows; ++i) { int64_t c = E->off[i + 1]; E->off[i + 1] = tot + c; tot += c; }
             /* off[i+1] now holds end of row i; off[0] = 0 */
             E->n = tot;
             E->e = malloc(sizeof(edge_t) * (size_t)(tot > 0 ? tot : 1));
             if (!E->e) return ORC_ERR_MEM;
         }
 #pragma omp parallel for schedule(dynamic, 64)
-        for (int64_t i = 0; i < N; ++i) {
+        for (int64_t row = 0; row < n_rows; ++row) {
+            const int64_t i = sel ? sel[row] : row;
             int64_t cnt = 0;
-            int64_t base = (pass == 1) ? (i == 0 ? 0 : E->off[i]) : 0;
+            int64_t base = (pass == 1) ? (row == 0 ? 0 : E->off[row]) : 0;
             const double *xi = E->xw + 3 * i;
             double d[3];
             if (mode == 0) {
@@ -239,11 +245,14 @@ static int build_edges(const double *pos, int64_t N, const double *box9, double 
                     }
                 }
             }
-            if (pass == 0) E->off[i + 1] = cnt;
+            if (pass == 0) E->off[row + 1] = cnt;
         }
     }
     free(cell_of); free(cstart); free(catoms);
     return ORC_OK;
+}
+static int build_edges(const double *pos, int64_t N, const double *box9, double R, int mode, edges_t *E) {
+    return build_edges_sel(pos, N, box9, R, mode, E, NULL, 0);
 }
 
 static int cmp_row5(const void *a, const void *b) {
@@ -266,6 +275,32 @@ int64_t oracle_neighbors(const double *pos, int64_t N, const double *box9, doubl
         for (int64_t i = 0; i < N; ++i)
             for (int64_t q = E.off[i]; q < E.off[i + 1]; ++q) {
                 edge_t *e = &E.e[q]; int32_t *r = rows + 5 * q;
+                r[0] = (int32_t)i; r[1] = e->j;
+                for (int d = 0; d < 3; ++d) r[2 + d] = e->S[d] + E.w[3 * i + d] - E.w[3 * e->j + d];
+            }
+        qsort(rows, (size_t)n, 5 * sizeof(int32_t), cmp_row5);
+    }
+    edges_free(&E);
+    return n;
+}
+
+/* The same rows for the selected atoms sel[0..n_sel) only (cell list): rows (i, j, Sx, Sy, Sz), caller frame,
+ * sorted; row_ptr[n_sel+1] gives each selected atom's slice after sorting by (i, ...) -- sel must be
+ * strictly ascending so that the sorted order is the selection order. Returns the row count or -(error). */
+int64_t oracle_neighbor_rows(const double *pos, int64_t N, const double *box9, double R, const int64_t *sel,
+                             int64_t n_sel, int64_t *row_ptr, int32_t *rows, int64_t cap) {
+    for (int64_t k = 0; k < n_sel; ++k)
+        if (sel[k] < 0 || sel[k] >= N || (k > 0 && sel[k] <= sel[k - 1])) return -(int64_t)ORC_ERR_ARG;
+    edges_t E;
+    int rc_ = build_edges_sel(pos, N, box9, R, 1, &E, sel, n_sel);
+    if (rc_) { edges_free(&E); return -(int64_t)rc_; }
+    int64_t n = E.n;
+    if (row_ptr) memcpy(row_ptr, E.off, sizeof(int64_t) * (size_t)(n_sel + 1));
+    if (rows && cap >= n) {
+        for (int64_t k = 0; k < n_sel; ++k)
+            for (int64_t q = E.off[k]; q < E.off[k + 1]; ++q) {
+                edge_t *e = &E.e[q]; int32_t *r = rows + 5 * q;
+                const int64_t i = sel[k];
                 r[0] = (int32_t)i; r[1] = e->j;
                 for (int d = 0; d < 3; ++d) r[2 + d] = e->S[d] + E.w[3 * i + d] - E.w[3 * e->j + d];
             }

@@ -21,7 +21,7 @@ REANN_OK, REANN_ERR_ARG, REANN_ERR_WEIGHTS, REANN_ERR_BOX, REANN_ERR_NO_NEIGHBOR
     REANN_ERR_OOM, REANN_ERR_UNSUPPORTED = range(8)
 
 EXPORTS = ["reann_create", "reann_build_neighbors", "reann_energy_forces", "reann_destroy", "reann_last_error",
-           "reann_get_neighbors", "reann_get_stats", "reann_set_profiling", "reann_set_stream",
+           "reann_get_neighbors", "reann_get_neighbor_rows", "reann_get_stats", "reann_set_profiling", "reann_set_stream",
            "reann_get_atomic_energies", "reann_verlet"]
 
 
@@ -38,7 +38,8 @@ class Stats(ctypes.Structure):
                 ("ms_edge_fwd", ctypes.c_double), ("ms_dense_fwd", ctypes.c_double), ("ms_gather", ctypes.c_double),
                 ("ms_dense_bwd", ctypes.c_double), ("ms_edge_bwd", ctypes.c_double),
                 ("ms_rev_gather", ctypes.c_double), ("ms_output", ctypes.c_double),
-                ("n_profiled_calls", ctypes.c_int64), ("bytes_device", ctypes.c_size_t)]
+                ("n_profiled_calls", ctypes.c_int64), ("bytes_device", ctypes.c_size_t),
+                ("ms_rev_gather_t0", ctypes.c_double), ("stash_chunks", ctypes.c_int64)]
 
 
 _lib = None
@@ -66,6 +67,8 @@ def lib() -> ctypes.CDLL:
         L.reann_last_error.argtypes = [vp]
         L.reann_get_neighbors.restype = ctypes.c_int
         L.reann_get_neighbors.argtypes = [vp, ctypes.POINTER(i64), vp, vp, vp]
+        L.reann_get_neighbor_rows.restype = ctypes.c_int
+        L.reann_get_neighbor_rows.argtypes = [vp, i64, vp, vp, vp, vp]
         L.reann_get_stats.restype = ctypes.c_int
         L.reann_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
         L.reann_set_profiling.restype = ctypes.c_int
@@ -156,6 +159,18 @@ def reann_get_neighbors(h, n_atoms: int):
     return row_ptr, j[:n.value], sh[:n.value]
 
 
+def reann_get_neighbor_rows(h, atoms):
+    """-> (row_ptr[len(atoms)+1], j[E], shift[E,3]) of the selected atoms, caller order / caller frame."""
+    atoms = np.ascontiguousarray(atoms, dtype=np.int64)
+    row_ptr = np.zeros(len(atoms) + 1, dtype=np.int64)
+    _check(h, lib().reann_get_neighbor_rows(h, len(atoms), _ptr(atoms), _ptr(row_ptr), None, None))
+    n = int(row_ptr[-1])
+    j = np.zeros(max(n, 1), dtype=np.int32)
+    sh = np.zeros((max(n, 1), 3), dtype=np.int8)
+    _check(h, lib().reann_get_neighbor_rows(h, len(atoms), _ptr(atoms), _ptr(row_ptr), _ptr(j), _ptr(sh)))
+    return row_ptr, j[:n], sh[:n]
+
+
 class Reann:
     """Convenience wrapper around one handle (host NumPy in, NumPy out unless tensors are given)."""
 
@@ -187,6 +202,9 @@ class Reann:
 
     def neighbors(self):
         return reann_get_neighbors(self.h, self.n)
+
+    def neighbor_rows(self, atoms):
+        return reann_get_neighbor_rows(self.h, atoms)
 
     def stats(self) -> dict:
         return reann_get_stats(self.h)

@@ -99,7 +99,8 @@ static int parse_blob(const unsigned char *p, size_t nbytes, BlobView &v, std::s
     v.H1c = hd[6]; v.H2c = hd[7]; v.H1e = hd[8]; v.H2e = hd[9];
     memcpy(&v.rc, p + 56, 8);
     if (v.S < 1 || v.T < 1 || v.nphi < 1 || v.norb < 1 || v.L < 0 || !(v.rc > 0) || v.H1c < 1 || v.H2c < 1 || v.H1e < 1 ||
-        v.H2e < 1 || v.S > 1024 || v.T > 1024 || v.nphi > 4096 || v.L > 64) {
+        v.H2e < 1 || v.S > 1024 || v.T > 1024 || v.nphi > 4096 || v.L > 64 || v.norb > (1 << 20) || v.H1c > (1 << 16) ||
+        v.H2c > (1 << 16) || v.H1e > (1 << 16) || v.H2e > (1 << 16)) {
         why = "header fields out of range"; return REANN_ERR_WEIGHTS;
     }
     size_t need = (size_t)2 * v.T * v.S * v.nphi + (size_t)v.S * v.nphi + (size_t)v.T * (v.L + 1) * v.nphi * v.norb;
@@ -411,7 +412,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         if (h->c_ext.bytes < need) { RC(dev_ensure(h, h->c_ext, need + need / 16)); }
         CU(h, cudaMemsetAsync(h->c_ext.p, 0, h->c_ext.bytes, h->stream)); // padded coefficients stay 0
     }
-    if (!h->b.p) {
+    if (!h->eval_bufs_ready) {
         RC(dev_ensure(h, h->b, sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(N, 1) * md.NB));
         // dense rows: tensor-core path = 128-row tiles (tile-quad layout, dense_tc.cu), SIMT path = sp_list rows
         const size_t rows = h->dense_tc ? (size_t)std::max(h->n_tiles, 1) * DENSE_TC_TM : (size_t)std::max<int64_t>(N, 1);
@@ -428,6 +429,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->vir_part, sizeof(double) * 9 * (size_t)h->n_vir_blocks));
         RC(dev_ensure(h, h->red_scratch, sizeof(double) * ((size_t)N / 256 + 2)));
         RC(dev_ensure(h, h->out_stage, sizeof(double) * (16 + 3 * (size_t)N)));
+        h->eval_bufs_ready = true;   // only now: a failed allocation above is retried by the next build
     }
     h->have_list = true;
     h->n_rebuilds++;
@@ -610,7 +612,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
                                     (float4 *)h->gst.p, (double *)h->Fc.p, virial ? (double *)h->vir_part.p : nullptr,
                                     ch_atom[(size_t)c], ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
             if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
-            mk.mark(7);
+            mk.mark(t >= 1 ? 7 : 9);
             // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after
             if (t >= 1 || c == C - 1)
                 launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
@@ -645,6 +647,12 @@ extern "C" int reann_get_neighbors(reann_t *h, int64_t *n_edges, int64_t *row_pt
     return neighbor_export(h, n_edges, row_ptr, j, shift);
 }
 
+extern "C" int reann_get_neighbor_rows(reann_t *h, int64_t n_sel, const int64_t *atoms, int64_t *row_ptr, int32_t *j,
+                                       int8_t *shift) {
+    if (!h) return REANN_ERR_ARG;
+    return neighbor_export_rows(h, n_sel, atoms, row_ptr, j, shift);
+}
+
 extern "C" int reann_get_stats(reann_t *h, reann_stats_t *out) {
     if (!h || !out) return REANN_ERR_ARG;
     memset(out, 0, sizeof(*out));
@@ -653,6 +661,7 @@ extern "C" int reann_get_stats(reann_t *h, reann_stats_t *out) {
     out->ms_build = h->ms[0]; out->ms_prep = h->ms[1]; out->ms_edge_fwd = h->ms[2]; out->ms_dense_fwd = h->ms[3];
     out->ms_gather = h->ms[4]; out->ms_dense_bwd = h->ms[5]; out->ms_edge_bwd = h->ms[6]; out->ms_rev_gather = h->ms[7];
     out->ms_output = h->ms[8]; out->n_profiled_calls = h->n_prof_calls; out->bytes_device = h->bytes_device;
+    out->ms_rev_gather_t0 = h->ms[9]; out->stash_chunks = h->stash_chunks;
     return REANN_OK;
 }
 

@@ -97,6 +97,7 @@ void exclusive_scan_i32_to_i64(const LaunchCtx &ctx, const int32_t *in, int64_t 
 struct reann; // handle (api.cu)
 int neighbor_build(reann *h, const double *d_pos);   // returns REANN_* code
 int neighbor_export(reann *h, int64_t *n_edges, int64_t *row_ptr, int32_t *j, int8_t *shift);
+int neighbor_export_rows(reann *h, int64_t n_sel, const int64_t *atoms, int64_t *row_ptr, int32_t *j, int8_t *shift);
 
 // ---- edge.cu ----
 void launch_skin_check(const LaunchCtx &ctx, const double *pos, const double *pos_build, int64_t N, double thr2,

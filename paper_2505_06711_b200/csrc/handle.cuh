@@ -26,6 +26,7 @@ struct reann {
 
     // ---- neighbour list, rebuilt on demand ----
     bool have_list = false;
+    bool eval_bufs_ready = false;  // every per-evaluation buffer of do_build() is allocated
     double box_build[9]{};
     int64_t G = 0, n_ext = 0, E_list = 0, E_rc_build = 0;
     DevBuf pos_build;             // double [N][3], caller order
@@ -72,7 +73,7 @@ struct reann {
     // ---- stats / profiling ----
     int64_t n_rebuilds = 0, n_calls = 0, n_prof_calls = 0;
     bool profiling = false;
-    double ms[9]{};               // build, prep, edge_fwd, dense_fwd, gather, dense_bwd, edge_bwd, rev_gather, output
+    double ms[10]{};              // build, prep, edge_fwd, dense_fwd, gather, dense_bwd, edge_bwd, rev_gather (t >= 1), output, rev_gather (t = 0)
     std::vector<cudaEvent_t> ev;  // event pool
     size_t bytes_device = 0;
 

@@ -251,6 +251,32 @@ __global__ void k_species_scatter(const XRec *__restrict__ xrec, int64_t N, int 
     if (k < N && xrec[k].species == s) sp_list[base + off[k]] = (int32_t)k;
 }
 
+// Introspection: rows of selected atoms (caller indices) in the caller's order and frame, one warp per row.
+// pass 0 (j_out == nullptr): cnt[k] = length of the row; pass 1: entries written from off[k] on.
+__global__ void __launch_bounds__(128) k_export_rows(const XRec *__restrict__ xrec, const int64_t *__restrict__ row_ptr,
+                                                     const int32_t *__restrict__ col, const int32_t *__restrict__ perm,
+                                                     const int32_t *__restrict__ inv_perm,
+                                                     const int32_t *__restrict__ wshift, int64_t n_sel,
+                                                     const int64_t *__restrict__ atoms, int64_t *__restrict__ cnt,
+                                                     const int64_t *__restrict__ off, int32_t *__restrict__ j_out,
+                                                     int8_t *__restrict__ shift_out) {
+    const int lane = threadIdx.x & 31;
+    const int64_t k = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (k >= n_sel) return;
+    const int64_t i = atoms[k], ki = inv_perm[i];
+    const int64_t r0 = row_ptr[ki], r1 = row_ptr[ki + 1];
+    if (!j_out) { if (lane == 0) cnt[k] = r1 - r0; return; }
+    for (int64_t e = r0 + lane; e < r1; e += 32) {
+        const XRec r = xrec[col[e]];
+        const int32_t jc = perm[r.owner];
+        const int64_t o = off[k] + (e - r0);
+        j_out[o] = jc;
+        shift_out[3 * o + 0] = (int8_t)(r.sx + wshift[3 * i + 0] - wshift[3 * (int64_t)jc + 0]);
+        shift_out[3 * o + 1] = (int8_t)(r.sy + wshift[3 * i + 1] - wshift[3 * (int64_t)jc + 1]);
+        shift_out[3 * o + 2] = (int8_t)(r.sz + wshift[3 * i + 2] - wshift[3 * (int64_t)jc + 2]);
+    }
+}
+
 uint32_t morton3(uint32_t x, uint32_t y, uint32_t z) {
     auto spread = [](uint64_t v) {
         v &= 0x1fffff;
@@ -436,5 +462,51 @@ int neighbor_export(reann *h, int64_t *n_edges, int64_t *row_ptr_out, int32_t *j
             shift_out[3 * o + 2] = (int8_t)(r.sz + wsh[3 * (size_t)i + 2] - wsh[3 * (size_t)jc + 2]);
         }
     }
+    return REANN_OK;
+}
+
+
+// Rows of selected atoms only (for sampled pair-set parity on systems whose full list is too large to export).
+int neighbor_export_rows(reann *h, int64_t n_sel, const int64_t *atoms, int64_t *row_ptr_out, int32_t *j_out,
+                         int8_t *shift_out) {
+    if (!h->have_list) return set_err(h, REANN_ERR_NO_NEIGHBORS, "no neighbour list built yet");
+    if (n_sel < 0 || !atoms || !row_ptr_out || (!!j_out != !!shift_out)) return set_err(h, REANN_ERR_ARG, "bad argument");
+    for (int64_t k = 0; k < n_sel; ++k)
+        if (atoms[k] < 0 || atoms[k] >= h->N) return set_err(h, REANN_ERR_ARG, "atom index out of range");
+    row_ptr_out[0] = 0;
+    if (n_sel == 0) return REANN_OK;
+    LaunchCtx ctx = h->ctx();
+    DevBuf d_atoms, d_cnt, d_off, d_j, d_sh;
+    auto cleanup = [&]() { for (DevBuf *b : {&d_atoms, &d_cnt, &d_off, &d_j, &d_sh}) if (b->p) { cudaFree(b->p); h->bytes_device -= b->bytes; b->p = nullptr; } };
+#define XRC(call) do { int r_ = (call); if (r_ != REANN_OK) { cleanup(); return r_; } } while (0)
+#define XCU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return set_err(h, REANN_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); } } while (0)
+    XRC(dev_ensure(h, d_atoms, sizeof(int64_t) * (size_t)n_sel));
+    XRC(dev_ensure(h, d_cnt, sizeof(int64_t) * (size_t)n_sel));
+    XRC(dev_ensure(h, d_off, sizeof(int64_t) * (size_t)n_sel));
+    XCU(cudaMemcpyAsync(d_atoms.p, atoms, sizeof(int64_t) * (size_t)n_sel, cudaMemcpyHostToDevice, h->stream));
+    LAUNCH(ctx, k_export_rows, div_up(n_sel, 4), 128, 0, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p,
+           (const int32_t *)h->col.p, (const int32_t *)h->perm.p, (const int32_t *)h->inv_perm.p,
+           (const int32_t *)h->wshift.p, n_sel, (const int64_t *)d_atoms.p, (int64_t *)d_cnt.p, (const int64_t *)nullptr,
+           (int32_t *)nullptr, (int8_t *)nullptr);
+    std::vector<int64_t> cnt((size_t)n_sel);
+    XCU(cudaMemcpyAsync(cnt.data(), d_cnt.p, sizeof(int64_t) * (size_t)n_sel, cudaMemcpyDeviceToHost, h->stream));
+    XCU(cudaStreamSynchronize(h->stream));
+    for (int64_t k = 0; k < n_sel; ++k) row_ptr_out[k + 1] = row_ptr_out[k] + cnt[(size_t)k];
+    const int64_t tot = row_ptr_out[n_sel];
+    if (j_out && tot > 0) {
+        XRC(dev_ensure(h, d_j, sizeof(int32_t) * (size_t)tot));
+        XRC(dev_ensure(h, d_sh, 3 * (size_t)tot));
+        XCU(cudaMemcpyAsync(d_off.p, row_ptr_out, sizeof(int64_t) * (size_t)n_sel, cudaMemcpyHostToDevice, h->stream));
+        LAUNCH(ctx, k_export_rows, div_up(n_sel, 4), 128, 0, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p,
+               (const int32_t *)h->col.p, (const int32_t *)h->perm.p, (const int32_t *)h->inv_perm.p,
+               (const int32_t *)h->wshift.p, n_sel, (const int64_t *)d_atoms.p, (int64_t *)d_cnt.p,
+               (const int64_t *)d_off.p, (int32_t *)d_j.p, (int8_t *)d_sh.p);
+        XCU(cudaMemcpyAsync(j_out, d_j.p, sizeof(int32_t) * (size_t)tot, cudaMemcpyDeviceToHost, h->stream));
+        XCU(cudaMemcpyAsync(shift_out, d_sh.p, 3 * (size_t)tot, cudaMemcpyDeviceToHost, h->stream));
+        XCU(cudaStreamSynchronize(h->stream));
+    }
+    cleanup();
+#undef XRC
+#undef XCU
     return REANN_OK;
 }

@@ -84,3 +84,21 @@ def test_box_errors(cfg1):
     tric = cfg1["box"].copy(); tric[1] = 0.3
     with pytest.raises(ValueError):
         oracle.neighbors(cfg1["pos"], tric, 7.0)            # non-orthorhombic unsupported
+
+
+@pytest.mark.parametrize("which", ["cfg1", "w260", "slab"])
+def test_selected_rows_equal_the_bruteforce_rows(which, cfg1):
+    """oracle.neighbor_rows (rows of selected atoms only; used for sampled pair-set parity on systems whose
+    full list does not fit the host) against the O(N^2 27) brute-force list, unwrapped positions included."""
+    if which == "cfg1":
+        pos, box, R = cfg1["pos"] + np.array([31.0, -17.0, 5.5]), cfg1["box"], cfg1["rc"] + cfg1["skin"]
+    elif which == "w260":
+        c = gen.make_config(2, n_mol=260, geometry_only=True); pos, box, R = c["pos"], c["box"], 6.5
+    else:
+        c = gen.make_config(5, n_mol=300, geometry_only=True); pos, box, R = c["pos"], c["box"], 8.0
+    full = oracle.neighbors(pos, box, R, "brute")
+    sel = np.unique(np.random.default_rng(4).integers(0, len(pos), 40))
+    rows, row_ptr = oracle.neighbor_rows(pos, box, R, sel)
+    want = full[np.isin(full[:, 0], sel)]
+    assert rows.shape == want.shape and (rows == want).all()
+    assert row_ptr[-1] == len(rows) and (np.diff(row_ptr) == [(full[:, 0] == i).sum() for i in sel]).all()
