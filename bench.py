@@ -62,20 +62,40 @@ def aggregate_throughput(n_units_per_rank: int, steps: int, ms_total_local: floa
     return world * n_units_per_rank * steps / (ms * 1e-3), ms / steps
 
 
-def load_traffic(k: int) -> dict:
+def csrc_sha() -> str:
+    """sha256 (first 16 hex digits) over the CUDA sources: ties an ncu capture to the kernels it was taken on."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2505_06711_b200", "csrc")
+    hsh = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, f), "rb") as fh:
+                hsh.update(f.encode() + b"\0" + fh.read())
+    return hsh.hexdigest()[:16]
+
+
+def load_traffic(k: int) -> tuple[dict, str]:
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture) of
-    the kernel groups, from the committed profile summary; only valid for the config it was captured on."""
-    p = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
-    out = {}
-    if os.path.exists(p):
-        with open(p) as f:
-            for line in f:
-                if line.startswith("#") or not line.strip():
-                    continue
-                group, cfg, nbytes = line.strip().split(",")[:3]
-                if group != "group" and int(cfg) == k:
-                    out[group] = float(nbytes)
-    return out
+    the kernel groups, from the newest committed profiles/r*_dram_traffic.csv. A capture is only reported for the
+    config it was taken on AND when its `# csrc_sha=` line equals the hash of the current kernel sources; otherwise
+    `traffic` is null and the note says which capture is stale."""
+    pdir = os.path.join(ROOT, "profiles")
+    files = sorted(f for f in os.listdir(pdir) if f.endswith("_dram_traffic.csv")) if os.path.isdir(pdir) else []
+    if not files:
+        return {}, "no capture committed"
+    out, sha = {}, None
+    with open(os.path.join(pdir, files[-1])) as f:
+        for line in f:
+            if line.startswith("# csrc_sha="):
+                sha = line.split("=", 1)[1].strip()
+            if line.startswith("#") or not line.strip():
+                continue
+            group, cfg, nbytes = line.strip().split(",")[:3]
+            if group != "group" and int(cfg) == k:
+                out[group] = float(nbytes)
+    if sha != csrc_sha():
+        return {}, f"profiles/{files[-1]} was captured on kernel sources {sha}, current sources are {csrc_sha()}: stale, not reported"
+    return out, f"profiles/{files[-1]} (csrc_sha {sha})"
 
 
 class ClockSampler:
@@ -208,17 +228,32 @@ def main():
     F = torch.zeros((n, 3), dtype=torch.float64, device="cuda")
     box = cfg["box"]
 
+    vir = torch.zeros(9, dtype=torch.float64, device="cuda")
+
     def md_step():
         m.verlet(pos, vel, F, inv_m, dt_fs, acc, True)
-        m.energy_forces(pos, box, E, F)
+        m.energy_forces(pos, box, E, F, vir)               # the full boundary call: E, F and the virial
         m.verlet(pos, vel, F, inv_m, dt_fs, acc, False)
+
+    def timed(fn, reps=1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
 
     # nvidia-smi takes a few hundred ms to attach to the driver and holds up CUDA calls while it does: start it
     # before the warm-up and wait for its first sample, so that only its periodic queries fall in the timed region
     sampler = ClockSampler(local_rank)
     sampler.start()
     m.build_neighbors(pos, box)
-    m.energy_forces(pos, box, E, F)
+    m.energy_forces(pos, box, E, F, vir)
+    # ---- "single evaluation incl. build" (BASELINE config 3; SURVEY 8(d) timing protocol): median of 5 ----
+    t_build = sorted(timed(lambda: m.build_neighbors(pos, box)) for _ in range(5))[2]
+    t_single = sorted(timed(lambda: (m.build_neighbors(pos, box), m.energy_forces(pos, box, E, F, vir))) for _ in range(5))[2]
     for _ in range(W):
         md_step()
     torch.cuda.synchronize()
@@ -228,8 +263,8 @@ def main():
     torch.cuda.synchronize()
     sampler.rows.clear()
 
-    # ---------------- device-resident timed region ----------------
-    m.set_profiling(True)
+    # ---------------- device-resident timed region (profiling OFF: the production path) ----------------
+    m.set_profiling(False)
     s0 = m.stats()
     if world > 1:
         dist.barrier()
@@ -247,17 +282,25 @@ def main():
     ms_total = ms_step * K
     clocks = sampler.stop()
     s1 = m.stats()
+
+    # ---------------- second, separate pass with per-group CUDA events (one more host sync per step) ----------------
+    Kp = max(3, min(K, 20))
+    m.set_profiling(True)
+    p0 = m.stats()
+    ms_prof = timed(md_step, Kp)
+    p1 = m.stats()
     m.set_profiling(False)
 
     # ---------------- end-to-end leg: host buffers through the C ABI ----------------
     # replay: positions of an MD trajectory advanced on the host side of the boundary (pinned memory);
-    # every step copies pos H2D inside reann_energy_forces and E, F back D2H.
+    # every step copies pos H2D inside reann_energy_forces and E, F, virial back D2H.
     pos_h = torch.empty((n, 3), dtype=torch.float64).pin_memory()
     F_h = torch.empty((n, 3), dtype=torch.float64).pin_memory()
     E_h = torch.empty(1, dtype=torch.float64).pin_memory()
+    V_h = torch.empty(9, dtype=torch.float64).pin_memory()
     pos_h.copy_(pos.cpu()); vel_h = vel.cpu().numpy().copy(); inv_m_h = (1.0 / cfg["masses"])[:, None]
-    pos_np, F_np, E_np = pos_h.numpy(), F_h.numpy(), E_h.numpy()
-    m.energy_forces(pos_np, box, E_np, F_np)
+    pos_np, F_np, E_np, V_np = pos_h.numpy(), F_h.numpy(), E_h.numpy(), V_h.numpy()
+    m.energy_forces(pos_np, box, E_np, F_np, V_np)
     Ke = max(3, min(K, 10))
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -266,30 +309,37 @@ def main():
     for _ in range(Ke):
         np.multiply(F_np, half_kick, out=tmp); vel_h += tmp   # host-side integrator (caller's job in e2e use)
         np.multiply(vel_h, dt_fs, out=tmp); pos_np += tmp
-        m.energy_forces(pos_np, box, E_np, F_np)              # H2D pos, kernels, D2H E/F, stream sync
+        m.energy_forces(pos_np, box, E_np, F_np, V_np)        # H2D pos, kernels, D2H E/F/virial, stream sync
         np.multiply(F_np, half_kick, out=tmp); vel_h += tmp
     t_e2e = time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e)
     e2e = {"value": world * n * Ke / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(n * 24),
-           "d2h_bytes_per_step": int(n * 24 + 8), "steps": Ke}
+           "d2h_bytes_per_step": int(n * 24 + 8 + 72), "steps": Ke}
 
     if rank == 0:
         peaks = load_peaks()
-        ncalls = max(1, s1["n_profiled_calls"] - s0["n_profiled_calls"])
-        groups = {g: (s1[g] - s0[g]) / ncalls for g in ("ms_prep", "ms_edge_fwd", "ms_dense_fwd", "ms_gather",
-                                                        "ms_dense_bwd", "ms_edge_bwd", "ms_rev_gather", "ms_output")}
+        ncalls = max(1, p1["n_profiled_calls"] - p0["n_profiled_calls"])
+        groups = {g: (p1[g] - p0[g]) / ncalls for g in ("ms_prep", "ms_edge_fwd", "ms_dense_fwd", "ms_gather",
+                                                        "ms_dense_bwd", "ms_edge_bwd", "ms_rev_gather",
+                                                        "ms_rev_gather_t0", "ms_output")}
         T, nphi, L = cfg["T"], cfg["n_gauss"], cfg["L"]
+        nphip = (nphi + 3) // 4 * 4
         Na = gen.n_monomials(L)
-        E_rc = s1["n_edges_rc"]
+        E_rc, E_list, n_ext = s1["n_edges_rc"], s1["n_edges_list"], s1["n_ext"]
         H1, H2 = cfg["H"]
         n_q = gen.n_orb_default(nphi, L)
-        # algorithmic work per launch (one layer), SURVEY.md 8(d) / DESIGN.md section 6: 1 FMA = 2 flop.
-        # dense groups = gram kernel + tensor-core chain; n_out is N_phi for the T-1 coefficient layers, 1 for the last
+        # Algorithmic work PER LAUNCH and launches per step of every kernel group (SURVEY.md 8(d) per-unit figures x
+        # units): 1 FMA = 2 flop. dense groups = contraction (radial-pair form) + MLP GEMMs;
+        # n_out is N_phi for the T-1 coefficient layers and 1 for the last. rev_gather has two launch kinds: layers
+        # t >= 1 read rev (4 B) + g_e (16 B) + kappa_e (4 N_phi B) per edge and write cbar; the t = 0 launch reads
+        # rev + g_e only (c^0 is constant) and writes nothing per atom but the forces.
         nout_avg = ((T - 1) * nphi + 1) / T
         dense_flops = 2.0 * n * (n_q * H1 + H1 * H2 + H2 * nout_avg)
-        work = {"ms_edge_fwd": ("alu", 2.0 * E_rc * nphi * Na), "ms_edge_bwd": ("alu", 4.0 * E_rc * nphi * Na),
-                "ms_dense_fwd": ("tensor", dense_flops), "ms_dense_bwd": ("tensor", dense_flops),
-                "ms_rev_gather": ("hbm", float(E_rc) * (4 * nphi + 16 + 4) + n * (4 * nphi + 24))}
+        work = {"ms_edge_fwd": ("alu", 2.0 * E_rc * nphi * Na, T), "ms_edge_bwd": ("alu", 4.0 * E_rc * nphi * Na, T),
+                "ms_dense_fwd": ("tensor", dense_flops, T), "ms_dense_bwd": ("tensor", dense_flops, T),
+                "ms_rev_gather_t0": ("hbm", float(E_rc) * (4 + 16) + n * 24.0, 1)}
+        if T > 1:
+            work["ms_rev_gather"] = ("hbm", float(E_rc) * (4 * nphip + 16 + 4) + n * (4.0 * nphip + 8), T - 1)
         sm_max = peaks.get("sm_max_mhz", 1965.0)
         alu_peak = N_SM * FP32_FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         # TF32 peak = measured BF16 dense peak x the guide's nominal TF32/BF16 ratio (1.13 / 2.25 PFLOP/s);
@@ -298,21 +348,33 @@ def main():
         peak_of = {"alu": (alu_peak, "TFLOP/s", f"148 SM x 128 FP32 FMA lanes x 2 x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)"),
                    "tensor": (tf32_peak, "TFLOP/s", f"0.5 x {peaks['_source']} sustained BF16 cuBLAS peak (TF32 nominal ratio)"),
                    "hbm": (peaks["hbm_gbs"], "GB/s", f"{peaks['_source']} HBM copy bandwidth")}
-        traffic = load_traffic(args.config)
+        traffic, traffic_note = load_traffic(args.config)
 
         def roof(g):
-            bound, amount = work[g]
-            ms = groups[g] / T
+            bound, amount, launches = work[g]
+            ms = groups[g] / launches
             peak, unit, src = peak_of[bound]
             ach = amount / (ms * 1e-3) / (1e9 if bound == "hbm" else 1e12) if ms > 0 else 0.0
             return {"bound": bound, "kernel": g.replace("ms_", ""), "achieved": ach, "peak": peak, "unit": unit,
                     "frac": ach / peak, "traffic": traffic.get(g.replace("ms_", "")), "peak_source": src,
-                    "ms_per_launch": ms, "launches_per_step": T}
+                    "ms_per_launch": ms, "launches_per_step": launches,
+                    "algorithmic_per_launch": amount, "algorithmic_unit": "bytes" if bound == "hbm" else "flop"}
 
         dom = max(work, key=lambda g: groups[g])
         roofline = roof(dom)
+        roofline["traffic_source"] = traffic_note
         roofline["ms_per_step_by_group"] = {k.replace("ms_", ""): v for k, v in groups.items()}
+        roofline["ms_per_step_by_group"]["note"] = (f"separate profiled pass of {Kp} steps at {ms_prof:.3f} ms/step "
+                                                    "(per-group CUDA events add one host sync per step); `value` is timed with profiling off")
         roofline["other_kernels"] = [roof(g) for g in work if g != dom]
+        # neighbour build (A1-A3), per rebuild: HBM bound; algorithmic bytes = positions in (24 B/atom) + ext records
+        # (32 B each) + CSR col and rev written (4 + 4 B per list entry) + row_ptr (8 B/atom)
+        nb_bytes = 24.0 * n + 32.0 * n_ext + 8.0 * E_list + 8.0 * n
+        roofline["other_kernels"].append({"bound": "hbm", "kernel": "neighbor_build", "achieved": nb_bytes / (t_build * 1e-3) / 1e9,
+                                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": nb_bytes / (t_build * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                          "traffic": None, "peak_source": peak_of["hbm"][2], "ms_per_launch": t_build,
+                                          "launches_per_step": (s1["n_rebuilds"] - s0["n_rebuilds"]) / K,
+                                          "algorithmic_per_launch": nb_bytes, "algorithmic_unit": "bytes"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
@@ -320,9 +382,12 @@ def main():
                                        f"T={T}, L={L}, n_gauss={nphi}, MLP {H1}x{H2}), velocity-Verlet 0.5 fs at 300 K",
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "working set (compact edge list + stash, >300 MB) exceeds the 126 MB L2; no flush needed",
+                           "virial": True, "profiling_in_timed_region": False,
                            "rebuilds_in_timed_region": s1["n_rebuilds"] - s0["n_rebuilds"],
-                           "n_edges_rc": E_rc, "n_edges_list": s1["n_edges_list"], "n_ext": s1["n_ext"],
-                           "device_bytes": s1["bytes_device"]},
+                           "n_edges_rc": E_rc, "n_edges_list": E_list, "n_ext": n_ext,
+                           "stash_chunks": s1["stash_chunks"], "device_bytes": s1["bytes_device"]},
+                "single_eval": {"ms": t_single, "value": n / (t_single * 1e-3), "unit": UNIT, "ms_build": t_build,
+                                "what": "reann_build_neighbors + one reann_energy_forces (E, F, virial), device pointers, median of 5"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": s1["n_launches"] - s0["n_launches"],
                 "roofline": roofline}
         if not args.no_cpu_baseline:
