@@ -179,8 +179,11 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
     md.npairs = n_gauss * (n_gauss + 1) / 2; md.NPp = md.npairs; md.nqp = ((L + 1) * md.NPp + 15) & ~15;
     md.K1 = (md.nqp + 31) & ~31;
     {
-        const char *e = getenv("REANN_DENSE");
-        h->dense_tc = !(e && strcmp(e, "simt") == 0);
+        auto is = [](const char *name, const char *val) { const char *e = getenv(name); return e && strcmp(e, val) == 0; };
+        h->dense_tc = !is("REANN_DENSE", "simt");
+        h->edge_fwd_mma = !is("REANN_EDGE_FWD", "simt");
+        h->edge_bwd_tc = !is("REANN_EDGE", "simt") && edge_bwd_tc_supported(md);
+        if (const char *e = getenv("REANN_STASH_CHUNKS")) h->stash_chunks_forced = std::max(0, atoi(e));
     }
     md.rc = rc; md.skin = skin;
     h->zs = 0;
@@ -425,7 +428,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
-        h->n_vir_blocks = edge_bwd_blocks(std::max<int64_t>(N, 1));
+        h->n_vir_blocks = std::max(edge_bwd_blocks(std::max<int64_t>(N, 1)), edge_bwd_tc_blocks(std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->vir_part, sizeof(double) * 9 * (size_t)h->n_vir_blocks));
         RC(dev_ensure(h, h->red_scratch, sizeof(double) * ((size_t)N / 256 + 2)));
         RC(dev_ensure(h, h->out_stage, sizeof(double) * (16 + 3 * (size_t)N)));
@@ -532,7 +535,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         CU(h, cudaMemGetInfo(&free_b, &total_b));
         const size_t budget = free_b > ((size_t)3 << 30) ? free_b - ((size_t)3 << 30) : free_b / 2;
         int C = 1;
-        if (const char *e = getenv("REANN_STASH_CHUNKS")) C = std::max(1, atoi(e));
+        if (h->stash_chunks_forced > 0) C = h->stash_chunks_forced;
         else while (C < 64 && (C == 1 ? whole : whole / C + whole / (8 * C)) > budget) ++C;
         h->stash_chunks = C;
         RC(dev_ensure(h, h->kappa, C == 1 ? whole : whole / C + whole / (8 * C)));
@@ -566,7 +569,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         mk.mark(2);
         int rcode = launch_edge_fwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
                                     (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
-                                    (const float *)h->alpha.p, b + t * bstride);
+                                    (const float *)h->alpha.p, b + t * bstride, h->edge_fwd_mma);
         if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
         mk.mark(3);
         const bool last = t == md.T - 1;
@@ -606,11 +609,11 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         mk.mark(6);
         for (int c = 0; c < C; ++c) {
             if (c > 0) mk.mark(6);
-            rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
-                                    (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
-                                    (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
-                                    (float4 *)h->gst.p, (double *)h->Fc.p, virial ? (double *)h->vir_part.p : nullptr,
-                                    ch_atom[(size_t)c], ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
+            rcode = (h->edge_bwd_tc ? launch_edge_bwd_tc : launch_edge_bwd)(
+                ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p, (const float4 *)h->geom.p,
+                c_ext + t * cstride, (const float *)h->rcen.p, (const float *)h->alpha.p, (const float *)h->bbar.p,
+                (float *)h->kappa.p, (float4 *)h->gst.p, virial ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
+                ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
             if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
             mk.mark(t >= 1 ? 7 : 9);
             // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after

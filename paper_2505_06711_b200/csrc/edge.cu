@@ -16,8 +16,10 @@
 #include <string.h>
 
 #include "common.cuh"
+#include "edge_common.cuh"
 
 namespace {
+using namespace edge;
 
 constexpr int EW = 4; // warps per block in the edge kernels
 
@@ -153,63 +155,6 @@ __global__ void k_ghost_gather(float *__restrict__ c_ext, const XRec *__restrict
     const float4 *src = reinterpret_cast<const float4 *>(c_ext + (int64_t)xrec[g].owner * nphip);
     reinterpret_cast<float4 *>(c_ext + g * nphip)[part] = src[part];
 }
-
-// ------------------------------------------------------------------------------------------ orbitals
-// Cartesian monomials in graded order: 1 | x y z | xx xy xz yy yz zz | xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz
-template <int NA>
-__device__ __forceinline__ void monomials(float x, float y, float z, float *A) {
-    A[0] = 1.0f;
-    if constexpr (NA > 1) { A[1] = x; A[2] = y; A[3] = z; }
-    if constexpr (NA > 4) { A[4] = x * x; A[5] = x * y; A[6] = x * z; A[7] = y * y; A[8] = y * z; A[9] = z * z; }
-    if constexpr (NA > 10) {
-        A[10] = A[4] * x; A[11] = A[4] * y; A[12] = A[4] * z; A[13] = A[7] * x; A[14] = A[5] * z;
-        A[15] = A[9] * x; A[16] = A[7] * y; A[17] = A[7] * z; A[18] = A[9] * y; A[19] = A[9] * z;
-    }
-}
-// sum_a P_a grad A_a
-template <int NA>
-__device__ __forceinline__ void monomial_vjp(const float *A, const float *P, float &gx, float &gy, float &gz) {
-    gx = gy = gz = 0.0f;
-    if constexpr (NA > 1) { gx = P[1]; gy = P[2]; gz = P[3]; }
-    if constexpr (NA > 4) {
-        const float x = A[1], y = A[2], z = A[3];
-        gx += 2.0f * x * P[4] + y * P[5] + z * P[6];
-        gy += x * P[5] + 2.0f * y * P[7] + z * P[8];
-        gz += x * P[6] + y * P[8] + 2.0f * z * P[9];
-    }
-    if constexpr (NA > 10) {
-        gx += 3.0f * A[4] * P[10] + 2.0f * A[5] * P[11] + 2.0f * A[6] * P[12] + A[7] * P[13] + A[8] * P[14] + A[9] * P[15];
-        gy += A[4] * P[11] + 2.0f * A[5] * P[13] + A[6] * P[14] + 3.0f * A[7] * P[16] + 2.0f * A[8] * P[17] + A[9] * P[18];
-        gz += A[4] * P[12] + A[5] * P[14] + 2.0f * A[6] * P[15] + A[7] * P[17] + 2.0f * A[8] * P[18] + 3.0f * A[9] * P[19];
-    }
-}
-
-// Packed FP32 pairs: Blackwell's fma.rn.f32x2 (SASS FFMA2) does two FP32 FMAs per issue slot at the same FLOP
-// rate (measured 74 TFLOP/s either way), which halves the instruction count of the FMA loops below.
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ void ffma2(f32x2 &c, f32x2 a, f32x2 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
-__device__ __forceinline__ f32x2 fmadd2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-
-__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-
-struct StashChunk { // reverse gather: kappa holds the edges [e_lo, e_hi); forces once; cbar = or +=
-    int64_t e_lo, e_hi;
-    int do_forces, accumulate;
-};
-struct AtomChunk { // edge backward: atoms [a0, a1) (a0 % EW == 0); kappa holds the edges from e_lo on
-    int64_t a0, a1, e_lo;
-};
-struct RadialTab { // per layer: [S][NPHIP]; alpha pre-multiplied by log2(e)
-    const float *rcen, *alpha2;
-    float inv_rc;
-};
 
 // ------------------------------------------------------------------------------------------ A5
 // Warp-autonomous: a warp owns APW = 32/LPA atoms; lane group `sub` (LPA lanes) owns atom `sub` and
@@ -492,7 +437,9 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
 // ------------------------------------------------------------------------------------------ A10
 // Warp per atom, one edge per lane; bbar_i is broadcast from shared memory, S_n and P_a stay in the
 // lane's registers, so there is no cross-lane reduction per edge. Orbitals are recomputed (nothing
-// per-edge is kept from the forward pass). Writes the per-edge stash g_e (float4) and kappa_e.
+// per-edge is kept from the forward pass). Writes the per-edge stash g_e (float4) and kappa_e; the forces are
+// gathered from the g_e stash by k_rev_gather. This FP32 ALU kernel serves the shapes the tcgen05 kernel of
+// edge_tc.cu does not (N_phi = 4, L = 0) and is its accuracy yardstick (REANN_EDGE=simt).
 // The radial tables sit in shared memory; c_j and the next pass's edge record are prefetched one
 // step ahead so that no global-load latency is exposed inside the FMA loop. VIR: accumulate the
 // virial (only when the caller asked for it).
@@ -503,8 +450,7 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
                                                       const float *__restrict__ c_ext, RadialTab rt, int S,
                                                       const float *__restrict__ bbar, int want_kappa,
                                                       float *__restrict__ kappa, float4 *__restrict__ gst,
-                                                      double *__restrict__ Fc, double *__restrict__ vir_part,
-                                                      AtomChunk ch) {
+                                                      double *__restrict__ vir_part, AtomChunk ch) {
     constexpr int NB = NPHIP * NA;
     __shared__ __align__(16) float bb_s[EW][NB];
     __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
@@ -513,7 +459,7 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
     const int64_t i0 = ch.a0 + (int64_t)blockIdx.x * EW + warp;
     const int64_t i = i0 < ch.a1 ? i0 : N;              // atoms [a0, a1) of this launch
     for (int k = threadIdx.x; k < S * NPHIP; k += EW * 32) { tab_s[0][k] = rt.rcen[k]; tab_s[1][k] = rt.alpha2[k]; }
-    float aF[3] = {0.f, 0.f, 0.f}, aV[VIR ? 9 : 1];
+    float aV[VIR ? 9 : 1];
 #pragma unroll
     for (int k = 0; k < (VIR ? 9 : 1); ++k) aV[k] = 0.f;
     if (i < N) {
@@ -625,7 +571,6 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
             const float rr = __fdividef(radial, g.w);
             gx = fmaf(rr, g.x, gx); gy = fmaf(rr, g.y, gy); gz = fmaf(rr, g.z, gz);
             gst[e] = make_float4(gx, gy, gz, 0.f);
-            aF[0] += gx; aF[1] += gy; aF[2] += gz;
             if constexpr (VIR) {
                 aV[0] -= g.x * gx; aV[1] -= g.x * gy; aV[2] -= g.x * gz;
                 aV[3] -= g.y * gx; aV[4] -= g.y * gy; aV[5] -= g.y * gz;
@@ -635,254 +580,12 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
         }
     }
     // fixed-order reductions: lanes (butterfly, FP32), then FP64 accumulation across layers / warps
-#pragma unroll
-    for (int d = 16; d >= 1; d >>= 1) {
-#pragma unroll
-        for (int k = 0; k < 3; ++k) aF[k] += __shfl_xor_sync(0xffffffffu, aF[k], d);
-        if constexpr (VIR) {
-#pragma unroll
-            for (int k = 0; k < 9; ++k) aV[k] += __shfl_xor_sync(0xffffffffu, aV[k], d);
-        }
-    }
-    if (lane == 0 && i < N) { Fc[3 * i] += (double)aF[0]; Fc[3 * i + 1] += (double)aF[1]; Fc[3 * i + 2] += (double)aF[2]; }
     if constexpr (VIR) {
-        if (lane == 0) {
 #pragma unroll
-            for (int k = 0; k < 9; ++k) vir_s[warp][k] = aV[k];
-        }
-        __syncthreads();
-        if (threadIdx.x < 9) {
-            double s = 0.0;
-#pragma unroll
-            for (int w = 0; w < EW; ++w) s += (double)vir_s[w][threadIdx.x];
-            vir_part[(ch.a0 / EW + (int64_t)blockIdx.x) * 9 + threadIdx.x] += s;
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------ A10 (MMA)
-// The same edge backward step with the two per-atom products on the tensor cores:
-//   S[e,n] = sum_a A[e,a] T[n,a],   P[e,a] = sum_n X[e,n] T[n,a],   T = bbar_i  (N_phi x N_a, fixed per atom)
-// as warp-level mma.sync m16n8k8 TF32 with 3xTF32 splitting (lo.hi + hi.lo first, then hi.hi; chains of
-// <= 9 accumulation steps into fresh accumulators). Measured on B200: 0.46 mma.sync/clk/SM = 471 TF32
-// FMA/clk/SM against 128 FP32 FMA/clk/SM, and -- what matters more here -- T sits in registers as B
-// fragments for the whole atom instead of being re-read from shared memory for every edge.
-// Warp per atom, rounds of 32 edges: (1) one edge per lane: radial functions, monomials -> shared memory
-// rows (X | A); (2) two M = 16 edge tiles through the MMAs, S | P back to shared memory; (3) one edge
-// per lane again (R_n, y_n kept in registers): radial part, kappa_e, sum_a P_a grad A_a, g_e.
-template <int NPHIP, int NA>
-struct BwdMma {
-    static constexpr int NAP = (NA + 7) & ~7, NT = NPHIP / 8, AT = NAP / 8;
-    static constexpr int RS = NPHIP + NAP + 4;   // row stride = 4 mod 8 floats: conflict-free fragment loads and row stores
-    static constexpr int SMEM = EW * 2 * 32 * RS * 4;
-    static_assert(NPHIP % 8 == 0 && NT <= AT, "MMA edge kernels need N_phi % 8 == 0 and N_phi <= padded N_a");
-};
-
-template <int NPHIP, int NA, bool VIR>
-__global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd_mma(int64_t N, const int64_t *__restrict__ rc_ptr,
-                                                          const uint32_t *__restrict__ col_rc,
-                                                          const float4 *__restrict__ geom,
-                                                          const float *__restrict__ c_ext, RadialTab rt, int S,
-                                                          const float *__restrict__ bbar, int want_kappa,
-                                                          float *__restrict__ kappa, float4 *__restrict__ gst,
-                                                          double *__restrict__ Fc, double *__restrict__ vir_part,
-                                                          AtomChunk ch) {
-    using C = BwdMma<NPHIP, NA>;
-    constexpr int NB = NPHIP * NA, NAP = C::NAP, NT = C::NT, AT = C::AT, RS = C::RS;
-    extern __shared__ __align__(16) float smem_f[];
-    __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
-    __shared__ float vir_s[VIR ? EW : 1][9];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g8 = lane >> 2, t4 = lane & 3;
-    float *sin = smem_f + (size_t)warp * 2 * 32 * RS, *sout = sin + 32 * RS;
-    const int64_t i0 = ch.a0 + (int64_t)blockIdx.x * EW + warp;
-    const int64_t i = i0 < ch.a1 ? i0 : N;              // atoms [a0, a1) of this launch
-    for (int k = threadIdx.x; k < S * NPHIP; k += EW * 32) { tab_s[0][k] = rt.rcen[k]; tab_s[1][k] = rt.alpha2[k]; }
-    __syncthreads();
-    float aF[3] = {0.f, 0.f, 0.f}, aV[VIR ? 9 : 1];
-#pragma unroll
-    for (int k = 0; k < (VIR ? 9 : 1); ++k) aV[k] = 0.f;
-    if (i < N) {
-        // ---- B fragments of T = bbar_i, split once per atom ----
-        // S: k = a, n = n:  b0 = T[nt*8+g][ks*8+t], b1 = T[nt*8+g][ks*8+t+4];  P: k = n, n = a:  b0 = T[ks*8+t][at*8+g], b1 = T[ks*8+t+4][at*8+g]
-        const float *Ti = bbar + i * (int64_t)NB;
-        uint32_t bsh[AT][NT][2], bsl[AT][NT][2], bph[NT][AT][2], bpl[NT][AT][2];
-#pragma unroll
-        for (int ks = 0; ks < AT; ++ks)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int a = ks * 8 + t4 + 4 * h, n = nt * 8 + g8;
-                    split_bits(a < NA ? __ldg(Ti + n * NA + a) : 0.f, bsh[ks][nt][h], bsl[ks][nt][h]);
-                }
-#pragma unroll
-        for (int ks = 0; ks < NT; ++ks)
-#pragma unroll
-            for (int at = 0; at < AT; ++at)
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int n = ks * 8 + t4 + 4 * h, a = at * 8 + g8;
-                    split_bits(a < NA ? __ldg(Ti + n * NA + a) : 0.f, bph[ks][at][h], bpl[ks][at][h]);
-                }
-        const int64_t beg = rc_ptr[i], end = rc_ptr[i + 1];
-        const float pi_rc = 3.14159265358979f * rt.inv_rc;
-        float4 g_nx = make_float4(0.f, 0.f, 0.f, 1.f);
-        uint32_t cj_nx = 0;
-        if (beg + lane < end) { g_nx = geom[beg + lane]; cj_nx = col_rc[beg + lane]; }
-        for (int64_t e0 = beg; e0 < end; e0 += 32) {
-            const int64_t e = e0 + lane;
-            const bool have = e < end;
-            // ---- phase 1: one edge per lane (the record of the next round is fetched one round ahead) ----
-            const float4 g = g_nx;
-            const uint32_t cj = cj_nx;
-            if (e + 32 < end) { g_nx = geom[e + 32]; cj_nx = col_rc[e + 32]; }
-            float Rn[NPHIP], yn[NPHIP];
-            float *row = sin + lane * RS;
-            if (have) {
-                const int sj = cj >> COL_SPECIES_SHIFT;
-                const float4 *cptr = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
-                float sn, cs;
-                sincospif(g.w * rt.inv_rc, &sn, &cs);
-                const float fc = 0.5f + 0.5f * cs, dfc = -0.5f * pi_rc * sn;
-#pragma unroll
-                for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
-                    const float4 cv = cptr[n4];
-                    const float4 rc4 = reinterpret_cast<const float4 *>(tab_s[0] + sj * NPHIP)[n4];
-                    const float4 al4 = reinterpret_cast<const float4 *>(tab_s[1] + sj * NPHIP)[n4];
-                    const float cva[4] = {cv.x, cv.y, cv.z, cv.w}, rca[4] = {rc4.x, rc4.y, rc4.z, rc4.w},
-                                ala[4] = {al4.x, al4.y, al4.z, al4.w};
-                    float xq[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const float d = g.w - rca[u];
-                        const float ex = exp2f(-ala[u] * d * d);
-                        // alpha2 = alpha*log2(e): d/dr exp(-alpha d^2) = -2 ln2 alpha2 d ex
-                        Rn[n4 * 4 + u] = ex * fc;
-                        xq[u] = cva[u] * Rn[n4 * 4 + u];
-                        yn[n4 * 4 + u] = cva[u] * ((-1.3862943611198906f * ala[u] * d * fc + dfc) * ex);
-                    }
-                    reinterpret_cast<float4 *>(row)[n4] = make_float4(xq[0], xq[1], xq[2], xq[3]);
-                }
-                float A[NAP];
-#pragma unroll
-                for (int a = NA; a < NAP; ++a) A[a] = 0.f;
-                monomials<NA>(g.x, g.y, g.z, A);
-#pragma unroll
-                for (int a4 = 0; a4 < NAP / 4; ++a4)
-                    reinterpret_cast<float4 *>(row + NPHIP)[a4] = make_float4(A[4 * a4], A[4 * a4 + 1], A[4 * a4 + 2], A[4 * a4 + 3]);
-            } else {
-#pragma unroll
-                for (int q = 0; q < (NPHIP + NAP) / 4; ++q) reinterpret_cast<float4 *>(row)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-            }
-            __syncwarp();
-            // ---- phase 2: two tiles of 16 edges through the MMAs ----
-#pragma unroll
-            for (int mt = 0; mt < 2; ++mt) {
-                if (e0 + mt * 16 >= end) break;                       // warp-uniform
-                const float *r0 = sin + (mt * 16 + g8) * RS, *r1 = r0 + 8 * RS;
-                float *o0 = sout + (mt * 16 + g8) * RS, *o1 = o0 + 8 * RS;
-                // S = A T^T (K = a, NT chains) and P = X T (K = n, AT chains): the NT + AT accumulation chains are
-                // independent, so they are issued step by step side by side (corrections first, then hi.hi)
-                uint32_t sh[AT][4], sl[AT][4], ph[NT][4], pl[NT][4];
-#pragma unroll
-                for (int ks = 0; ks < AT; ++ks) {
-                    const int c = NPHIP + ks * 8 + t4;
-                    split_bits(r0[c], sh[ks][0], sl[ks][0]); split_bits(r1[c], sh[ks][1], sl[ks][1]);
-                    split_bits(r0[c + 4], sh[ks][2], sl[ks][2]); split_bits(r1[c + 4], sh[ks][3], sl[ks][3]);
-                }
-#pragma unroll
-                for (int ks = 0; ks < NT; ++ks) {
-                    const int c = ks * 8 + t4;
-                    split_bits(r0[c], ph[ks][0], pl[ks][0]); split_bits(r1[c], ph[ks][1], pl[ks][1]);
-                    split_bits(r0[c + 4], ph[ks][2], pl[ks][2]); split_bits(r1[c + 4], ph[ks][3], pl[ks][3]);
-                }
-                float ds[NT][4], dp[AT][4];
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) ds[nt][0] = ds[nt][1] = ds[nt][2] = ds[nt][3] = 0.f;
-#pragma unroll
-                for (int at = 0; at < AT; ++at) dp[at][0] = dp[at][1] = dp[at][2] = dp[at][3] = 0.f;
-#pragma unroll
-                for (int ks = 0; ks < AT; ++ks) {
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) mma_tf32(ds[nt], sl[ks], bsh[ks][nt][0], bsh[ks][nt][1]);
-                    if (ks < NT) {
-#pragma unroll
-                        for (int at = 0; at < AT; ++at) mma_tf32(dp[at], pl[ks], bph[ks][at][0], bph[ks][at][1]);
-                    }
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) mma_tf32(ds[nt], sh[ks], bsl[ks][nt][0], bsl[ks][nt][1]);
-                    if (ks < NT) {
-#pragma unroll
-                        for (int at = 0; at < AT; ++at) mma_tf32(dp[at], ph[ks], bpl[ks][at][0], bpl[ks][at][1]);
-                    }
-                }
-#pragma unroll
-                for (int ks = 0; ks < AT; ++ks) {
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) mma_tf32(ds[nt], sh[ks], bsh[ks][nt][0], bsh[ks][nt][1]);
-                    if (ks < NT) {
-#pragma unroll
-                        for (int at = 0; at < AT; ++at) mma_tf32(dp[at], ph[ks], bph[ks][at][0], bph[ks][at][1]);
-                    }
-                }
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) {
-                    *reinterpret_cast<float2 *>(o0 + nt * 8 + 2 * t4) = make_float2(ds[nt][0], ds[nt][1]);
-                    *reinterpret_cast<float2 *>(o1 + nt * 8 + 2 * t4) = make_float2(ds[nt][2], ds[nt][3]);
-                }
-#pragma unroll
-                for (int at = 0; at < AT; ++at) {
-                    *reinterpret_cast<float2 *>(o0 + NPHIP + at * 8 + 2 * t4) = make_float2(dp[at][0], dp[at][1]);
-                    *reinterpret_cast<float2 *>(o1 + NPHIP + at * 8 + 2 * t4) = make_float2(dp[at][2], dp[at][3]);
-                }
-            }
-            __syncwarp();
-            // ---- phase 3: one edge per lane ----
-            if (have) {
-                const float *orow = sout + lane * RS;
-                float radial = 0.f;
-                float4 *kp = reinterpret_cast<float4 *>(kappa + (e - ch.e_lo) * (int64_t)NPHIP);
-#pragma unroll
-                for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
-                    const float4 s4 = reinterpret_cast<const float4 *>(orow)[n4];
-                    radial = fmaf(yn[n4 * 4], s4.x, radial); radial = fmaf(yn[n4 * 4 + 1], s4.y, radial);
-                    radial = fmaf(yn[n4 * 4 + 2], s4.z, radial); radial = fmaf(yn[n4 * 4 + 3], s4.w, radial);
-                    if (want_kappa)
-                        kp[n4] = make_float4(Rn[n4 * 4] * s4.x, Rn[n4 * 4 + 1] * s4.y, Rn[n4 * 4 + 2] * s4.z, Rn[n4 * 4 + 3] * s4.w);
-                }
-                float A[NA], P[NAP];
-                monomials<NA>(g.x, g.y, g.z, A);
-#pragma unroll
-                for (int a4 = 0; a4 < NAP / 4; ++a4) {
-                    const float4 p4 = reinterpret_cast<const float4 *>(orow + NPHIP)[a4];
-                    P[4 * a4] = p4.x; P[4 * a4 + 1] = p4.y; P[4 * a4 + 2] = p4.z; P[4 * a4 + 3] = p4.w;
-                }
-                float gx, gy, gz;
-                monomial_vjp<NA>(A, P, gx, gy, gz);
-                const float rr = __fdividef(radial, g.w);
-                gx = fmaf(rr, g.x, gx); gy = fmaf(rr, g.y, gy); gz = fmaf(rr, g.z, gz);
-                gst[e] = make_float4(gx, gy, gz, 0.f);
-                aF[0] += gx; aF[1] += gy; aF[2] += gz;
-                if constexpr (VIR) {
-                    aV[0] -= g.x * gx; aV[1] -= g.x * gy; aV[2] -= g.x * gz;
-                    aV[3] -= g.y * gx; aV[4] -= g.y * gy; aV[5] -= g.y * gz;
-                    aV[6] -= g.z * gx; aV[7] -= g.z * gy; aV[8] -= g.z * gz;
-                }
-            }
-            __syncwarp();
-        }
-    }
-    // fixed-order reductions: lanes (butterfly, FP32), then FP64 accumulation across layers / warps
-#pragma unroll
-    for (int d = 16; d >= 1; d >>= 1) {
-#pragma unroll
-        for (int k = 0; k < 3; ++k) aF[k] += __shfl_xor_sync(0xffffffffu, aF[k], d);
-        if constexpr (VIR) {
+        for (int d = 16; d >= 1; d >>= 1)
 #pragma unroll
             for (int k = 0; k < 9; ++k) aV[k] += __shfl_xor_sync(0xffffffffu, aV[k], d);
-        }
     }
-    if (lane == 0 && i < N) { Fc[3 * i] += (double)aF[0]; Fc[3 * i + 1] += (double)aF[1]; Fc[3 * i + 2] += (double)aF[2]; }
     if constexpr (VIR) {
         if (lane == 0) {
 #pragma unroll
@@ -900,7 +603,8 @@ __global__ void __launch_bounds__(EW * 32, 3) k_edge_bwd_mma(int64_t N, const in
 
 // ------------------------------------------------------------------------------------------ A11
 // Reverse gather (the paper's backward GA -> LA gradient message as a vJp of N_phi numbers per
-// edge): cbar_k[n] = sum_e kappa[rev(e)][n];  F_k -= sum_e g[rev(e)].
+// edge): cbar_k[n] = sum_{e in row(k)} kappa[rev(e)][n];  F_k += sum_{e in row(k)} (g_e - g_rev(e))
+// (Eq. 3).
 template <int NPHIP>
 __global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                         const uint32_t *__restrict__ rev_rc,
@@ -917,8 +621,8 @@ __global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t
     if (ch.do_forces) {
         double f0 = 0.0, f1 = 0.0, f2 = 0.0;
         for (int64_t e = beg + lane; e < end; e += 32) {
-            const float4 g = gst[rev_rc[e]];
-            f0 -= (double)g.x; f1 -= (double)g.y; f2 -= (double)g.z;
+            const float4 g = gst[rev_rc[e]], o = gst[e];
+            f0 += (double)(o.x - g.x); f1 += (double)(o.y - g.y); f2 += (double)(o.z - g.z);
         }
 #pragma unroll
         for (int d = 16; d >= 1; d >>= 1) {
@@ -1035,13 +739,6 @@ void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, i
     if (work > 0) LAUNCH(ctx, k_ghost_gather, div_up(work, 256), 256, 0, c_ext, xrec, N, n_ext, nphip);
 }
 
-// REANN_EDGE_FWD=simt keeps the FP32 ALU forward kernel where the mma.sync one applies (N_phi = 16, L >= 2)
-static bool edge_fwd_mma_enabled() {
-    static int v = -1;
-    if (v < 0) { const char *e = getenv("REANN_EDGE_FWD"); v = (e && strcmp(e, "simt") == 0) ? 0 : 1; }
-    return v == 1;
-}
-
 template <int NA>
 static int run_edge_fwd_mma(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
                             const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
@@ -1054,11 +751,14 @@ template <int NPHIP, int NA, int PN, int PA>
 static int run_edge_fwd(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
                         const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
     using C = FwdCfg<NPHIP, NA, PN, PA>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) return REANN_ERR_UNSUPPORTED;
+    if (!attr_set[dev]) {   // the attribute is per device
         if (cudaFuncSetAttribute(k_edge_fwd<NPHIP, NA, PN, PA>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) != cudaSuccess)
             return REANN_ERR_CUDA;
-        attr_set = true;
+        attr_set[dev] = true;
     }
     LAUNCH(ctx, (k_edge_fwd<NPHIP, NA, PN, PA>), div_up(N, (int64_t)EW * C::APW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
     return REANN_OK;
@@ -1075,10 +775,10 @@ static int run_edge_fwd(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, 
 
 int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
-                    const float *alpha, float *b) {
+                    const float *alpha, float *b, bool allow_mma) {
     if (N <= 0) return REANN_OK;
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
-    if (md.nphip == 16 && md.Na >= 10 && edge_fwd_mma_enabled())
+    if (md.nphip == 16 && md.Na >= 10 && allow_mma)
         return md.Na == 20 ? run_edge_fwd_mma<20>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b)
                            : run_edge_fwd_mma<10>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
 #define M(NP, NA_, PN_, PA_) return run_edge_fwd<NP, NA_, PN_, PA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
@@ -1086,42 +786,11 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 #undef M
 }
 
-// REANN_EDGE=mma selects the mma.sync version of the edge backward kernel (needs N_phi % 8 == 0, L >= 2). It is
-// parity-green but, one atom per warp and 12 warps per SM, still latency-bound: 1.14 ms against 1.09 ms of the
-// FP32 ALU kernel on config 3, which therefore stays the default.
-static bool edge_mma_enabled() {
-    static int v = -1;
-    if (v < 0) { const char *e = getenv("REANN_EDGE"); v = (e && strcmp(e, "mma") == 0) ? 1 : 0; }
-    return v == 1;
-}
-
-template <int NPHIP, int NA>
-static int run_edge_bwd_mma(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
-                            const float4 *geom, const float *c_ext, RadialTab rt, int S, const float *bbar,
-                            int want_kappa, float *kappa, float4 *gst, double *Fc, double *vir_part, AtomChunk ch) {
-    using C = BwdMma<NPHIP, NA>;
-    const unsigned nblk = div_up(ch.a1 - ch.a0, EW);
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_edge_bwd_mma<NPHIP, NA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) != cudaSuccess ||
-            cudaFuncSetAttribute(k_edge_bwd_mma<NPHIP, NA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) != cudaSuccess)
-            return REANN_ERR_CUDA;
-        attr_set = true;
-    }
-    if (vir_part)
-        LAUNCH(ctx, (k_edge_bwd_mma<NPHIP, NA, true>), nblk, EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, S,
-               bbar, want_kappa, kappa, gst, Fc, vir_part, ch);
-    else
-        LAUNCH(ctx, (k_edge_bwd_mma<NPHIP, NA, false>), nblk, EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, S,
-               bbar, want_kappa, kappa, gst, Fc, vir_part, ch);
-    return REANN_OK;
-}
-
 int edge_bwd_blocks(int64_t N) { return (int)div_up(N, EW); }
 
 int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
-                    const float *alpha, const float *bbar, float *kappa, float4 *gst, double *Fc, double *vir_part,
+                    const float *alpha, const float *bbar, float *kappa, float4 *gst, double *vir_part,
                     int64_t a0, int64_t a1, int64_t e_lo) {
     if (N <= 0 || a1 <= a0) return REANN_OK;
     const AtomChunk ch{a0, a1, e_lo};
@@ -1129,16 +798,12 @@ int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
     const int want_kappa = t >= 1;
 #define M(NP, NA_, PN_, PA_)                                                                                      \
-    if constexpr (NP % 8 == 0 && NA_ >= 10) {                                                                     \
-        if (edge_mma_enabled()) return run_edge_bwd_mma<NP, NA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, md.S, bbar, \
-                                                                 want_kappa, kappa, gst, Fc, vir_part, ch);       \
-    }                                                                                                             \
     if (vir_part)                                                                                                 \
         LAUNCH(ctx, (k_edge_bwd<NP, NA_, true>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,            \
-               md.S, bbar, want_kappa, kappa, gst, Fc, vir_part, ch);                                             \
+               md.S, bbar, want_kappa, kappa, gst, vir_part, ch);                                                 \
     else                                                                                                          \
         LAUNCH(ctx, (k_edge_bwd<NP, NA_, false>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,           \
-               md.S, bbar, want_kappa, kappa, gst, Fc, vir_part, ch);                                             \
+               md.S, bbar, want_kappa, kappa, gst, vir_part, ch);                                                 \
     return REANN_OK;
     EDGE_DISPATCH(M)
 #undef M
