@@ -182,7 +182,6 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         auto is = [](const char *name, const char *val) { const char *e = getenv(name); return e && strcmp(e, val) == 0; };
         h->dense_tc = !is("REANN_DENSE", "simt");
         h->edge_fwd_mma = !is("REANN_EDGE_FWD", "simt");
-        h->edge_bwd_tc = !is("REANN_EDGE", "simt") && edge_bwd_tc_supported(md);
         if (const char *e = getenv("REANN_STASH_CHUNKS")) h->stash_chunks_forced = std::max(0, atoi(e));
     }
     md.rc = rc; md.skin = skin;
@@ -428,7 +427,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
-        h->n_vir_blocks = std::max(edge_bwd_blocks(std::max<int64_t>(N, 1)), edge_bwd_tc_blocks(std::max<int64_t>(N, 1)));
+        h->n_vir_blocks = edge_bwd_blocks(std::max<int64_t>(N, 1));
         RC(dev_ensure(h, h->vir_part, sizeof(double) * 9 * (size_t)h->n_vir_blocks));
         RC(dev_ensure(h, h->red_scratch, sizeof(double) * ((size_t)N / 256 + 2)));
         RC(dev_ensure(h, h->out_stage, sizeof(double) * (16 + 3 * (size_t)N)));
@@ -609,11 +608,11 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         mk.mark(6);
         for (int c = 0; c < C; ++c) {
             if (c > 0) mk.mark(6);
-            rcode = (h->edge_bwd_tc ? launch_edge_bwd_tc : launch_edge_bwd)(
-                ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p, (const float4 *)h->geom.p,
-                c_ext + t * cstride, (const float *)h->rcen.p, (const float *)h->alpha.p, (const float *)h->bbar.p,
-                (float *)h->kappa.p, (float4 *)h->gst.p, virial ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
-                ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
+            rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
+                                    (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
+                                    (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
+                                    (float4 *)h->gst.p, virial ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
+                                    ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
             if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
             mk.mark(t >= 1 ? 7 : 9);
             // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after

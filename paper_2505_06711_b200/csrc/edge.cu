@@ -438,8 +438,7 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
 // Warp per atom, one edge per lane; bbar_i is broadcast from shared memory, S_n and P_a stay in the
 // lane's registers, so there is no cross-lane reduction per edge. Orbitals are recomputed (nothing
 // per-edge is kept from the forward pass). Writes the per-edge stash g_e (float4) and kappa_e; the forces are
-// gathered from the g_e stash by k_rev_gather. This FP32 ALU kernel serves the shapes the tcgen05 kernel of
-// edge_tc.cu does not (N_phi = 4, L = 0) and is its accuracy yardstick (REANN_EDGE=simt).
+// gathered from the g_e stash by k_rev_gather.
 // The radial tables sit in shared memory; c_j and the next pass's edge record are prefetched one
 // step ahead so that no global-load latency is exposed inside the FMA loop. VIR: accumulate the
 // virial (only when the caller asked for it).

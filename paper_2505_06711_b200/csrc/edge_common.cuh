@@ -1,5 +1,5 @@
-// edge_common.cuh -- device helpers shared by the edge kernels (edge.cu: FP32 ALU / mma.sync kernels; edge_tc.cu:
-// tcgen05 edge backward): Cartesian monomials and their vector-Jacobian product, packed FP32 pairs, launch structs.
+// edge_common.cuh -- device helpers of the edge kernels (edge.cu): Cartesian monomials and their vector-Jacobian
+// product, packed FP32 pairs, launch structs.
 #pragma once
 #include "common.cuh"
 

@@ -17,7 +17,6 @@ struct reann {
     // kernel selection, read from the environment once at reann_create
     bool dense_tc = true;         // REANN_DENSE=simt selects the FP32 SIMT GEMM chain instead
     bool edge_fwd_mma = true;     // REANN_EDGE_FWD=simt: FP32 ALU edge forward where the mma.sync kernel applies
-    bool edge_bwd_tc = true;      // REANN_EDGE=simt: FP32 ALU edge backward where the tcgen05 kernel applies
     int stash_chunks_forced = 0;  // REANN_STASH_CHUNKS=n
     DevBuf rcen, alpha, c0;       // [T][S][nphip] (alpha pre-multiplied by log2(e)), [S][nphip]
     std::vector<DenseW> h_wtab;   // host copy of the table (device pointers inside)

@@ -380,12 +380,11 @@ def test_full_size_config5_sampled(R):
     m.close()
 
 
-@pytest.mark.parametrize("env", [{"REANN_EDGE": "simt", "REANN_EDGE_FWD": "simt"}, {"REANN_DENSE": "simt"}],
-                         ids=["edge_bwd_simt+edge_fwd_simt", "dense_simt"])
+@pytest.mark.parametrize("env", [{"REANN_EDGE_FWD": "simt"}, {"REANN_DENSE": "simt"}], ids=["edge_fwd_simt", "dense_simt"])
 def test_non_default_kernel_variants_parity(env):
-    """The kernels behind the library's environment switches: REANN_EDGE=simt (FP32 ALU edge
-    backward instead of the tcgen05 one) with REANN_EDGE_FWD=simt (FP32 ALU edge forward), and REANN_DENSE=simt
-    (FP32 ALU GEMM chain). Same parity gates as the default kernels."""
+    """The kernels behind the library's environment switches: REANN_EDGE_FWD=simt (FP32 ALU edge
+    forward instead of the mma.sync one) and REANN_DENSE=simt (FP32 ALU GEMM chain). Same parity gates as the
+    default kernels."""
     import os, subprocess, sys
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     code = (
