@@ -61,7 +61,7 @@ constexpr uint32_t TMEM_COLS = 512;    // allocation (power of two >= NBUF * COL
 
 // barrier slots (8 bytes each) in the barrier area
 enum { BAR_BFULL = 0, BAR_MMA = 3, BAR_AFULL = 6, BAR_AH = 9, BAR_QFULL = 13, BAR_QEMPTY = 15, BAR_DFULL = 17,
-       BAR_DEMPTY = 20, BAR_ARES = 23, BAR_COUNT = 24 };
+       BAR_DEMPTY = 20, BAR_ARES = 23, BAR_TDONE = 24, BAR_COUNT = 25 };
 
 // Optional timeline trace of one CTA (development aid, compiled only with -DREANN_TC_TRACE):
 // role 0 = control thread, 1 = compute thread 0; slot k = clock64().
@@ -69,7 +69,7 @@ enum { BAR_BFULL = 0, BAR_MMA = 3, BAR_AFULL = 6, BAR_AH = 9, BAR_QFULL = 13, BA
 __device__ long long g_tc_trace[2 * 2 * 128];
 #define TC_TRACE(kern, role, k)                                                                      \
     do {                                                                                             \
-        if (blockIdx.x == 200 && (k) < 128) g_tc_trace[((kern) * 2 + (role)) * 128 + (k)] = clock64(); \
+        if (blockIdx.x == 5 && (k) < 128) g_tc_trace[((kern) * 2 + (role)) * 128 + (k)] = clock64(); \
     } while (0)
 #else
 #define TC_TRACE(kern, role, k) ((void)0)
@@ -110,6 +110,7 @@ __device__ __forceinline__ uint32_t tc_prologue(unsigned char *smem, uint32_t *t
             mbar_init(bar0 + 8 * (BAR_DEMPTY + d), NCOMPUTE);
         }
         mbar_init(bar0 + 8 * BAR_ARES, NCOMPUTE);
+        mbar_init(bar0 + 8 * BAR_TDONE, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == CTL_WARP) {
@@ -130,45 +131,60 @@ __device__ __forceinline__ void tc_epilogue(uint32_t tmem) {
 }
 
 // ---- control-thread helpers ----
+// The kernels are persistent (a CTA walks over tiles): `sb` / `gb` are the steps / accumulator groups issued for
+// earlier tiles, so that ring slots and mbarrier parities run on over tile boundaries; i and g are tile-local.
 struct Ctl {
     uint32_t bar0, a0, b0, tmem;
+    int sb, gb;
     __device__ __forceinline__ uint32_t bar(int k) const { return bar0 + 8u * (uint32_t)k; }
     // stream the weight chunk of step i into its B slot (after the MMAs of step i-3 released it)
-    __device__ __forceinline__ void copy_b(int i, const float *src, int n_rows) const {
+    __device__ __forceinline__ void copy_b(int i_loc, const float *src, int n_rows) const {
+        const int i = sb + i_loc;
         const int s = i % NSTAGE;
         if (i >= NSTAGE) mbar_wait(bar(BAR_MMA + s), (uint32_t)(((i / NSTAGE) - 1) & 1));
         const uint32_t bytes = (uint32_t)n_rows * KC * 4 * 2;
-        mbar_expect_tx(bar(BAR_BFULL + s), bytes);
-        bulk_g2s(b0 + (uint32_t)s * B_SLOT, src, bytes, bar(BAR_BFULL + s));
+        if (elect_one()) {
+            mbar_expect_tx(bar(BAR_BFULL + s), bytes);
+            bulk_g2s(b0 + (uint32_t)s * B_SLOT, src, bytes, bar(BAR_BFULL + s));
+        }
+        __syncwarp();
     }
     // One K chunk = one accumulation group (step i, group buffer i % NBUF):
     //   D[:, 0:n) = A_lo B_hi^T + A_hi B_lo^T  (4 x K = 8),  then  D += A_hi B_hi^T  (4 x K = 8)
-    __device__ __forceinline__ void mma_chunk(int i, int a_slot, int n_rows, int g) const {
+    __device__ __forceinline__ void mma_chunk(int i_loc, int a_slot, int n_rows, int g_loc) const {
+        const int i = sb + i_loc, g = gb + g_loc;
         const int s = i % NSTAGE, d = g % NBUF;
         if (g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        issue(i, a_slot, n_rows, dm, true, false, true);
-        issue(i, a_slot, n_rows, dm, false, true, false);
-        tc_commit(bar(BAR_MMA + s));
-        tc_commit(bar(BAR_DFULL + d));
+        if (elect_one()) {
+            issue(i, a_slot, n_rows, dm, true, false, true);
+            issue(i, a_slot, n_rows, dm, false, true, false);
+            tc_commit(bar(BAR_MMA + s));
+            tc_commit(bar(BAR_DFULL + d));
+        }
+        __syncwarp();
     }
     // Two K chunks (steps i, i+1) = one accumulation group of K = 64: all corrections first, then hi.hi of both
-    __device__ __forceinline__ void mma_pair(int i, int a_slot0, int a_slot1, int n_rows, int g) const {
+    __device__ __forceinline__ void mma_pair(int i_loc, int a_slot0, int a_slot1, int n_rows, int g_loc) const {
+        const int i = sb + i_loc, g = gb + g_loc;
         const int d = g % NBUF;
         if (g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
         mbar_wait(bar(BAR_BFULL + i % NSTAGE), (uint32_t)((i / NSTAGE) & 1));
         mbar_wait(bar(BAR_BFULL + (i + 1) % NSTAGE), (uint32_t)(((i + 1) / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        issue(i, a_slot0, n_rows, dm, true, false, true);
-        issue(i + 1, a_slot1, n_rows, dm, true, false, false);
-        issue(i, a_slot0, n_rows, dm, false, true, false);
-        tc_commit(bar(BAR_MMA + i % NSTAGE));
-        issue(i + 1, a_slot1, n_rows, dm, false, true, false);
-        tc_commit(bar(BAR_MMA + (i + 1) % NSTAGE));
-        tc_commit(bar(BAR_DFULL + d));
+        if (elect_one()) {
+            issue(i, a_slot0, n_rows, dm, true, false, true);
+            issue(i + 1, a_slot1, n_rows, dm, true, false, false);
+            issue(i, a_slot0, n_rows, dm, false, true, false);
+            tc_commit(bar(BAR_MMA + i % NSTAGE));
+            issue(i + 1, a_slot1, n_rows, dm, false, true, false);
+            tc_commit(bar(BAR_MMA + (i + 1) % NSTAGE));
+            tc_commit(bar(BAR_DFULL + d));
+        }
+        __syncwarp();
     }
     // the MMAs of one chunk: corrections (A_lo B_hi + A_hi B_lo) and / or main (A_hi B_hi); fresh: overwrite D first
     __device__ __forceinline__ void issue(int i, int a_slot, int n_rows, uint32_t dm, bool corr, bool main, bool fresh) const {
@@ -243,7 +259,7 @@ struct TcFwdArgs {
     const float *Q;         // tile-quad layout, K1 columns
     float *z_stash;         // tile-quad layout, zs columns (z1 | z2)
     float *out;             // rows of stride out_stride, atom order
-    int out_stride, K1, nout, zs;
+    int out_stride, K1, nout, zs, n_tiles;
 };
 
 template <int NCH1, int NCH2>
@@ -252,156 +268,176 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
     __shared__ uint32_t tmem_base_s;
     constexpr int H1p = NCH1 * 32, H2p = NCH2 * 32, CW1 = H1p / 2, CW2 = H2p / 2;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const DenseTile tile = A.tiles[blockIdx.x];
-    const DenseWT W = A.w[tile.species];
+    const int warp_u = __shfl_sync(0xffffffffu, warp, 0);           // warp-uniform for the compiler
     const uint32_t bar0 = smem_u32(smem + SM_BAR);
     const uint32_t tmem = tc_prologue(smem, &tmem_base_s, CW1 >= 32 ? 128u : 256u);
     const int n1 = A.K1 / KC, total = n1 + NCH1;
-    const float *Qt = A.Q + (size_t)blockIdx.x * A.K1 * TM;
+    // running counters over the tiles of this CTA: steps (B ring, MMA barriers), groups (TMEM buffers), Q chunks (A ring)
+    int sb = 0, gb = 0, qb = 0, it = 0;
 
-    if (warp == CTL_WARP) {
-        if (lane == 0) {
-            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem};
+    if (warp_u == CTL_WARP) {
+        {   // the whole warp walks the control flow (warp-uniform: descriptors in uniform registers); one lane acts
+            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0};
             const uint32_t stg = c.a0 + 3u * A_SLOT;
-            auto issue_q = [&](int j) {   // raw Q chunk j -> staging buffer j & 1
-                const int qs = j & 1;
-                if (j >= 2) mbar_wait(c.bar(BAR_QEMPTY + qs), (uint32_t)(((j >> 1) - 1) & 1));
-                mbar_expect_tx(c.bar(BAR_QFULL + qs), A_HALF);
-                bulk_g2s(stg + (uint32_t)qs * A_HALF, Qt + (size_t)j * (KC * TM), A_HALF, c.bar(BAR_QFULL + qs));
-            };
-            auto copy_b = [&](int i) {
-                if (i < n1) c.copy_b(i, W.g1 + (size_t)i * (2 * H1p * KC), H1p);
-                else c.copy_b(i, W.g2 + (size_t)(i - n1) * (2 * H2p * KC), H2p);
-            };
-            issue_q(0);
-            if (n1 > 1) issue_q(1);
-            copy_b(0);
-            if (total > 1) copy_b(1);
-            for (int i = 0; i < total; ++i) {
-                const int s = i % NSTAGE;
-                if (i < n1) {
-                    mbar_wait(c.bar(BAR_AFULL + s), (uint32_t)((i / NSTAGE) & 1));
-                    if (i + 2 < n1) issue_q(i + 2);
-                    TC_TRACE(0, 0, 2 * i);
-                    c.mma_chunk(i, s, H1p, i);
-                } else {
-                    mbar_wait(c.bar(BAR_AH + (i - n1)), 0);
-                    TC_TRACE(0, 0, 2 * i);
-                    c.mma_chunk(i, i - n1, H2p, i);
+            for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+                const DenseTile tile = A.tiles[tile_idx];
+                const DenseWT W = A.w[tile.species];
+                const float *Qt = A.Q + (size_t)tile_idx * A.K1 * TM;
+                c.sb = sb; c.gb = gb;
+                auto issue_q = [&](int j_loc) {   // raw Q chunk -> staging buffer (J & 1)
+                    const int j = qb + j_loc, qs = j & 1;
+                    if (j >= 2) mbar_wait(c.bar(BAR_QEMPTY + qs), (uint32_t)(((j >> 1) - 1) & 1));
+                    if (elect_one()) {
+                        mbar_expect_tx(c.bar(BAR_QFULL + qs), A_HALF);
+                        bulk_g2s(stg + (uint32_t)qs * A_HALF, Qt + (size_t)j_loc * (KC * TM), A_HALF, c.bar(BAR_QFULL + qs));
+                    }
+                    __syncwarp();
+                };
+                auto copy_b = [&](int i) {
+                    if (i < n1) c.copy_b(i, W.g1 + (size_t)i * (2 * H1p * KC), H1p);
+                    else c.copy_b(i, W.g2 + (size_t)(i - n1) * (2 * H2p * KC), H2p);
+                };
+                copy_b(0);
+                if (total > 1) copy_b(1);
+                // the staging area doubles as the fourth operand slot of GEMM 2: wait for the previous tile to be done
+                if (it > 0) mbar_wait(c.bar(BAR_TDONE), (uint32_t)((it - 1) & 1));
+                issue_q(0);
+                if (n1 > 1) issue_q(1);
+                for (int i = 0; i < total; ++i) {
+                    if (i < n1) {
+                        const int j = qb + i, sa = j % NSTAGE;
+                        mbar_wait(c.bar(BAR_AFULL + sa), (uint32_t)((j / NSTAGE) & 1));
+                        if (i + 2 < n1) issue_q(i + 2);
+                        TC_TRACE(0, 0, 2 * i);
+                        c.mma_chunk(i, sa, H1p, i);
+                    } else {
+                        mbar_wait(c.bar(BAR_AH + (i - n1)), (uint32_t)(it & 1));
+                        TC_TRACE(0, 0, 2 * i);
+                        c.mma_chunk(i, i - n1, H2p, i);
+                    }
+                    TC_TRACE(0, 0, 2 * i + 1);
+                    if (i + 2 < total) copy_b(i + 2);
                 }
-                TC_TRACE(0, 0, 2 * i + 1);
-                if (i + 2 < total) copy_b(i + 2);
+                sb += total; gb += total; qb += n1;
             }
         }
     } else {
         const int m = (warp & 3) * 32 + lane, hf = warp >> 2;
-        const bool valid = m < tile.count;
         const uint32_t tl = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         unsigned char *a_base = smem + SM_A;
-        float *zt = A.z_stash + (size_t)blockIdx.x * A.zs * TM + m * 4;   // + (col/4) * 512
-        if (tid == 0) TC_TRACE(0, 1, 100);
-        // ---- GEMM 1: z1 = Q U.  Convert raw Q chunk i (staging -> hi/lo A slot), drain group i-1 ----
-        float acc1[CW1];
+        for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+            const DenseTile tile = A.tiles[tile_idx];
+            const DenseWT W = A.w[tile.species];
+            const bool valid = m < tile.count;
+            float *zt = A.z_stash + (size_t)tile_idx * A.zs * TM + m * 4;   // + (col/4) * 512
+            if (tid == 0) TC_TRACE(0, 1, 100);
+            // ---- GEMM 1: z1 = Q U.  Convert raw Q chunk i (staging -> hi/lo A slot), drain group i-1 ----
+            float acc1[CW1];
 #pragma unroll
-        for (int c = 0; c < CW1; ++c) acc1[c] = 0.f;
-        const int crow = warp * 16 + (lane & 7), ckq = lane >> 3;
+            for (int c = 0; c < CW1; ++c) acc1[c] = 0.f;
+            const int crow = warp * 16 + (lane & 7), ckq = lane >> 3;
 #pragma unroll 1
-        for (int i = 0; i < n1; ++i) {
-            const int s = i % NSTAGE, qs = i & 1;
-            mbar_wait(bar0 + 8 * (BAR_QFULL + qs), (uint32_t)((i >> 1) & 1));
-            wait_stage_free(bar0, i);
-            const unsigned char *stg = smem + SM_A + 3 * A_SLOT + qs * A_HALF;
-            float4 v[4];
+            for (int i = 0; i < n1; ++i) {
+                const int j = qb + i, sa = j % NSTAGE, qs = j & 1;
+                mbar_wait(bar0 + 8 * (BAR_QFULL + qs), (uint32_t)((j >> 1) & 1));
+                wait_stage_free(bar0, sb + i);       // MMAs of step - 3 (they read A slot sa when they belong to this tile)
+                const unsigned char *stg = smem + SM_A + 3 * A_SLOT + qs * A_HALF;
+                float4 v[4];
 #pragma unroll
-            for (int rb = 0; rb < 2; ++rb)
+                for (int rb = 0; rb < 2; ++rb)
 #pragma unroll
-                for (int j = 0; j < 2; ++j)
-                    v[rb * 2 + j] = *reinterpret_cast<const float4 *>(stg + (ckq + 4 * j) * (int)A_LBO + (crow + rb * 8) * 16);
+                    for (int jj = 0; jj < 2; ++jj)
+                        v[rb * 2 + jj] = *reinterpret_cast<const float4 *>(stg + (ckq + 4 * jj) * (int)A_LBO + (crow + rb * 8) * 16);
 #pragma unroll
-            for (int rb = 0; rb < 2; ++rb)
+                for (int rb = 0; rb < 2; ++rb)
 #pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const float x[4] = {v[rb * 2 + j].x, v[rb * 2 + j].y, v[rb * 2 + j].z, v[rb * 2 + j].w};
-                    store_split4(a_base + s * A_SLOT, ckq + 4 * j, crow + rb * 8, x);
-                }
-            fence_async_smem();
-            mbar_arrive(bar0 + 8 * (BAR_AFULL + s));
-            mbar_arrive(bar0 + 8 * (BAR_QEMPTY + qs));
-            if (tid == 0) TC_TRACE(0, 1, 2 * i);
-            if (i >= 1) drain_group<CW1>(acc1, bar0, tl, i - 1, hf * CW1, true);
-            if (tid == 0) TC_TRACE(0, 1, 2 * i + 1);
-        }
-        drain_group<CW1>(acc1, bar0, tl, n1 - 1, hf * CW1, true);
-        if (tid == 0) TC_TRACE(0, 1, 101);
-        // ---- z1 = acc + b1 (stash), h1 = SiLU(z1) -> A operand of GEMM 2 ----
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const float x[4] = {v[rb * 2 + jj].x, v[rb * 2 + jj].y, v[rb * 2 + jj].z, v[rb * 2 + jj].w};
+                        store_split4(a_base + sa * A_SLOT, ckq + 4 * jj, crow + rb * 8, x);
+                    }
+                fence_async_smem();
+                mbar_arrive(bar0 + 8 * (BAR_AFULL + sa));
+                mbar_arrive(bar0 + 8 * (BAR_QEMPTY + qs));
+                if (tid == 0) TC_TRACE(0, 1, 2 * i);
+                if (i >= 1) drain_group<CW1>(acc1, bar0, tl, gb + i - 1, hf * CW1, true);
+                if (tid == 0) TC_TRACE(0, 1, 2 * i + 1);
+            }
+            drain_group<CW1>(acc1, bar0, tl, gb + n1 - 1, hf * CW1, true);
+            if (tid == 0) TC_TRACE(0, 1, 101);
+            // ---- z1 = acc + b1 (stash), h1 = SiLU(z1) -> A operand of GEMM 2 ----
 #pragma unroll
-        for (int k4 = 0; k4 < CW1 / 4; ++k4) {
-            const int col = hf * CW1 + k4 * 4;
-            const float4 b4 = __ldg(reinterpret_cast<const float4 *>(W.b1 + col));
-            const float4 z = make_float4(acc1[k4 * 4] + b4.x, acc1[k4 * 4 + 1] + b4.y, acc1[k4 * 4 + 2] + b4.z,
-                                         acc1[k4 * 4 + 3] + b4.w);
-            if (valid) *reinterpret_cast<float4 *>(zt + (size_t)(col >> 2) * (TM * 4)) = z;
-            acc1[k4 * 4] = silu_f(z.x); acc1[k4 * 4 + 1] = silu_f(z.y);
-            acc1[k4 * 4 + 2] = silu_f(z.z); acc1[k4 * 4 + 3] = silu_f(z.w);
-        }
-        store_operand<CW1>(acc1, a_base, bar0, hf * CW1, m);
-        if (tid == 0) TC_TRACE(0, 1, 102);
-        // ---- GEMM 2: z2 = h1 W2 ----
-        float acc2[CW2];
+            for (int k4 = 0; k4 < CW1 / 4; ++k4) {
+                const int col = hf * CW1 + k4 * 4;
+                const float4 b4 = __ldg(reinterpret_cast<const float4 *>(W.b1 + col));
+                const float4 z = make_float4(acc1[k4 * 4] + b4.x, acc1[k4 * 4 + 1] + b4.y, acc1[k4 * 4 + 2] + b4.z,
+                                             acc1[k4 * 4 + 3] + b4.w);
+                if (valid) *reinterpret_cast<float4 *>(zt + (size_t)(col >> 2) * (TM * 4)) = z;
+                acc1[k4 * 4] = silu_f(z.x); acc1[k4 * 4 + 1] = silu_f(z.y);
+                acc1[k4 * 4 + 2] = silu_f(z.z); acc1[k4 * 4 + 3] = silu_f(z.w);
+            }
+            store_operand<CW1>(acc1, a_base, bar0, hf * CW1, m);
+            if (tid == 0) TC_TRACE(0, 1, 102);
+            // ---- GEMM 2: z2 = h1 W2 ----
+            float acc2[CW2];
 #pragma unroll
-        for (int c = 0; c < CW2; ++c) acc2[c] = 0.f;
+            for (int c = 0; c < CW2; ++c) acc2[c] = 0.f;
 #pragma unroll 1
-        for (int kc = 0; kc < NCH1; ++kc) drain_group<CW2>(acc2, bar0, tl, n1 + kc, hf * CW2, true);
-        if (tid == 0) TC_TRACE(0, 1, 103);
-        // ---- z2 (stash), h2 = SiLU(z2), out = h2 W3 + b3 in FP32 (partial over this column half) ----
-        float o[16];
+            for (int kc = 0; kc < NCH1; ++kc) drain_group<CW2>(acc2, bar0, tl, gb + n1 + kc, hf * CW2, true);
+            if (tid == 0) TC_TRACE(0, 1, 103);
+            // ---- z2 (stash), h2 = SiLU(z2), out = h2 W3 + b3 in FP32 (partial over this column half) ----
+            float o[16];
 #pragma unroll
-        for (int c = 0; c < 16; ++c) o[c] = 0.f;
+            for (int c = 0; c < 16; ++c) o[c] = 0.f;
 #pragma unroll
-        for (int k4 = 0; k4 < CW2 / 4; ++k4) {
-            const int col = hf * CW2 + k4 * 4;
-            const float4 b4 = __ldg(reinterpret_cast<const float4 *>(W.b2 + col));
-            const float4 z = make_float4(acc2[k4 * 4] + b4.x, acc2[k4 * 4 + 1] + b4.y, acc2[k4 * 4 + 2] + b4.z,
-                                         acc2[k4 * 4 + 3] + b4.w);
-            if (valid) *reinterpret_cast<float4 *>(zt + (size_t)((H1p + col) >> 2) * (TM * 4)) = z;
-            const float hv[4] = {silu_f(z.x), silu_f(z.y), silu_f(z.z), silu_f(z.w)};
-            if (A.nout == 1) {
-                const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + col));
-                o[0] = fmaf(hv[0], w4.x, o[0]); o[0] = fmaf(hv[1], w4.y, o[0]);
-                o[0] = fmaf(hv[2], w4.z, o[0]); o[0] = fmaf(hv[3], w4.w, o[0]);
-            } else {
+            for (int k4 = 0; k4 < CW2 / 4; ++k4) {
+                const int col = hf * CW2 + k4 * 4;
+                const float4 b4 = __ldg(reinterpret_cast<const float4 *>(W.b2 + col));
+                const float4 z = make_float4(acc2[k4 * 4] + b4.x, acc2[k4 * 4 + 1] + b4.y, acc2[k4 * 4 + 2] + b4.z,
+                                             acc2[k4 * 4 + 3] + b4.w);
+                if (valid) *reinterpret_cast<float4 *>(zt + (size_t)((H1p + col) >> 2) * (TM * 4)) = z;
+                const float hv[4] = {silu_f(z.x), silu_f(z.y), silu_f(z.z), silu_f(z.w)};
+                if (A.nout == 1) {
+                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + col));
+                    o[0] = fmaf(hv[0], w4.x, o[0]); o[0] = fmaf(hv[1], w4.y, o[0]);
+                    o[0] = fmaf(hv[2], w4.z, o[0]); o[0] = fmaf(hv[3], w4.w, o[0]);
+                } else {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const float4 *wr = reinterpret_cast<const float4 *>(W.w3p + (size_t)(col + u) * 16);
+                    for (int u = 0; u < 4; ++u) {
+                        const float4 *wr = reinterpret_cast<const float4 *>(W.w3p + (size_t)(col + u) * 16);
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const float4 w4 = __ldg(wr + q);
-                        o[q * 4] = fmaf(hv[u], w4.x, o[q * 4]); o[q * 4 + 1] = fmaf(hv[u], w4.y, o[q * 4 + 1]);
-                        o[q * 4 + 2] = fmaf(hv[u], w4.z, o[q * 4 + 2]); o[q * 4 + 3] = fmaf(hv[u], w4.w, o[q * 4 + 3]);
+                        for (int q = 0; q < 4; ++q) {
+                            const float4 w4 = __ldg(wr + q);
+                            o[q * 4] = fmaf(hv[u], w4.x, o[q * 4]); o[q * 4 + 1] = fmaf(hv[u], w4.y, o[q * 4 + 1]);
+                            o[q * 4 + 2] = fmaf(hv[u], w4.z, o[q * 4 + 2]); o[q * 4 + 3] = fmaf(hv[u], w4.w, o[q * 4 + 3]);
+                        }
                     }
                 }
             }
-        }
-        // combine the two column halves through shared memory (A slot 0 is free: every MMA has completed)
-        float *xch = reinterpret_cast<float *>(smem + SM_A);
-        if (hf == 1) {
+            // combine the two column halves through shared memory (A slot 0 is free: every MMA has completed)
+            float *xch = reinterpret_cast<float *>(smem + SM_A);
+            if (hf == 1) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
-                *reinterpret_cast<float4 *>(xch + (q * TM + m) * 4) = make_float4(o[q * 4], o[q * 4 + 1], o[q * 4 + 2], o[q * 4 + 3]);
-        }
-        compute_sync();
-        if (hf == 0 && valid) {
-            float *dst = A.out + (size_t)A.sp_list[tile.start + m] * A.out_stride;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const float4 p4 = *reinterpret_cast<const float4 *>(xch + (q * TM + m) * 4);
-                const float pv[4] = {p4.x, p4.y, p4.z, p4.w};
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (q * 4 + u < A.nout) dst[q * 4 + u] = (o[q * 4 + u] + pv[u]) + __ldg(W.b3 + q * 4 + u);
+                for (int q = 0; q < 4; ++q)
+                    *reinterpret_cast<float4 *>(xch + (q * TM + m) * 4) = make_float4(o[q * 4], o[q * 4 + 1], o[q * 4 + 2], o[q * 4 + 3]);
             }
+            compute_sync();
+            if (hf == 0 && valid) {
+                float *dst = A.out + (size_t)A.sp_list[tile.start + m] * A.out_stride;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 p4 = *reinterpret_cast<const float4 *>(xch + (q * TM + m) * 4);
+                    const float pv[4] = {p4.x, p4.y, p4.z, p4.w};
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (q * 4 + u < A.nout) dst[q * 4 + u] = (o[q * 4 + u] + pv[u]) + __ldg(W.b3 + q * 4 + u);
+                }
+            }
+            if (tid == 0) TC_TRACE(0, 1, 104);
+            // tile done: the operand slots (and the exchange area) may be reused by the next tile
+            compute_sync();
+            if (tid == 0) mbar_arrive(bar0 + 8 * BAR_TDONE);
+            sb += total; gb += total; qb += n1;
         }
-        if (tid == 0) TC_TRACE(0, 1, 104);
     }
     tc_epilogue(tmem);
 }
@@ -413,7 +449,7 @@ struct TcBwdArgs {
     const int32_t *sp_list;
     const float *z_stash, *outbar; // outbar == nullptr: energy layer (outbar = 1)
     float *Qbar;                   // tile-quad layout, K1 columns
-    int outbar_stride, K1, nout, zs;
+    int outbar_stride, K1, nout, zs, n_tiles;
 };
 
 template <int NCH1, int NCH2>
@@ -422,198 +458,226 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
     __shared__ uint32_t tmem_base_s;
     constexpr int H1p = NCH1 * 32, H2p = NCH2 * 32, CW1 = H1p / 2, CW2 = H2p / 2;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const DenseTile tile = A.tiles[blockIdx.x];
-    const DenseWT W = A.w[tile.species];
+    const int warp_u = __shfl_sync(0xffffffffu, warp, 0);           // warp-uniform for the compiler
     const uint32_t bar0 = smem_u32(smem + SM_BAR);
     const uint32_t tmem = tc_prologue(smem, &tmem_base_s, CW2 >= 32 ? 128u : 256u);
     // steps: [R1 (only when outbar is given: K = n_out padded to 32)] NCH2 x R2, nblk x NCH1 x R3
     constexpr int GR3 = NCH1 >= 2 ? 2 : 1;         // K chunks per accumulator group of R3
     const int o1 = A.outbar ? 1 : 0, i3 = o1 + NCH2;
-    const int nblk = (A.K1 + 127) / 128, total = i3 + nblk * NCH1;
+    const int nblk = (A.K1 + 127) / 128, total = i3 + nblk * NCH1, ngroups = i3 + nblk * (NCH1 / GR3);
+    int sb = 0, gb = 0, it = 0;                     // running steps / groups / tiles of this CTA (persistent kernel)
 
-    if (warp == CTL_WARP) {
-        if (lane == 0) {
-            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem};
-            auto rows_of = [&](int i) { return i < o1 ? H2p : i < i3 ? H1p : min(128, A.K1 - ((i - i3) / NCH1) * 128); };
-            auto copy_b = [&](int i) {
-                if (i < o1) { c.copy_b(i, W.r1, H2p); return; }
-                if (i < i3) { c.copy_b(i, W.r2 + (size_t)(i - o1) * (2 * H1p * KC), H1p); return; }
-                const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1, nr = rows_of(i);
-                c.copy_b(i, W.r3 + (size_t)nb * NCH1 * (2 * 128 * KC) + (size_t)kc * (2 * nr * KC), nr);
-            };
-            copy_b(0);
-            if (total > 1) copy_b(1);
-            for (int i = 0; i < total; ++i) {
-                if (i < o1) {
-                    mbar_wait(c.bar(BAR_AFULL), 0);
-                    TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, 0, H2p, i);
-                } else if (i < i3) {
-                    mbar_wait(c.bar(BAR_AH + (i - o1)), 0);
-                    TC_TRACE(1, 0, 2 * i);
-                    c.mma_chunk(i, i - o1, H1p, i);
-                } else {
-                    // R3: groups of GR3 chunks (K = 32 GR3 per accumulator); group index continues after R2
-                    if (i == i3) mbar_wait(c.bar(BAR_ARES), 0);
-                    const int kc = (i - i3) % NCH1, g = i3 + (i - i3) / GR3;
-                    TC_TRACE(1, 0, 2 * i);
-                    if (GR3 == 2) {
-                        if (i + 2 < total) copy_b(i + 2);          // in flight during this group's MMAs
-                        c.mma_pair(i, kc, kc + 1, rows_of(i), g);
-                        if (i + 3 < total) copy_b(i + 3);          // waits for the hi.hi MMAs of chunk i
-                        TC_TRACE(1, 0, 2 * i + 1);
-                        ++i;
-                        continue;
+    if (warp_u == CTL_WARP) {
+        {   // the whole warp walks the control flow (warp-uniform); one elected lane acts
+            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0};
+            for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+                const DenseTile tile = A.tiles[tile_idx];
+                const DenseWT W = A.w[tile.species];
+                c.sb = sb; c.gb = gb;
+                auto rows_of = [&](int i) { return i < o1 ? H2p : i < i3 ? H1p : min(128, A.K1 - ((i - i3) / NCH1) * 128); };
+                auto copy_b = [&](int i) {
+                    if (i < o1) { c.copy_b(i, W.r1, H2p); return; }
+                    if (i < i3) { c.copy_b(i, W.r2 + (size_t)(i - o1) * (2 * H1p * KC), H1p); return; }
+                    const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1, nr = rows_of(i);
+                    c.copy_b(i, W.r3 + (size_t)nb * NCH1 * (2 * 128 * KC) + (size_t)kc * (2 * nr * KC), nr);
+                };
+                copy_b(0);
+                if (total > 1) copy_b(1);
+                for (int i = 0; i < total; ++i) {
+                    if (i < o1) {
+                        mbar_wait(c.bar(BAR_AFULL), (uint32_t)(it & 1));
+                        TC_TRACE(1, 0, 2 * i);
+                        c.mma_chunk(i, 0, H2p, i);
+                    } else if (i < i3) {
+                        mbar_wait(c.bar(BAR_AH + (i - o1)), (uint32_t)(it & 1));
+                        TC_TRACE(1, 0, 2 * i);
+                        c.mma_chunk(i, i - o1, H1p, i);
                     } else {
-                        c.mma_chunk(i, kc, rows_of(i), g);
+                        // R3: groups of GR3 chunks (K = 32 GR3 per accumulator); group index continues after R2
+                        if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
+                        const int kc = (i - i3) % NCH1, g = i3 + (i - i3) / GR3;
+                        TC_TRACE(1, 0, 2 * i);
+                        if (GR3 == 2) {
+                            if (i + 2 < total) copy_b(i + 2);          // in flight during this group's MMAs
+                            c.mma_pair(i, kc, kc + 1, rows_of(i), g);
+                            if (i + 3 < total) copy_b(i + 3);          // waits for the hi.hi MMAs of chunk i
+                            TC_TRACE(1, 0, 2 * i + 1);
+                            ++i;
+                            continue;
+                        } else {
+                            c.mma_chunk(i, kc, rows_of(i), g);
+                        }
                     }
+                    TC_TRACE(1, 0, 2 * i + 1);
+                    if (i + 2 < total) copy_b(i + 2);
                 }
-                TC_TRACE(1, 0, 2 * i + 1);
-                if (i + 2 < total) copy_b(i + 2);
+                sb += total; gb += ngroups;
             }
         }
     } else {
         const int m = (warp & 3) * 32 + lane, hf = warp >> 2;
-        const bool valid = m < tile.count;
         const uint32_t tl = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         unsigned char *a_base = smem + SM_A;
-        const float *zt = A.z_stash + (size_t)blockIdx.x * A.zs * TM + m * 4;
-        if (tid == 0) TC_TRACE(1, 1, 100);
-        // ---- h2bar = outbar W3^T: tensor core (K = n_out padded to 32) or, for the energy layer, W3's column;
-        //      z2bar = h2bar SiLU'(z2) -> A operand of GEMM R2. The z stash is read ahead of the drains. ----
-        {
-            float4 z2[CW2 / 4];
-#pragma unroll
-            for (int k4 = 0; k4 < CW2 / 4; ++k4) {
-                z2[k4] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (valid) z2[k4] = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((H1p + hf * CW2 + k4 * 4) >> 2) * (TM * 4)));
-            }
-            float x[CW2];
-            if (o1) {
-                // operand: row m of outbar in columns 0..15 (column half 0), zeros in 16..31 (half 1)
-                float ob[16];
-#pragma unroll
-                for (int c = 0; c < 16; ++c) ob[c] = 0.f;
-                if (valid && hf == 0) {
-                    const float4 *src =
-                        reinterpret_cast<const float4 *>(A.outbar + (size_t)A.sp_list[tile.start + m] * A.outbar_stride);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        if (q * 4 < A.nout) {
-                            const float4 t = __ldg(src + q);
-                            ob[q * 4] = t.x; ob[q * 4 + 1] = t.y; ob[q * 4 + 2] = t.z; ob[q * 4 + 3] = t.w;
-                        }
-#pragma unroll
-                    for (int c = 0; c < 16; ++c)
-                        if (c >= A.nout) ob[c] = 0.f;
-                }
-#pragma unroll
-                for (int k4 = 0; k4 < 4; ++k4) store_split4(a_base, hf * 4 + k4, m, ob + k4 * 4);
-                fence_async_smem();
-                mbar_arrive(bar0 + 8 * BAR_AFULL);
-#pragma unroll
-                for (int c = 0; c < CW2; ++c) x[c] = 0.f;
-                drain_group<CW2>(x, bar0, tl, 0, hf * CW2, true);   // the R1 MMAs have completed: slot 0 is free again
-            } else {
+        for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+            const DenseTile tile = A.tiles[tile_idx];
+            const DenseWT W = A.w[tile.species];
+            const bool valid = m < tile.count;
+            const float *zt = A.z_stash + (size_t)tile_idx * A.zs * TM + m * 4;
+            if (tid == 0) TC_TRACE(1, 1, 100);
+            // ---- h2bar = outbar W3^T: tensor core (K = n_out padded to 32) or, for the energy layer, W3's column;
+            //      z2bar = h2bar SiLU'(z2) -> A operand of GEMM R2. The z stash is read ahead of the drains.
+            //      (every MMA of the previous tile has completed: its last group was drained by this thread) ----
+            {
+                float4 z2[CW2 / 4];
 #pragma unroll
                 for (int k4 = 0; k4 < CW2 / 4; ++k4) {
-                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + hf * CW2 + k4 * 4));
-                    x[k4 * 4] = w4.x; x[k4 * 4 + 1] = w4.y; x[k4 * 4 + 2] = w4.z; x[k4 * 4 + 3] = w4.w;
+                    z2[k4] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (valid) z2[k4] = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((H1p + hf * CW2 + k4 * 4) >> 2) * (TM * 4)));
+                }
+                float x[CW2];
+                if (o1) {
+                    // operand: row m of outbar in columns 0..15 (column half 0), zeros in 16..31 (half 1)
+                    float ob[16];
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) ob[c] = 0.f;
+                    if (valid && hf == 0) {
+                        const float4 *src =
+                            reinterpret_cast<const float4 *>(A.outbar + (size_t)A.sp_list[tile.start + m] * A.outbar_stride);
+#pragma unroll
+                        for (int q = 0; q < 4; ++q)
+                            if (q * 4 < A.nout) {
+                                const float4 t = __ldg(src + q);
+                                ob[q * 4] = t.x; ob[q * 4 + 1] = t.y; ob[q * 4 + 2] = t.z; ob[q * 4 + 3] = t.w;
+                            }
+#pragma unroll
+                        for (int c = 0; c < 16; ++c)
+                            if (c >= A.nout) ob[c] = 0.f;
+                    }
+#pragma unroll
+                    for (int k4 = 0; k4 < 4; ++k4) store_split4(a_base, hf * 4 + k4, m, ob + k4 * 4);
+                    fence_async_smem();
+                    mbar_arrive(bar0 + 8 * BAR_AFULL);
+#pragma unroll
+                    for (int c = 0; c < CW2; ++c) x[c] = 0.f;
+                    drain_group<CW2>(x, bar0, tl, gb, hf * CW2, true);   // the R1 MMAs have completed: slot 0 is free again
+                } else {
+#pragma unroll
+                    for (int k4 = 0; k4 < CW2 / 4; ++k4) {
+                        const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + hf * CW2 + k4 * 4));
+                        x[k4 * 4] = w4.x; x[k4 * 4 + 1] = w4.y; x[k4 * 4 + 2] = w4.z; x[k4 * 4 + 3] = w4.w;
+                    }
+                }
+#pragma unroll
+                for (int k4 = 0; k4 < CW2 / 4; ++k4) {
+                    x[k4 * 4] = valid ? x[k4 * 4] * dsilu_f(z2[k4].x) : 0.f;
+                    x[k4 * 4 + 1] = valid ? x[k4 * 4 + 1] * dsilu_f(z2[k4].y) : 0.f;
+                    x[k4 * 4 + 2] = valid ? x[k4 * 4 + 2] * dsilu_f(z2[k4].z) : 0.f;
+                    x[k4 * 4 + 3] = valid ? x[k4 * 4 + 3] * dsilu_f(z2[k4].w) : 0.f;
+                }
+                store_operand<CW2>(x, a_base, bar0, hf * CW2, m);
+            }
+            if (tid == 0) TC_TRACE(1, 1, 101);
+            // ---- GEMM R2: h1bar = z2bar W2^T; z1bar = h1bar SiLU'(z1) -> resident A operand of GEMM R3 ----
+            {
+                float4 z1[CW1 / 4];
+#pragma unroll
+                for (int k4 = 0; k4 < CW1 / 4; ++k4) {
+                    z1[k4] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (valid) z1[k4] = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((hf * CW1 + k4 * 4) >> 2) * (TM * 4)));
+                }
+                float h1b[CW1];
+#pragma unroll
+                for (int c = 0; c < CW1; ++c) h1b[c] = 0.f;
+#pragma unroll 1
+                for (int kc = 0; kc < NCH2; ++kc) drain_group<CW1>(h1b, bar0, tl, gb + o1 + kc, hf * CW1, true);
+                // all MMAs of R2 have completed: the A slots may be overwritten
+#pragma unroll
+                for (int k4 = 0; k4 < CW1 / 4; ++k4) {
+                    const int col = hf * CW1 + k4 * 4;
+                    const float4 z = z1[k4];
+                    const float xv[4] = {valid ? h1b[k4 * 4] * dsilu_f(z.x) : 0.f, valid ? h1b[k4 * 4 + 1] * dsilu_f(z.y) : 0.f,
+                                         valid ? h1b[k4 * 4 + 2] * dsilu_f(z.z) : 0.f, valid ? h1b[k4 * 4 + 3] * dsilu_f(z.w) : 0.f};
+                    store_split4(a_base + (col >> 5) * A_SLOT, (col & 31) >> 2, m, xv);
+                }
+                fence_async_smem();
+                mbar_arrive(bar0 + 8 * BAR_ARES);
+            }
+            if (tid == 0) TC_TRACE(1, 1, 102);
+            // ---- GEMM R3: Qbar = z1bar U^T in blocks of <= 128 columns; this thread takes 64 of them ----
+            float *qt = A.Qbar + (size_t)tile_idx * A.K1 * TM + m * 4;
+#pragma unroll 1
+            for (int nb = 0; nb < nblk; ++nb) {
+                const int ncols = min(128, A.K1 - nb * 128);
+                const bool mine = hf * 64 < ncols;
+                float q[64];
+#pragma unroll
+                for (int c = 0; c < 64; ++c) q[c] = 0.f;
+#pragma unroll 1
+                for (int gi = 0; gi < NCH1 / GR3; ++gi) {
+                    const int g = gb + i3 + nb * (NCH1 / GR3) + gi;
+                    if (ncols - hf * 64 >= 64) drain_group<64>(q, bar0, tl, g, hf * 64, true);
+                    else if (ncols - hf * 64 >= 32) drain_group<32>(q, bar0, tl, g, hf * 64, true);
+                    else drain_group<32>(q, bar0, tl, g, hf * 64, false);
+                    if (tid == 0) TC_TRACE(1, 1, g - gb);
+                }
+                if (valid && mine) {
+#pragma unroll
+                    for (int c4 = 0; c4 < 16; ++c4) {
+                        const int col = nb * 128 + hf * 64 + c4 * 4;
+                        if (col < A.K1)
+                            *reinterpret_cast<float4 *>(qt + (size_t)(col >> 2) * (TM * 4)) =
+                                make_float4(q[c4 * 4], q[c4 * 4 + 1], q[c4 * 4 + 2], q[c4 * 4 + 3]);
+                    }
                 }
             }
-#pragma unroll
-            for (int k4 = 0; k4 < CW2 / 4; ++k4) {
-                x[k4 * 4] = valid ? x[k4 * 4] * dsilu_f(z2[k4].x) : 0.f;
-                x[k4 * 4 + 1] = valid ? x[k4 * 4 + 1] * dsilu_f(z2[k4].y) : 0.f;
-                x[k4 * 4 + 2] = valid ? x[k4 * 4 + 2] * dsilu_f(z2[k4].z) : 0.f;
-                x[k4 * 4 + 3] = valid ? x[k4 * 4 + 3] * dsilu_f(z2[k4].w) : 0.f;
-            }
-            store_operand<CW2>(x, a_base, bar0, hf * CW2, m);
+            if (tid == 0) TC_TRACE(1, 1, 103);
+            sb += total; gb += ngroups;
         }
-        if (tid == 0) TC_TRACE(1, 1, 101);
-        // ---- GEMM R2: h1bar = z2bar W2^T; z1bar = h1bar SiLU'(z1) -> resident A operand of GEMM R3 ----
-        {
-            float4 z1[CW1 / 4];
-#pragma unroll
-            for (int k4 = 0; k4 < CW1 / 4; ++k4) {
-                z1[k4] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (valid) z1[k4] = __ldg(reinterpret_cast<const float4 *>(zt + (size_t)((hf * CW1 + k4 * 4) >> 2) * (TM * 4)));
-            }
-            float h1b[CW1];
-#pragma unroll
-            for (int c = 0; c < CW1; ++c) h1b[c] = 0.f;
-#pragma unroll 1
-            for (int kc = 0; kc < NCH2; ++kc) drain_group<CW1>(h1b, bar0, tl, o1 + kc, hf * CW1, true);
-            // all MMAs of R2 have completed: the A slots may be overwritten
-#pragma unroll
-            for (int k4 = 0; k4 < CW1 / 4; ++k4) {
-                const int col = hf * CW1 + k4 * 4;
-                const float4 z = z1[k4];
-                const float xv[4] = {valid ? h1b[k4 * 4] * dsilu_f(z.x) : 0.f, valid ? h1b[k4 * 4 + 1] * dsilu_f(z.y) : 0.f,
-                                     valid ? h1b[k4 * 4 + 2] * dsilu_f(z.z) : 0.f, valid ? h1b[k4 * 4 + 3] * dsilu_f(z.w) : 0.f};
-                store_split4(a_base + (col >> 5) * A_SLOT, (col & 31) >> 2, m, xv);
-            }
-            fence_async_smem();
-            mbar_arrive(bar0 + 8 * BAR_ARES);
-        }
-        if (tid == 0) TC_TRACE(1, 1, 102);
-        // ---- GEMM R3: Qbar = z1bar U^T in blocks of <= 128 columns; this thread takes 64 of them ----
-        float *qt = A.Qbar + (size_t)blockIdx.x * A.K1 * TM + m * 4;
-#pragma unroll 1
-        for (int nb = 0; nb < nblk; ++nb) {
-            const int ncols = min(128, A.K1 - nb * 128);
-            const bool mine = hf * 64 < ncols;
-            float q[64];
-#pragma unroll
-            for (int c = 0; c < 64; ++c) q[c] = 0.f;
-#pragma unroll 1
-            for (int gi = 0; gi < NCH1 / GR3; ++gi) {
-                const int g = i3 + nb * (NCH1 / GR3) + gi;
-                if (ncols - hf * 64 >= 64) drain_group<64>(q, bar0, tl, g, hf * 64, true);
-                else if (ncols - hf * 64 >= 32) drain_group<32>(q, bar0, tl, g, hf * 64, true);
-                else drain_group<32>(q, bar0, tl, g, hf * 64, false);
-                if (tid == 0) TC_TRACE(1, 1, g);
-            }
-            if (valid && mine) {
-#pragma unroll
-                for (int c4 = 0; c4 < 16; ++c4) {
-                    const int col = nb * 128 + hf * 64 + c4 * 4;
-                    if (col < A.K1)
-                        *reinterpret_cast<float4 *>(qt + (size_t)(col >> 2) * (TM * 4)) =
-                            make_float4(q[c4 * 4], q[c4 * 4 + 1], q[c4 * 4 + 2], q[c4 * 4 + 3]);
-                }
-            }
-        }
-        if (tid == 0) TC_TRACE(1, 1, 103);
     }
     tc_epilogue(tmem);
 }
 
 // ============================================================================ host
+// persistent grid: one CTA per SM (224 KB of shared memory, all 512 TMEM columns), each walking over its tiles
+static int tc_grid(int n_tiles) {
+    static int n_sm[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) dev = 0;
+    if (!n_sm[dev] && (cudaDeviceGetAttribute(&n_sm[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm[dev] <= 0))
+        n_sm[dev] = 148;
+    return n_tiles < n_sm[dev] ? n_tiles : n_sm[dev];
+}
 template <int N1, int N2>
 int run_tc_fwd(const LaunchCtx &ctx, const TcFwdArgs &A, int n_tiles) {
-    static bool attr = false;
-    if (!attr) {
+    static bool attr[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) return REANN_ERR_UNSUPPORTED;
+    if (!attr[dev]) {   // the attribute is per device
         if (cudaFuncSetAttribute(k_dense_tc_fwd<N1, N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_TOTAL) != cudaSuccess) {
             cudaGetLastError();
             return REANN_ERR_UNSUPPORTED;
         }
-        attr = true;
+        attr[dev] = true;
     }
-    LAUNCH(ctx, (k_dense_tc_fwd<N1, N2>), n_tiles, NTHREADS, SM_TOTAL, A);
+    LAUNCH(ctx, (k_dense_tc_fwd<N1, N2>), tc_grid(n_tiles), NTHREADS, SM_TOTAL, A);
     return REANN_OK;
 }
 template <int N1, int N2>
 int run_tc_bwd(const LaunchCtx &ctx, const TcBwdArgs &A, int n_tiles) {
-    static bool attr = false;
-    if (!attr) {
+    static bool attr[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) return REANN_ERR_UNSUPPORTED;
+    if (!attr[dev]) {   // the attribute is per device
         if (cudaFuncSetAttribute(k_dense_tc_bwd<N1, N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_TOTAL) != cudaSuccess) {
             cudaGetLastError();
             return REANN_ERR_UNSUPPORTED;
         }
-        attr = true;
+        attr[dev] = true;
     }
-    LAUNCH(ctx, (k_dense_tc_bwd<N1, N2>), n_tiles, NTHREADS, SM_TOTAL, A);
+    LAUNCH(ctx, (k_dense_tc_bwd<N1, N2>), tc_grid(n_tiles), NTHREADS, SM_TOTAL, A);
     return REANN_OK;
 }
 #define TC_DISPATCH(FN, ...)                                                                    \
@@ -641,7 +705,7 @@ int launch_dense_tc_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDi
     if (ld.nout > 16) return REANN_ERR_UNSUPPORTED;
     TcFwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.Q = Q; A.z_stash = z_stash; A.out = out; A.out_stride = out_stride;
-    A.K1 = md.K1; A.nout = ld.nout; A.zs = zs;
+    A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles;
     TC_DISPATCH(run_tc_fwd, ctx, A, n_tiles)
 }
 
@@ -652,6 +716,6 @@ int launch_dense_tc_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDi
     if (ld.nout > 16) return REANN_ERR_UNSUPPORTED;
     TcBwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.z_stash = z_stash; A.outbar = outbar; A.Qbar = Qbar;
-    A.outbar_stride = outbar_stride; A.K1 = md.K1; A.nout = ld.nout; A.zs = zs;
+    A.outbar_stride = outbar_stride; A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles;
     TC_DISPATCH(run_tc_bwd, ctx, A, n_tiles)
 }

@@ -325,21 +325,23 @@ __device__ __forceinline__ void split_bits(float x, uint32_t &hi, uint32_t &lo) 
 // stores and the mma.sync fragment loads are conflict-free; phase 2: four K = 8 steps of
 // mma.sync.m16n8k8 TF32 (3xTF32: lo.hi + hi.lo + hi.hi into a fresh accumulator per step, summed in FP32
 // registers: accumulating the ~36 steps of an atom inside the MMA truncates like tcgen05 does and was measured
-// to cost 1.4e-6 eV/atom on config 2, above the 1e-6 gate). Needs N_phi = 16.
+// to cost 1.4e-6 eV/atom on config 2, above the 1e-6 gate). N_phi (padded to 4) in {8, 12, 16}: the M = 16 rows
+// beyond N_phi are zero.
 template <int NA>
 struct FwdMma {
     static constexpr int NAP = (NA + 7) & ~7, AT = NAP / 8, TS = 36;
     static constexpr int ROWS = 16 + NAP, SMEM = EW * ROWS * TS * 4;
 };
 
-template <int NA>
+template <int NPHIP, int NA>
 __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                           const uint32_t *__restrict__ col_rc,
                                                           const float4 *__restrict__ geom,
                                                           const float *__restrict__ c_ext, RadialTab rt,
                                                           float *__restrict__ b) {
     using C = FwdMma<NA>;
-    constexpr int NPHIP = 16, NAP = C::NAP, AT = C::AT, TS = C::TS;
+    constexpr int NAP = C::NAP, AT = C::AT, TS = C::TS;
+    static_assert(NPHIP == 8 || NPHIP == 12 || NPHIP == 16, "mma.sync edge forward: N_phi padded to 8, 12 or 16");
     extern __shared__ __align__(16) float smem_f[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g8 = lane >> 2, t4 = lane & 3;
     float *XT = smem_f + (size_t)warp * C::ROWS * TS, *AT_s = XT + 16 * TS;
@@ -381,7 +383,7 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
                 const float we = __shfl_sync(0xffffffffu, g.w, rr);
                 const float fce = __shfl_sync(0xffffffffu, fc, rr);
                 float4 xv = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (e0 + rr < end) {
+                if (e0 + rr < end && part * 4 < NPHIP) {
                     const int sj = cje >> COL_SPECIES_SHIFT;
                     const float4 cv = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cje & COL_IDX_MASK) * NPHIP)[part];
                     const float4 rc4 = reinterpret_cast<const float4 *>(rt.rcen + sj * NPHIP)[part];
@@ -429,7 +431,7 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
         const int a = at * 8 + 2 * t4;
         if (a < NA) {
             *reinterpret_cast<float2 *>(bi + g8 * NA + a) = make_float2(acc[at][0], acc[at][1]);
-            *reinterpret_cast<float2 *>(bi + (g8 + 8) * NA + a) = make_float2(acc[at][2], acc[at][3]);
+            if (g8 + 8 < NPHIP) *reinterpret_cast<float2 *>(bi + (g8 + 8) * NA + a) = make_float2(acc[at][2], acc[at][3]);
         }
     }
 }
@@ -657,9 +659,12 @@ __global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t
 
 // ------------------------------------------------------------------------------------------ A12
 constexpr int OUT_TPB = 256;
+// Two-level, fixed-order FP64 reductions. Block b of k_output_a: caller atoms [256 b, 256 (b+1)) (un-permute F, E_i)
+// and its share of the virial partials of the edge backward blocks; partial[b][0] = sum E_i, [1..9] = virial.
 __global__ void __launch_bounds__(OUT_TPB) k_output_a(int64_t N, const int32_t *__restrict__ inv_perm,
                                                       const double *__restrict__ Fc, const float *__restrict__ Ei,
                                                       double *__restrict__ F_out, double *__restrict__ Ei_caller,
+                                                      const double *__restrict__ vir_part, int n_vir, int want_vir,
                                                       double *__restrict__ partial) {
     __shared__ double red[OUT_TPB];
     const int64_t i = (int64_t)blockIdx.x * OUT_TPB + threadIdx.x; // caller index
@@ -676,16 +681,31 @@ __global__ void __launch_bounds__(OUT_TPB) k_output_a(int64_t N, const int32_t *
         if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
         __syncthreads();
     }
-    if (threadIdx.x == 0) partial[blockIdx.x] = red[0];
+    if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * 10] = red[0];
+    if (!want_vir) return;
+    // virial partials [v0, v1) of this block, nine sums: thread t takes component t % 9 of every (t / 9)-th entry
+    const int per = (n_vir + gridDim.x - 1) / gridDim.x;
+    const int v0 = min(n_vir, (int)blockIdx.x * per), v1 = min(n_vir, v0 + per);
+    const int q = threadIdx.x % 9, lane9 = threadIdx.x / 9;                       // 28 groups of 9 threads (252 used)
+    double s = 0.0;
+    if (lane9 < 28)
+        for (int k = v0 + lane9; k < v1; k += 28) s += vir_part[(int64_t)k * 9 + q];
+    __syncthreads();
+    red[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x < 9) {
+        double t = 0.0;
+        for (int g = 0; g < 28; ++g) t += red[g * 9 + threadIdx.x];
+        partial[(int64_t)blockIdx.x * 10 + 1 + threadIdx.x] = t;
+    }
 }
 __global__ void __launch_bounds__(OUT_TPB) k_output_b(int n_part, const double *__restrict__ partial,
-                                                      const double *__restrict__ vir_part, int n_vir,
                                                       double *__restrict__ E_out, double *__restrict__ vir_out) {
     __shared__ double red[OUT_TPB];
     for (int q = 0; q < 10; ++q) {
+        if (q > 0 && !vir_out) break;
         double s = 0.0;
-        if (q == 0) { for (int k = threadIdx.x; k < n_part; k += OUT_TPB) s += partial[k]; }
-        else if (vir_out) { for (int k = threadIdx.x; k < n_vir; k += OUT_TPB) s += vir_part[(int64_t)k * 9 + (q - 1)]; }
+        for (int k = threadIdx.x; k < n_part; k += OUT_TPB) s += partial[(int64_t)k * 10 + q];
         red[threadIdx.x] = s;
         __syncthreads();
         for (int st = OUT_TPB / 2; st > 0; st >>= 1) {
@@ -694,7 +714,7 @@ __global__ void __launch_bounds__(OUT_TPB) k_output_b(int n_part, const double *
         }
         if (threadIdx.x == 0) {
             if (q == 0) { if (E_out) *E_out = red[0]; }
-            else if (vir_out) vir_out[q - 1] = red[0];
+            else vir_out[q - 1] = red[0];
         }
         __syncthreads();
     }
@@ -738,11 +758,11 @@ void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, i
     if (work > 0) LAUNCH(ctx, k_ghost_gather, div_up(work, 256), 256, 0, c_ext, xrec, N, n_ext, nphip);
 }
 
-template <int NA>
+template <int NPHIP, int NA>
 static int run_edge_fwd_mma(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
                             const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
     using C = FwdMma<NA>;
-    LAUNCH(ctx, (k_edge_fwd_mma<NA>), div_up(N, EW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    LAUNCH(ctx, (k_edge_fwd_mma<NPHIP, NA>), div_up(N, EW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
     return REANN_OK;
 }
 
@@ -777,9 +797,17 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
                     const float *alpha, float *b, bool allow_mma) {
     if (N <= 0) return REANN_OK;
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
-    if (md.nphip == 16 && md.Na >= 10 && allow_mma)
-        return md.Na == 20 ? run_edge_fwd_mma<20>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b)
-                           : run_edge_fwd_mma<10>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    if (md.nphip >= 8 && md.Na >= 10 && allow_mma) {
+        switch (md.nphip * 100 + md.Na) {
+            case 1620: return run_edge_fwd_mma<16, 20>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+            case 1610: return run_edge_fwd_mma<16, 10>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+            case 1220: return run_edge_fwd_mma<12, 20>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+            case 1210: return run_edge_fwd_mma<12, 10>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+            case 820: return run_edge_fwd_mma<8, 20>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+            case 810: return run_edge_fwd_mma<8, 10>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+            default: break;
+        }
+    }
 #define M(NP, NA_, PN_, PA_) return run_edge_fwd<NP, NA_, PN_, PA_>(ctx, N, rc_ptr, col_rc, geom, c_ext, rt, b);
     EDGE_DISPATCH(M)
 #undef M
@@ -825,8 +853,8 @@ void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, con
                    const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
                    double *Ei_caller, double *scratch) {
     const int nb = (int)div_up(N > 0 ? N : 1, OUT_TPB);
-    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, scratch);
-    LAUNCH(ctx, k_output_b, 1, OUT_TPB, 0, nb, (const double *)scratch, vir_part, n_vir_blocks, E_out, vir_out);
+    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, vir_part, n_vir_blocks, vir_out != nullptr, scratch);
+    LAUNCH(ctx, k_output_b, 1, OUT_TPB, 0, nb, (const double *)scratch, E_out, vir_out);
 }
 
 void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
