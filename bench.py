@@ -194,9 +194,14 @@ def main():
     ap.add_argument("--ref-atoms", type=int, default=24000, help="atoms of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--T", type=int, default=None, help="override the number of layers (config 4 sweep)")
+    ap.add_argument("--mlp-mode", default="fp32", choices=["fp32", "tf32"],
+                    help="fp32 (default, 3xTF32 tensor-core GEMMs at FP32-class accuracy, the headline) or tf32 (plain TF32 "
+                         "GEMMs, one accumulator per GEMM; tolerance restated in DESIGN.md section 2)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.mlp_mode == "tf32":
+        os.environ["REANN_MLP_MODE"] = "tf32"      # read by the library once, at reann_create
 
     import torch
     import torch.distributed as dist
@@ -377,12 +382,12 @@ def main():
                                           "algorithmic_per_launch": nb_bytes, "algorithmic_unit": "bytes"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32", "data": "synthetic",
+                "dtype": "f32" if args.mlp_mode == "fp32" else "tf32 (MLP GEMMs), f32 elsewhere", "data": "synthetic",
                 "config": {"workload": f"config {args.config}: {cfg['name']} ({n} atoms, rc={cfg['rc']}, skin={cfg['skin']}, "
                                        f"T={T}, L={L}, n_gauss={nphi}, MLP {H1}x{H2}), velocity-Verlet 0.5 fs at 300 K",
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "working set (compact edge list + stash, >300 MB) exceeds the 126 MB L2; no flush needed",
-                           "virial": True, "profiling_in_timed_region": False,
+                           "virial": True, "profiling_in_timed_region": False, "mlp_mode": args.mlp_mode,
                            "rebuilds_in_timed_region": s1["n_rebuilds"] - s0["n_rebuilds"],
                            "n_edges_rc": E_rc, "n_edges_list": E_list, "n_ext": n_ext,
                            "stash_chunks": s1["stash_chunks"], "device_bytes": s1["bytes_device"]},

@@ -182,6 +182,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         auto is = [](const char *name, const char *val) { const char *e = getenv(name); return e && strcmp(e, val) == 0; };
         h->dense_tc = !is("REANN_DENSE", "simt");
         h->edge_fwd_mma = !is("REANN_EDGE_FWD", "simt");
+        h->mlp_tf32 = is("REANN_MLP_MODE", "tf32") && h->dense_tc;
         if (const char *e = getenv("REANN_STASH_CHUNKS")) h->stash_chunks_forced = std::max(0, atoi(e));
     }
     md.rc = rc; md.skin = skin;
@@ -577,7 +578,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         rcode = h->dense_tc
                     ? launch_dense_tc_fwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
                                           (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
-                                          last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip)
+                                          last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip, h->mlp_tf32)
                     : launch_dense_fwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
                                        (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
                                        last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip);
@@ -598,7 +599,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         int rcode = h->dense_tc
                         ? launch_dense_tc_bwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
                                               (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
-                                              last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p)
+                                              last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p, h->mlp_tf32)
                         : launch_dense_bwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
                                            (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
                                            last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);

@@ -150,7 +150,7 @@ int launch_dense_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims 
 #define DENSE_TC_TM 128
 int launch_dense_tc_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
                         const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash,
-                        int zs, float *out, int out_stride);
+                        int zs, float *out, int out_stride, bool tf32 /* REANN_MLP_MODE=tf32 */);
 int launch_dense_tc_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
                         const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *z_stash, int zs,
-                        const float *outbar, int outbar_stride, float *Qbar);
+                        const float *outbar, int outbar_stride, float *Qbar, bool tf32);

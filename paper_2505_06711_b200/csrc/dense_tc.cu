@@ -136,13 +136,14 @@ __device__ __forceinline__ void tc_epilogue(uint32_t tmem) {
 struct Ctl {
     uint32_t bar0, a0, b0, tmem;
     int sb, gb;
+    bool tf32;   // REANN_MLP_MODE=tf32: hi images only, one accumulator per GEMM (see mma_chunk_1x)
     __device__ __forceinline__ uint32_t bar(int k) const { return bar0 + 8u * (uint32_t)k; }
     // stream the weight chunk of step i into its B slot (after the MMAs of step i-3 released it)
     __device__ __forceinline__ void copy_b(int i_loc, const float *src, int n_rows) const {
         const int i = sb + i_loc;
         const int s = i % NSTAGE;
         if (i >= NSTAGE) mbar_wait(bar(BAR_MMA + s), (uint32_t)(((i / NSTAGE) - 1) & 1));
-        const uint32_t bytes = (uint32_t)n_rows * KC * 4 * 2;
+        const uint32_t bytes = (uint32_t)n_rows * KC * 4 * (tf32 ? 1 : 2);     // the lo image follows the hi image
         if (elect_one()) {
             mbar_expect_tx(bar(BAR_BFULL + s), bytes);
             bulk_g2s(b0 + (uint32_t)s * B_SLOT, src, bytes, bar(BAR_BFULL + s));
@@ -163,6 +164,22 @@ struct Ctl {
             issue(i, a_slot, n_rows, dm, false, true, false);
             tc_commit(bar(BAR_MMA + s));
             tc_commit(bar(BAR_DFULL + d));
+        }
+        __syncwarp();
+    }
+    // Plain TF32 (the fast mode with a restated tolerance): D (+)= A_hi B_hi^T only, the chunks of one GEMM accumulate
+    // in ONE buffer (first: overwrite; last: hand the buffer to the compute threads) -- one TMEM drain per GEMM
+    __device__ __forceinline__ void mma_chunk_1x(int i_loc, int a_slot, int n_rows, int g_loc, bool first, bool last) const {
+        const int i = sb + i_loc, g = gb + g_loc;
+        const int s = i % NSTAGE, d = g % NBUF;
+        if (first && g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
+        mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
+        tc_fence_after();
+        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
+        if (elect_one()) {
+            issue(i, a_slot, n_rows, dm, false, true, first);
+            tc_commit(bar(BAR_MMA + s));
+            if (last) tc_commit(bar(BAR_DFULL + d));
         }
         __syncwarp();
     }
@@ -201,7 +218,7 @@ struct Ctl {
                 umma_tf32(dm, al, bh, idesc, (fresh && kk == 0) ? 0u : 1u);
                 umma_tf32(dm, ah, bl, idesc, 1u);
             }
-            if (main) umma_tf32(dm, ah, bh, idesc, 1u);
+            if (main) umma_tf32(dm, ah, bh, idesc, (fresh && !corr && kk == 0) ? 0u : 1u);
         }
     }
 };
@@ -259,7 +276,7 @@ struct TcFwdArgs {
     const float *Q;         // tile-quad layout, K1 columns
     float *z_stash;         // tile-quad layout, zs columns (z1 | z2)
     float *out;             // rows of stride out_stride, atom order
-    int out_stride, K1, nout, zs, n_tiles;
+    int out_stride, K1, nout, zs, n_tiles, tf32;
 };
 
 template <int NCH1, int NCH2>
@@ -277,7 +294,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
 
     if (warp_u == CTL_WARP) {
         {   // the whole warp walks the control flow (warp-uniform: descriptors in uniform registers); one lane acts
-            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0};
+            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
             const uint32_t stg = c.a0 + 3u * A_SLOT;
             for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
                 const DenseTile tile = A.tiles[tile_idx];
@@ -309,16 +326,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                         mbar_wait(c.bar(BAR_AFULL + sa), (uint32_t)((j / NSTAGE) & 1));
                         if (i + 2 < n1) issue_q(i + 2);
                         TC_TRACE(0, 0, 2 * i);
-                        c.mma_chunk(i, sa, H1p, i);
+                        if (A.tf32) c.mma_chunk_1x(i, sa, H1p, 0, i == 0, i == n1 - 1);
+                        else c.mma_chunk(i, sa, H1p, i);
                     } else {
                         mbar_wait(c.bar(BAR_AH + (i - n1)), (uint32_t)(it & 1));
                         TC_TRACE(0, 0, 2 * i);
-                        c.mma_chunk(i, i - n1, H2p, i);
+                        if (A.tf32) c.mma_chunk_1x(i, i - n1, H2p, 1, i == n1, i == total - 1);
+                        else c.mma_chunk(i, i - n1, H2p, i);
                     }
                     TC_TRACE(0, 0, 2 * i + 1);
                     if (i + 2 < total) copy_b(i + 2);
                 }
-                sb += total; gb += total; qb += n1;
+                sb += total; gb += A.tf32 ? 2 : total; qb += n1;
             }
         }
     } else {
@@ -359,10 +378,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 mbar_arrive(bar0 + 8 * (BAR_AFULL + sa));
                 mbar_arrive(bar0 + 8 * (BAR_QEMPTY + qs));
                 if (tid == 0) TC_TRACE(0, 1, 2 * i);
-                if (i >= 1) drain_group<CW1>(acc1, bar0, tl, gb + i - 1, hf * CW1, true);
+                if (i >= 1 && !A.tf32) drain_group<CW1>(acc1, bar0, tl, gb + i - 1, hf * CW1, true);
                 if (tid == 0) TC_TRACE(0, 1, 2 * i + 1);
             }
-            drain_group<CW1>(acc1, bar0, tl, gb + n1 - 1, hf * CW1, true);
+            drain_group<CW1>(acc1, bar0, tl, A.tf32 ? gb : gb + n1 - 1, hf * CW1, true);
             if (tid == 0) TC_TRACE(0, 1, 101);
             // ---- z1 = acc + b1 (stash), h1 = SiLU(z1) -> A operand of GEMM 2 ----
 #pragma unroll
@@ -381,8 +400,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
             float acc2[CW2];
 #pragma unroll
             for (int c = 0; c < CW2; ++c) acc2[c] = 0.f;
+            if (A.tf32) drain_group<CW2>(acc2, bar0, tl, gb + 1, hf * CW2, true);
+            else {
 #pragma unroll 1
-            for (int kc = 0; kc < NCH1; ++kc) drain_group<CW2>(acc2, bar0, tl, gb + n1 + kc, hf * CW2, true);
+                for (int kc = 0; kc < NCH1; ++kc) drain_group<CW2>(acc2, bar0, tl, gb + n1 + kc, hf * CW2, true);
+            }
             if (tid == 0) TC_TRACE(0, 1, 103);
             // ---- z2 (stash), h2 = SiLU(z2), out = h2 W3 + b3 in FP32 (partial over this column half) ----
             float o[16];
@@ -436,7 +458,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
             // tile done: the operand slots (and the exchange area) may be reused by the next tile
             compute_sync();
             if (tid == 0) mbar_arrive(bar0 + 8 * BAR_TDONE);
-            sb += total; gb += total; qb += n1;
+            sb += total; gb += A.tf32 ? 2 : total; qb += n1;
         }
     }
     tc_epilogue(tmem);
@@ -449,7 +471,7 @@ struct TcBwdArgs {
     const int32_t *sp_list;
     const float *z_stash, *outbar; // outbar == nullptr: energy layer (outbar = 1)
     float *Qbar;                   // tile-quad layout, K1 columns
-    int outbar_stride, K1, nout, zs, n_tiles;
+    int outbar_stride, K1, nout, zs, n_tiles, tf32;
 };
 
 template <int NCH1, int NCH2>
@@ -469,7 +491,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
 
     if (warp_u == CTL_WARP) {
         {   // the whole warp walks the control flow (warp-uniform); one elected lane acts
-            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0};
+            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
             for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
                 const DenseTile tile = A.tiles[tile_idx];
                 const DenseWT W = A.w[tile.species];
@@ -487,11 +509,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                     if (i < o1) {
                         mbar_wait(c.bar(BAR_AFULL), (uint32_t)(it & 1));
                         TC_TRACE(1, 0, 2 * i);
-                        c.mma_chunk(i, 0, H2p, i);
+                        if (A.tf32) c.mma_chunk_1x(i, 0, H2p, 0, true, true);
+                        else c.mma_chunk(i, 0, H2p, i);
                     } else if (i < i3) {
                         mbar_wait(c.bar(BAR_AH + (i - o1)), (uint32_t)(it & 1));
                         TC_TRACE(1, 0, 2 * i);
-                        c.mma_chunk(i, i - o1, H1p, i);
+                        if (A.tf32) c.mma_chunk_1x(i, i - o1, H1p, o1, i == o1, i == i3 - 1);
+                        else c.mma_chunk(i, i - o1, H1p, i);
+                    } else if (A.tf32) {
+                        // R3, plain TF32: one accumulator per block of <= 128 output columns (K = H1p)
+                        if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
+                        const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1;
+                        c.mma_chunk_1x(i, kc, rows_of(i), o1 + 1 + nb, kc == 0, kc == NCH1 - 1);
                     } else {
                         // R3: groups of GR3 chunks (K = 32 GR3 per accumulator); group index continues after R2
                         if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
@@ -511,7 +540,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                     TC_TRACE(1, 0, 2 * i + 1);
                     if (i + 2 < total) copy_b(i + 2);
                 }
-                sb += total; gb += ngroups;
+                sb += total; gb += A.tf32 ? o1 + 1 + nblk : ngroups;
             }
         }
     } else {
@@ -588,8 +617,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                 float h1b[CW1];
 #pragma unroll
                 for (int c = 0; c < CW1; ++c) h1b[c] = 0.f;
+                if (A.tf32) drain_group<CW1>(h1b, bar0, tl, gb + o1, hf * CW1, true);
+                else {
 #pragma unroll 1
-                for (int kc = 0; kc < NCH2; ++kc) drain_group<CW1>(h1b, bar0, tl, gb + o1 + kc, hf * CW1, true);
+                    for (int kc = 0; kc < NCH2; ++kc) drain_group<CW1>(h1b, bar0, tl, gb + o1 + kc, hf * CW1, true);
+                }
                 // all MMAs of R2 have completed: the A slots may be overwritten
 #pragma unroll
                 for (int k4 = 0; k4 < CW1 / 4; ++k4) {
@@ -612,9 +644,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                 float q[64];
 #pragma unroll
                 for (int c = 0; c < 64; ++c) q[c] = 0.f;
+                const int ngr = A.tf32 ? 1 : NCH1 / GR3;
 #pragma unroll 1
-                for (int gi = 0; gi < NCH1 / GR3; ++gi) {
-                    const int g = gb + i3 + nb * (NCH1 / GR3) + gi;
+                for (int gi = 0; gi < ngr; ++gi) {
+                    const int g = A.tf32 ? gb + o1 + 1 + nb : gb + i3 + nb * (NCH1 / GR3) + gi;
                     if (ncols - hf * 64 >= 64) drain_group<64>(q, bar0, tl, g, hf * 64, true);
                     else if (ncols - hf * 64 >= 32) drain_group<32>(q, bar0, tl, g, hf * 64, true);
                     else drain_group<32>(q, bar0, tl, g, hf * 64, false);
@@ -631,7 +664,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                 }
             }
             if (tid == 0) TC_TRACE(1, 1, 103);
-            sb += total; gb += ngroups;
+            sb += total; gb += A.tf32 ? o1 + 1 + nblk : ngroups;
         }
     }
     tc_epilogue(tmem);
@@ -700,22 +733,22 @@ extern "C" int reann_debug_tc_trace(long long *out) {
 
 int launch_dense_tc_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
                         const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *Q, float *z_stash,
-                        int zs, float *out, int out_stride) {
+                        int zs, float *out, int out_stride, bool tf32) {
     if (n_tiles <= 0) return REANN_OK;
     if (ld.nout > 16) return REANN_ERR_UNSUPPORTED;
     TcFwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.Q = Q; A.z_stash = z_stash; A.out = out; A.out_stride = out_stride;
-    A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles;
+    A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles; A.tf32 = tf32;
     TC_DISPATCH(run_tc_fwd, ctx, A, n_tiles)
 }
 
 int launch_dense_tc_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims &ld, const DenseWT *d_w,
                         const DenseTile *tiles, int n_tiles, const int32_t *sp_list, const float *z_stash, int zs,
-                        const float *outbar, int outbar_stride, float *Qbar) {
+                        const float *outbar, int outbar_stride, float *Qbar, bool tf32) {
     if (n_tiles <= 0) return REANN_OK;
     if (ld.nout > 16) return REANN_ERR_UNSUPPORTED;
     TcBwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.z_stash = z_stash; A.outbar = outbar; A.Qbar = Qbar;
-    A.outbar_stride = outbar_stride; A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles;
+    A.outbar_stride = outbar_stride; A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles; A.tf32 = tf32;
     TC_DISPATCH(run_tc_bwd, ctx, A, n_tiles)
 }

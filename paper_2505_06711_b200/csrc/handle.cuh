@@ -18,6 +18,7 @@ struct reann {
     bool dense_tc = true;         // REANN_DENSE=simt selects the FP32 SIMT GEMM chain instead
     bool edge_fwd_mma = true;     // REANN_EDGE_FWD=simt: FP32 ALU edge forward where the mma.sync kernel applies
     int stash_chunks_forced = 0;  // REANN_STASH_CHUNKS=n
+    bool mlp_tf32 = false;        // REANN_MLP_MODE=tf32: plain TF32 GEMMs (one accumulator per GEMM), tolerance restated
     DevBuf rcen, alpha, c0;       // [T][S][nphip] (alpha pre-multiplied by log2(e)), [S][nphip]
     std::vector<DenseW> h_wtab;   // host copy of the table (device pointers inside)
 

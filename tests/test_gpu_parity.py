@@ -402,6 +402,34 @@ def test_non_default_kernel_variants_parity(env):
     assert r.stdout.count("[parity] variant") == 2
 
 
+def test_fast_mlp_mode_tf32_restated_tolerance():
+    """REANN_MLP_MODE=tf32: plain TF32 tensor-core GEMMs (operands rounded to 11 significant bits, one accumulator
+    per GEMM). north_star: "tolerance restated for any BF16 [reduced-precision] MLP variant". Restated gates
+    (B-7; twice the largest error measured over these cases): |dE|/N <= 2e-3 eV/atom and
+    rms|dF| <= 0.06 rms|F| (the T = 6 stack of config 4 is the worst case: 1.0e-3 and 0.039); the FP32-class
+    default keeps north_star's 1e-6 / 5e-4. The mode is read once per handle, hence the subprocess."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import sys; sys.path.insert(0, %r)\n"
+        "import numpy as np, gen, oracle\nimport paper_2505_06711_b200 as R\n"
+        "worst_E = worst_F = 0.0\n"
+        "for k, kw in ((1, {}), (2, dict(n_mol=300)), (3, dict(n_mol=700)), (4, dict(ncell=7, T=6))):\n"
+        "    cfg = gen.make_config(k, **kw)\n"
+        "    m = R.Reann.from_config(cfg); m.build_neighbors(cfg['pos'], cfg['box'])\n"
+        "    E, F, V = m.energy_forces(cfg['pos'], cfg['box'])\n"
+        "    ref = oracle.energy_forces(cfg['blob'], cfg['species'], cfg['pos'], cfg['box'])\n"
+        "    dE = abs(E - ref['E']) / m.n; rF = np.sqrt(((F - ref['F']) ** 2).mean() / (ref['F'] ** 2).mean())\n"
+        "    print('[tf32] cfg%%d dE/N=%%.2e rms dF/rms F=%%.2e' %% (k, dE, rF))\n"
+        "    assert dE <= 2e-3 * max(1.0, abs(ref['E']) / m.n) and rF <= 0.06, (k, dE, rF)\n"
+        "    assert dE > 2e-6 or rF > 1e-4, 'suspiciously exact: is the tf32 mode really on?'\n"
+        "    m.close()\n" % root)
+    r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, REANN_MLP_MODE="tf32"), capture_output=True,
+                       text=True, timeout=600)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("[tf32]") == 4
+
+
 def test_stash_chunks_memory_limited_path(R, monkeypatch):
     """Config 5 needs the kappa stash in chunks of atoms to fit 180 GB; REANN_STASH_CHUNKS forces the same code
     path on a small system: parity with the oracle, and the same result as the unchunked run up to the
