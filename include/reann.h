@@ -15,10 +15,17 @@
  *    Positions need not be wrapped into the box.
  *  - Ownership: the caller owns every array it passes; the library copies what it keeps
  *    (weights, species) and never retains caller pointers past the call.
- *  - With device pointers the work is enqueued on the handle's stream; the call synchronises
- *    the stream once (to read the skin-check flag) and returns with the output kernels
- *    enqueued, not necessarily finished. With host pointers the call returns after the
- *    results are copied back.
+ *  - Synchronisation: reann_energy_forces enqueues the whole evaluation on the handle's stream
+ *    without a host round trip in the middle (the skin criterion and the capacity of the
+ *    compact-edge buffers are checked on the device; the kernels after the check return at once
+ *    when either fails) and synchronises the stream ONCE, at the end, to read that flag word: a
+ *    rebuild or a buffer growth is followed by a second pass inside the same call. When the
+ *    call returns, the outputs are complete (device or host pointers alike). With device
+ *    pointers the steady-state launch sequence is a CUDA graph, re-captured after every rebuild
+ *    (REANN_GRAPH=0 switches it off). The handle never works on the legacy default stream (a
+ *    graph cannot be captured there): until reann_set_stream gives it a stream, or when that
+ *    stream is 0, it uses a blocking stream of its own, which is ordered after earlier work of
+ *    the default stream. Systems whose per-edge stash is held in chunks synchronise once more.
  *  - Every function returns a REANN_* code, never throws or aborts; reann_last_error() gives
  *    text for the last failure on that handle.
  *  - Determinism: same inputs give bitwise-identical outputs (no floating-point atomics;
@@ -27,8 +34,9 @@
  *    that skin-triggered rebuilds do not allocate. When the per-edge stash of the reverse pass
  *    (4 n_gauss bytes per edge within rc) does not fit into the free device memory it is held
  *    for a fraction of the atoms at a time (transparent to the caller).
- *  - Environment switches read by the library (kernel selection, for testing):
- *    REANN_DENSE=simt, REANN_EDGE_FWD=simt, REANN_EDGE=mma, REANN_STASH_CHUNKS=n.
+ *  - Environment switches, read once per handle at reann_create:
+ *    REANN_DENSE=simt, REANN_EDGE_FWD=simt (kernel selection, for testing), REANN_STASH_CHUNKS=n,
+ *    REANN_GRAPH=0, REANN_MLP_MODE=tf32 (plain TF32 MLP GEMMs; accuracy restated in DESIGN.md).
  */
 #ifndef REANN_H
 #define REANN_H

@@ -184,6 +184,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         h->edge_fwd_mma = !is("REANN_EDGE_FWD", "simt");
         h->mlp_tf32 = is("REANN_MLP_MODE", "tf32") && h->dense_tc;
         if (const char *e = getenv("REANN_STASH_CHUNKS")) h->stash_chunks_forced = std::max(0, atoi(e));
+        h->use_graph = !is("REANN_GRAPH", "0");
     }
     md.rc = rc; md.skin = skin;
     h->zs = 0;
@@ -338,6 +339,8 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
     }
     CRC(dev_ensure(h, h->flags, 64));
     CCU(cudaMemset(h->flags.p, 0, 64));
+    CCU(cudaStreamCreate(&h->own_stream));
+    h->stream = h->own_stream;
     CCU(cudaMallocHost((void **)&h->h_flags, 64));
     *out = h;
     return REANN_OK;
@@ -346,6 +349,8 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
 extern "C" void reann_destroy(reann_t *h) {
     if (!h) return;
     if (h->stream) cudaStreamSynchronize(h->stream); else cudaDeviceSynchronize();
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    if (h->own_stream) cudaStreamDestroy(h->own_stream);
     DevBuf *bufs[] = {&h->w_all, &h->w_tab, &h->wt_all, &h->wt_tab, &h->rcen, &h->alpha, &h->c0, &h->species_caller, &h->tiles,
                       &h->pos_build, &h->wshift, &h->perm, &h->inv_perm, &h->xrec, &h->img_index, &h->cell_start,
                       &h->cell_rank, &h->row_ptr, &h->col, &h->rev, &h->sp_list, &h->scratch_a, &h->scratch_b,
@@ -360,10 +365,17 @@ extern "C" void reann_destroy(reann_t *h) {
 
 extern "C" const char *reann_last_error(const reann_t *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
+static void graph_drop(reann *h) {
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+}
+
+// The legacy default stream (0) cannot be captured into a CUDA graph, so the handle then works on a blocking stream
+// of its own: it is ordered after earlier work of the default stream, and every call ends with a synchronisation.
 extern "C" int reann_set_stream(reann_t *h, void *cuda_stream) {
     if (!h) return REANN_ERR_ARG;
-    if (h->stream) cudaStreamSynchronize(h->stream); else cudaDeviceSynchronize();
-    h->stream = (cudaStream_t)cuda_stream;
+    cudaStreamSynchronize(h->stream);
+    graph_drop(h);
+    h->stream = cuda_stream ? (cudaStream_t)cuda_stream : h->own_stream;
     return REANN_OK;
 }
 
@@ -473,8 +485,19 @@ struct Marks {
     }
 };
 
-// skin check + speculative rc-filter count on the current list; ONE stream sync to read both
-static int prep_and_sync(reann *h, const double *d_pos, bool *rebuild, int64_t *n_rc) {
+// ---- device flag word (h->flags[0]) of one evaluation; the kernels after the rc-filter count return at once when
+// it is non-zero (LaunchCtx::skip), the host reads it after the evaluation ----
+enum { FLAG_REBUILD = 1, FLAG_OVERFLOW = 2 };
+
+__global__ void k_cap_check(const int64_t *__restrict__ n_rc, int64_t cap, int32_t *__restrict__ flags,
+                            int64_t *__restrict__ n_rc_out) {
+    if (*n_rc > cap) atomicOr(flags, FLAG_OVERFLOW);
+    *n_rc_out = *n_rc;
+}
+
+// A4 + per-step prep on the current list: skin check (sets FLAG_REBUILD), positions of the ext atoms, rc-filter count,
+// offsets of the compact rows, capacity check (sets FLAG_OVERFLOW). No host synchronisation.
+static int enqueue_prep(reann *h, const double *d_pos) {
     LaunchCtx ctx = h->ctx();
     const int64_t N = h->N;
     const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
@@ -487,73 +510,48 @@ static int prep_and_sync(reann *h, const double *d_pos, bool *rebuild, int64_t *
     launch_filter_count(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p, N, Lx,
                         Ly, Lz, h->md.rc * h->md.rc, (uint16_t *)h->rank16.p, (int32_t *)h->rc_cnt.p);
     exclusive_scan_i32_to_i64(ctx, (const int32_t *)h->rc_cnt.p, (int64_t *)h->rc_ptr.p, N, h->scan_ws.p);
-    CU(h, cudaMemcpyAsync(h->h_flags, flags, 4, cudaMemcpyDeviceToHost, h->stream));
-    CU(h, cudaMemcpyAsync(h->h_flags + 2, (int64_t *)h->rc_ptr.p + N, 8, cudaMemcpyDeviceToHost, h->stream));
-    CU(h, cudaStreamSynchronize(h->stream));
-    *rebuild = (h->h_flags[0] & 1) != 0;
-    memcpy(n_rc, h->h_flags + 2, 8);
+    LAUNCH(ctx, k_cap_check, 1, 1, 0, (const int64_t *)h->rc_ptr.p + N, h->cap_rc, flags, (int64_t *)(flags + 2));
     return REANN_OK;
 }
 
-extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *box9, double *E, double *F,
-                                   double *virial) {
-    if (!h) return REANN_ERR_ARG;
-    if (!h->have_list) return set_err(h, REANN_ERR_NO_NEIGHBORS, "call reann_build_neighbors first");
-    RC(check_box(h, box9));
+// (re)size the buffers that follow the compact edge count; chooses the stash chunk count (config 5)
+static int ensure_rc_capacity(reann *h, int64_t n_rc) {
+    if (n_rc <= h->cap_rc) return REANN_OK;
+    const ModelDims &md = h->md;
+    const int64_t cap = n_rc + n_rc / 16 + 1024;
+    dev_free(h, h->kappa);
+    RC(dev_ensure(h, h->col_rc, sizeof(uint32_t) * (size_t)cap));
+    RC(dev_ensure(h, h->rev_rc, sizeof(uint32_t) * (size_t)cap));
+    RC(dev_ensure(h, h->geom, sizeof(float4) * (size_t)cap));
+    RC(dev_ensure(h, h->gst, sizeof(float4) * (size_t)cap));
+    // kappa stash (4 N_phi bytes per edge, one layer live): whole if it fits into what is left of the device
+    // memory, else in chunks of atoms -- k_edge_bwd / k_rev_gather then run once per chunk (config 5)
+    const size_t whole = sizeof(float) * (size_t)cap * md.nphip;
+    size_t free_b = 0, total_b = 0;
+    CU(h, cudaMemGetInfo(&free_b, &total_b));
+    const size_t budget = free_b > ((size_t)3 << 30) ? free_b - ((size_t)3 << 30) : free_b / 2;
+    int C = 1;
+    if (h->stash_chunks_forced > 0) C = h->stash_chunks_forced;
+    else while (C < 64 && (C == 1 ? whole : whole / C + whole / (8 * C)) > budget) ++C;
+    h->stash_chunks = C;
+    RC(dev_ensure(h, h->kappa, C == 1 ? whole : whole / C + whole / (8 * C)));
+    h->cap_rc = cap;
+    return REANN_OK;
+}
+
+struct OutPtrs {      // where the kernels write (device), and what has to be copied back to host pointers
+    double *dE, *dF, *dV;
+    bool E_host, F_host, V_host;
+};
+
+// everything after the prep: compact list, T forward layers, reverse pass, outputs. ch_atom / ch_edge: stash chunks.
+static int enqueue_layers(reann *h, Marks &mk, const OutPtrs &o, bool want_vir, const std::vector<int64_t> &ch_atom,
+                          const std::vector<int64_t> &ch_edge, bool guarded) {
     const ModelDims &md = h->md;
     const int64_t N = h->N;
-    const double *d_pos = nullptr;
-    RC(device_positions(h, pos, &d_pos));
-    h->n_calls++;
-    Marks mk{h, {}};
-    mk.mark(1);
     LaunchCtx ctx = h->ctx();
-
-    // ---- A4 + rc-filter count; rebuild when the skin criterion or a box change asks for it ----
-    bool rebuild = false;
-    int64_t n_rc = 0;
-    const bool box_changed = memcmp(box9, h->box_build, sizeof(double) * 9) != 0;
-    if (N > 0) {
-        if (!box_changed) RC(prep_and_sync(h, d_pos, &rebuild, &n_rc));
-        if (box_changed || rebuild) {
-            RC(do_build(h, d_pos, box9));
-            RC(prep_and_sync(h, d_pos, &rebuild, &n_rc));
-        }
-    }
-    h->E_rc = n_rc;
-    if (n_rc > h->cap_rc) {
-        const int64_t cap = n_rc + n_rc / 16 + 1024;
-        dev_free(h, h->kappa);
-        RC(dev_ensure(h, h->col_rc, sizeof(uint32_t) * (size_t)cap));
-        RC(dev_ensure(h, h->rev_rc, sizeof(uint32_t) * (size_t)cap));
-        RC(dev_ensure(h, h->geom, sizeof(float4) * (size_t)cap));
-        RC(dev_ensure(h, h->gst, sizeof(float4) * (size_t)cap));
-        // kappa stash (4 N_phi bytes per edge, one layer live): whole if it fits into what is left of the device
-        // memory, else in chunks of atoms -- k_edge_bwd / k_rev_gather then run once per chunk (config 5)
-        const size_t whole = sizeof(float) * (size_t)cap * md.nphip;
-        size_t free_b = 0, total_b = 0;
-        CU(h, cudaMemGetInfo(&free_b, &total_b));
-        const size_t budget = free_b > ((size_t)3 << 30) ? free_b - ((size_t)3 << 30) : free_b / 2;
-        int C = 1;
-        if (h->stash_chunks_forced > 0) C = h->stash_chunks_forced;
-        else while (C < 64 && (C == 1 ? whole : whole / C + whole / (8 * C)) > budget) ++C;
-        h->stash_chunks = C;
-        RC(dev_ensure(h, h->kappa, C == 1 ? whole : whole / C + whole / (8 * C)));
-        h->cap_rc = cap;
-    }
-    // atom / edge ranges of the stash chunks
-    const int C = (N > 0) ? h->stash_chunks : 1;
-    std::vector<int64_t> ch_atom((size_t)C + 1, 0), ch_edge((size_t)C + 1, 0);
-    ch_atom[(size_t)C] = N; ch_edge[(size_t)C] = n_rc;
-    if (C > 1) {
-        for (int c = 1; c < C; ++c) ch_atom[(size_t)c] = ((N * c / C) + 3) & ~(int64_t)3;
-        for (int c = 1; c < C; ++c)
-            CU(h, cudaMemcpyAsync(&ch_edge[(size_t)c], (const int64_t *)h->rc_ptr.p + ch_atom[(size_t)c], 8, cudaMemcpyDeviceToHost, h->stream));
-        CU(h, cudaStreamSynchronize(h->stream));
-        int64_t widest = 0;
-        for (int c = 0; c < C; ++c) widest = std::max(widest, ch_edge[(size_t)c + 1] - ch_edge[(size_t)c]);
-        RC(dev_ensure(h, h->kappa, sizeof(float) * (size_t)widest * md.nphip));
-    }
+    if (guarded) ctx.skip = (const int32_t *)h->flags.p;
+    const int C = (int)ch_atom.size() - 1;
     const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
     launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
                        (const uint32_t *)h->rev.p, N, Lx, Ly, Lz, (const uint16_t *)h->rank16.p,
@@ -612,7 +610,7 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
             rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
                                     (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
                                     (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
-                                    (float4 *)h->gst.p, virial ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
+                                    (float4 *)h->gst.p, want_vir ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
                                     ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
             if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
             mk.mark(t >= 1 ? 7 : 9);
@@ -625,20 +623,121 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
     }
     // ---- outputs (A12) ----
     mk.mark(8);
+    launch_output(ctx, N, (const int32_t *)h->inv_perm.p, (const double *)h->Fc.p, (const float *)h->Ei.p,
+                  (const double *)h->vir_part.p, N > 0 ? h->n_vir_blocks : 0, o.dE, o.dF, o.dV, (double *)h->Ei_caller.p,
+                  (double *)h->red_scratch.p);
+    return REANN_OK;
+}
+
+extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *box9, double *E, double *F,
+                                   double *virial) {
+    if (!h) return REANN_ERR_ARG;
+    if (!h->have_list) return set_err(h, REANN_ERR_NO_NEIGHBORS, "call reann_build_neighbors first");
+    RC(check_box(h, box9));
+    const ModelDims &md = h->md;
+    const int64_t N = h->N;
+    const double *d_pos = nullptr;
+    RC(device_positions(h, pos, &d_pos));
+    h->n_calls++;
+    Marks mk{h, {}};
+    mk.mark(1);
+
     const bool E_dev = is_device_ptr(E), F_dev = is_device_ptr(F), V_dev = is_device_ptr(virial);
     double *stage = (double *)h->out_stage.p;
-    double *dE = E ? (E_dev ? E : stage) : stage;
-    double *dV = virial ? (V_dev ? virial : stage + 1) : nullptr;
-    double *dF = F ? (F_dev ? F : stage + 16) : nullptr;
-    launch_output(ctx, N, (const int32_t *)h->inv_perm.p, (const double *)h->Fc.p, (const float *)h->Ei.p,
-                  (const double *)h->vir_part.p, N > 0 ? h->n_vir_blocks : 0, dE, dF, dV, (double *)h->Ei_caller.p,
-                  (double *)h->red_scratch.p);
-    bool need_sync = false;
-    if (E && !E_dev) { CU(h, cudaMemcpyAsync(E, stage, 8, cudaMemcpyDeviceToHost, h->stream)); need_sync = true; }
-    if (virial && !V_dev) { CU(h, cudaMemcpyAsync(virial, stage + 1, 72, cudaMemcpyDeviceToHost, h->stream)); need_sync = true; }
-    if (F && !F_dev && N > 0) { CU(h, cudaMemcpyAsync(F, stage + 16, sizeof(double) * 3 * (size_t)N, cudaMemcpyDeviceToHost, h->stream)); need_sync = true; }
-    mk.mark(8);
-    if (need_sync) CU(h, cudaStreamSynchronize(h->stream));
+    OutPtrs o;
+    o.dE = E ? (E_dev ? E : stage) : stage;
+    o.dV = virial ? (V_dev ? virial : stage + 1) : nullptr;
+    o.dF = F ? (F_dev ? F : stage + 16) : nullptr;
+    o.E_host = E && !E_dev; o.F_host = F && !F_dev && N > 0; o.V_host = virial && !V_dev;
+
+    if (memcmp(box9, h->box_build, sizeof(double) * 9) != 0 && N > 0) RC(do_build(h, d_pos, box9));   // box changed
+
+    // One pass = the whole evaluation enqueued on the current list with NO host round trip in the middle: the skin
+    // criterion and the capacity of the compact-edge buffers are checked on the device, the kernels that follow
+    // return at once when either fails, and the host looks at the flag word after the evaluation (one stream
+    // synchronisation per call) and redoes the step after a rebuild / after growing the buffers. Systems whose
+    // kappa stash is held in chunks (config 5) need the chunk boundaries on the host and synchronise once more.
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        if (N == 0) {
+            std::vector<int64_t> ca{0, 0}, ce{0, 0};
+            RC(enqueue_layers(h, mk, o, virial != nullptr, ca, ce, false));
+            break;
+        }
+        const bool chunked = h->stash_chunks > 1 || h->cap_rc == 0;
+        int32_t flag = 0;
+        int64_t n_rc = 0;
+        if (!chunked) {
+            // ---------------- fast path: a CUDA graph of the steady-state launch sequence when every pointer is a
+            // device pointer (replayed while the list, the buffers and the caller's pointers stay the same) ----------------
+            const bool graphable = h->use_graph && !h->profiling && !o.E_host && !o.F_host && !o.V_host && pos == d_pos;
+            const reann::GraphKey key{d_pos, o.dE, o.dF, o.dV, h->n_rebuilds, h->cap_rc, h->stream};
+            if (graphable && h->gexec && memcmp(&key, &h->gkey, sizeof(key)) == 0) {
+                CU(h, cudaGraphLaunch(h->gexec, h->stream));
+                h->n_launches += h->g_kernels;
+            } else {
+                const bool capture = graphable;
+                const int64_t launches0 = h->n_launches;
+                if (capture) { graph_drop(h); CU(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal)); }
+                int rcode = enqueue_prep(h, d_pos);
+                const std::vector<int64_t> ca{0, N}, ce{0, INT64_MAX};   // one chunk: every edge (the count stays on the device)
+                if (rcode == REANN_OK) rcode = enqueue_layers(h, mk, o, virial != nullptr, ca, ce, true);
+                if (rcode == REANN_OK && cudaMemcpyAsync(h->h_flags, h->flags.p, 16, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+                    rcode = set_err(h, REANN_ERR_CUDA, "copy of the flag word failed");
+                if (capture) {
+                    cudaGraph_t g = nullptr;
+                    const cudaError_t e1 = cudaStreamEndCapture(h->stream, &g);
+                    if (rcode != REANN_OK) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return rcode; }
+                    if (e1 != cudaSuccess || !g) { cudaGetLastError(); return set_err(h, REANN_ERR_CUDA, "stream capture failed: %s", cudaGetErrorString(e1)); }
+                    const cudaError_t e2 = cudaGraphInstantiate(&h->gexec, g, 0);
+                    cudaGraphDestroy(g);
+                    if (e2 != cudaSuccess) { h->gexec = nullptr; cudaGetLastError(); return set_err(h, REANN_ERR_CUDA, "graph instantiation failed: %s", cudaGetErrorString(e2)); }
+                    h->gkey = key;
+                    h->g_kernels = h->n_launches - launches0;
+                    CU(h, cudaGraphLaunch(h->gexec, h->stream));
+                } else if (rcode != REANN_OK) return rcode;
+            }
+            if (o.E_host) CU(h, cudaMemcpyAsync(E, stage, 8, cudaMemcpyDeviceToHost, h->stream));
+            if (o.V_host) CU(h, cudaMemcpyAsync(virial, stage + 1, 72, cudaMemcpyDeviceToHost, h->stream));
+            if (o.F_host) CU(h, cudaMemcpyAsync(F, stage + 16, sizeof(double) * 3 * (size_t)N, cudaMemcpyDeviceToHost, h->stream));
+            mk.mark(8);
+            CU(h, cudaStreamSynchronize(h->stream));
+            flag = h->h_flags[0];
+            memcpy(&n_rc, h->h_flags + 2, 8);
+        } else {
+            // ---------------- chunked / first-call path: read the compact edge count and the chunk boundaries first ----------------
+            RC(enqueue_prep(h, d_pos));
+            CU(h, cudaMemcpyAsync(h->h_flags, h->flags.p, 16, cudaMemcpyDeviceToHost, h->stream));
+            CU(h, cudaStreamSynchronize(h->stream));
+            flag = h->h_flags[0];
+            memcpy(&n_rc, h->h_flags + 2, 8);
+            if (!(flag & FLAG_REBUILD)) {
+                RC(ensure_rc_capacity(h, n_rc));
+                flag &= ~FLAG_OVERFLOW;
+                const int C = h->stash_chunks;
+                std::vector<int64_t> ch_atom((size_t)C + 1, 0), ch_edge((size_t)C + 1, 0);
+                ch_atom[(size_t)C] = N; ch_edge[(size_t)C] = n_rc;
+                if (C > 1) {
+                    for (int c = 1; c < C; ++c) ch_atom[(size_t)c] = ((N * c / C) + 3) & ~(int64_t)3;
+                    for (int c = 1; c < C; ++c)
+                        CU(h, cudaMemcpyAsync(&ch_edge[(size_t)c], (const int64_t *)h->rc_ptr.p + ch_atom[(size_t)c], 8, cudaMemcpyDeviceToHost, h->stream));
+                    CU(h, cudaStreamSynchronize(h->stream));
+                    int64_t widest = 0;
+                    for (int c = 0; c < C; ++c) widest = std::max(widest, ch_edge[(size_t)c + 1] - ch_edge[(size_t)c]);
+                    RC(dev_ensure(h, h->kappa, sizeof(float) * (size_t)widest * md.nphip));
+                }
+                RC(enqueue_layers(h, mk, o, virial != nullptr, ch_atom, ch_edge, false));
+                if (o.E_host) CU(h, cudaMemcpyAsync(E, stage, 8, cudaMemcpyDeviceToHost, h->stream));
+                if (o.V_host) CU(h, cudaMemcpyAsync(virial, stage + 1, 72, cudaMemcpyDeviceToHost, h->stream));
+                if (o.F_host) CU(h, cudaMemcpyAsync(F, stage + 16, sizeof(double) * 3 * (size_t)N, cudaMemcpyDeviceToHost, h->stream));
+                mk.mark(8);
+                CU(h, cudaStreamSynchronize(h->stream));
+            }
+        }
+        if (flag & FLAG_REBUILD) { RC(do_build(h, d_pos, box9)); mk.m.clear(); mk.mark(1); continue; }   // A4: rebuild, redo
+        if (flag & FLAG_OVERFLOW) { RC(ensure_rc_capacity(h, n_rc)); graph_drop(h); mk.m.clear(); mk.mark(1); continue; }
+        h->E_rc = n_rc;
+        break;
+    }
     mk.finish();
     CU(h, cudaGetLastError());
     return REANN_OK;

@@ -79,7 +79,12 @@ struct ModelDims {
 struct LaunchCtx {
     cudaStream_t stream;
     int64_t *n_launches;
+    // device flag word: non-zero = this evaluation is void (the skin criterion asks for a rebuild, or the compact
+    // edge list outgrew its buffers); every kernel after the rc-filter count returns at once when it is set, the
+    // host reads it after the evaluation and redoes the step (api.cu). nullptr: no guard.
+    const int32_t *skip;
 };
+#define SKIP_GUARD(skip) do { if ((skip) != nullptr && *(skip) != 0) return; } while (0)
 #define LAUNCH(ctx, kernel, grid, block, smem, ...)                          \
     do {                                                                     \
         kernel<<<(grid), (block), (smem), (ctx).stream>>>(__VA_ARGS__);      \

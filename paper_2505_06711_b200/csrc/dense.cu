@@ -105,6 +105,7 @@ struct FwdArgs {
     float *z_stash;         // [N][zs], tile order
     float *out;             // rows of stride out_stride, atom order
     int out_stride, nqp, H1p, H2p, nout, zs;
+    const int32_t *skip;    // see LaunchCtx
 };
 
 // A chunk from row-major global rows -> K-major shared [KC][TM]
@@ -122,6 +123,7 @@ __device__ __forceinline__ void load_a_chunk(float *__restrict__ As, const float
 
 template <int NC1, int NC2>
 __global__ void __launch_bounds__(DT) k_dense_fwd(FwdArgs A) {
+    SKIP_GUARD(A.skip);
     extern __shared__ __align__(16) float sm[];
     const DenseTile tile = A.tiles[blockIdx.x];
     const DenseW W = A.w[tile.species];
@@ -188,10 +190,12 @@ struct BwdArgs {
     const float *z_stash, *outbar; // outbar == nullptr: energy layer, outbar = 1
     float *Qbar;                   // [N][nqp], tile order
     int outbar_stride, nqp, H1p, H2p, nout, zs;
+    const int32_t *skip;
 };
 
 template <int NC1, int NC2>
 __global__ void __launch_bounds__(DT) k_dense_bwd(BwdArgs A) {
+    SKIP_GUARD(A.skip);
     extern __shared__ __align__(16) float sm[];
     const DenseTile tile = A.tiles[blockIdx.x];
     const DenseW W = A.w[tile.species];
@@ -318,7 +322,7 @@ int launch_dense_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims 
     if (n_tiles <= 0) return REANN_OK;
     FwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.Q = Q; A.z_stash = z_stash; A.out = out;
-    A.out_stride = out_stride; A.nqp = md.nqp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs;
+    A.out_stride = out_stride; A.nqp = md.nqp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs; A.skip = ctx.skip;
     const size_t smem = sizeof(float) * ((size_t)KC * TM + KC * 128 + (size_t)TM * (A.H1p + A.H2p));
     NC_DISPATCH(run_fwd, ctx, A, n_tiles, smem)
 }
@@ -329,7 +333,7 @@ int launch_dense_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDims 
     if (n_tiles <= 0) return REANN_OK;
     BwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.z_stash = z_stash; A.outbar = outbar; A.Qbar = Qbar;
-    A.outbar_stride = outbar_stride; A.nqp = md.nqp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs;
+    A.outbar_stride = outbar_stride; A.nqp = md.nqp; A.H1p = ld.H1p; A.H2p = ld.H2p; A.nout = ld.nout; A.zs = zs; A.skip = ctx.skip;
     const size_t smem = sizeof(float) * ((size_t)TM * (A.H1p + A.H2p) + KC * 128 + TM * (A.nout + 1));
     NC_DISPATCH(run_bwd, ctx, A, n_tiles, smem)
 }

@@ -277,10 +277,12 @@ struct TcFwdArgs {
     float *z_stash;         // tile-quad layout, zs columns (z1 | z2)
     float *out;             // rows of stride out_stride, atom order
     int out_stride, K1, nout, zs, n_tiles, tf32;
+    const int32_t *skip;    // see LaunchCtx
 };
 
 template <int NCH1, int NCH2>
 __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
+    SKIP_GUARD(A.skip);
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ uint32_t tmem_base_s;
     constexpr int H1p = NCH1 * 32, H2p = NCH2 * 32, CW1 = H1p / 2, CW2 = H2p / 2;
@@ -472,10 +474,12 @@ struct TcBwdArgs {
     const float *z_stash, *outbar; // outbar == nullptr: energy layer (outbar = 1)
     float *Qbar;                   // tile-quad layout, K1 columns
     int outbar_stride, K1, nout, zs, n_tiles, tf32;
+    const int32_t *skip;
 };
 
 template <int NCH1, int NCH2>
 __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
+    SKIP_GUARD(A.skip);
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ uint32_t tmem_base_s;
     constexpr int H1p = NCH1 * 32, H2p = NCH2 * 32, CW1 = H1p / 2, CW2 = H2p / 2;
@@ -738,7 +742,7 @@ int launch_dense_tc_fwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDi
     if (ld.nout > 16) return REANN_ERR_UNSUPPORTED;
     TcFwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.Q = Q; A.z_stash = z_stash; A.out = out; A.out_stride = out_stride;
-    A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles; A.tf32 = tf32;
+    A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles; A.tf32 = tf32; A.skip = ctx.skip;
     TC_DISPATCH(run_tc_fwd, ctx, A, n_tiles)
 }
 
@@ -749,6 +753,6 @@ int launch_dense_tc_bwd(const LaunchCtx &ctx, const ModelDims &md, const LayerDi
     if (ld.nout > 16) return REANN_ERR_UNSUPPORTED;
     TcBwdArgs A;
     A.w = d_w; A.tiles = tiles; A.sp_list = sp_list; A.z_stash = z_stash; A.outbar = outbar; A.Qbar = Qbar;
-    A.outbar_stride = outbar_stride; A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles; A.tf32 = tf32;
+    A.outbar_stride = outbar_stride; A.K1 = md.K1; A.nout = ld.nout; A.zs = zs; A.n_tiles = n_tiles; A.tf32 = tf32; A.skip = ctx.skip;
     TC_DISPATCH(run_tc_bwd, ctx, A, n_tiles)
 }

@@ -101,7 +101,8 @@ __global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict_
                                                          double Ly, double Lz, const uint16_t *__restrict__ rank16,
                                                          const int64_t *__restrict__ rc_ptr,
                                                          uint32_t *__restrict__ col_rc, float4 *__restrict__ geom,
-                                                         uint32_t *__restrict__ rev_rc) {
+                                                         uint32_t *__restrict__ rev_rc, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     const int lane = threadIdx.x & 31;
     const int64_t i = (int64_t)blockIdx.x * EW + (threadIdx.x >> 5);
     if (i >= N) return;
@@ -146,7 +147,8 @@ __global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict_
 // ------------------------------------------------------------------------------------------ A8
 // c_ext[N+g][:] = c[owner[g]][:]  -- the paper's forward LA -> GA message.
 __global__ void k_ghost_gather(float *__restrict__ c_ext, const XRec *__restrict__ xrec, int64_t N, int64_t n_ext,
-                               int nphip) {
+                               int nphip, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     const int q4 = nphip >> 2;
     int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int64_t g = N + idx / q4;
@@ -181,7 +183,8 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
                                                       const uint32_t *__restrict__ col_rc,
                                                       const float4 *__restrict__ geom,
                                                       const float *__restrict__ c_ext, RadialTab rt,
-                                                      float *__restrict__ b) {
+                                                      float *__restrict__ b, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     using C = FwdCfg<NPHIP, NA, PN, PA>;
     extern __shared__ __align__(16) float smem_f[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -338,7 +341,8 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
                                                           const uint32_t *__restrict__ col_rc,
                                                           const float4 *__restrict__ geom,
                                                           const float *__restrict__ c_ext, RadialTab rt,
-                                                          float *__restrict__ b) {
+                                                          float *__restrict__ b, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     using C = FwdMma<NA>;
     constexpr int NAP = C::NAP, AT = C::AT, TS = C::TS;
     static_assert(NPHIP == 8 || NPHIP == 12 || NPHIP == 16, "mma.sync edge forward: N_phi padded to 8, 12 or 16");
@@ -451,7 +455,8 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
                                                       const float *__restrict__ c_ext, RadialTab rt, int S,
                                                       const float *__restrict__ bbar, int want_kappa,
                                                       float *__restrict__ kappa, float4 *__restrict__ gst,
-                                                      double *__restrict__ vir_part, AtomChunk ch) {
+                                                      double *__restrict__ vir_part, AtomChunk ch, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     constexpr int NB = NPHIP * NA;
     __shared__ __align__(16) float bb_s[EW][NB];
     __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
@@ -612,7 +617,8 @@ __global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t
                                                         const float *__restrict__ kappa,
                                                         const float4 *__restrict__ gst, int want_cbar,
                                                         float *__restrict__ cbar, double *__restrict__ Fc,
-                                                        StashChunk ch) {
+                                                        StashChunk ch, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     constexpr int PARTS = NPHIP / 4, EPS = 32 / PARTS; // float4 parts per edge, edges per warp step
     __shared__ float4 red_s[EW][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -665,7 +671,8 @@ __global__ void __launch_bounds__(OUT_TPB) k_output_a(int64_t N, const int32_t *
                                                       const double *__restrict__ Fc, const float *__restrict__ Ei,
                                                       double *__restrict__ F_out, double *__restrict__ Ei_caller,
                                                       const double *__restrict__ vir_part, int n_vir, int want_vir,
-                                                      double *__restrict__ partial) {
+                                                      double *__restrict__ partial, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     __shared__ double red[OUT_TPB];
     const int64_t i = (int64_t)blockIdx.x * OUT_TPB + threadIdx.x; // caller index
     double e = 0.0;
@@ -700,7 +707,8 @@ __global__ void __launch_bounds__(OUT_TPB) k_output_a(int64_t N, const int32_t *
     }
 }
 __global__ void __launch_bounds__(OUT_TPB) k_output_b(int n_part, const double *__restrict__ partial,
-                                                      double *__restrict__ E_out, double *__restrict__ vir_out) {
+                                                      double *__restrict__ E_out, double *__restrict__ vir_out, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     __shared__ double red[OUT_TPB];
     for (int q = 0; q < 10; ++q) {
         if (q > 0 && !vir_out) break;
@@ -751,18 +759,18 @@ void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *
 void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
                         const uint32_t *rev, int64_t N, double Lx, double Ly, double Lz, const uint16_t *rank16,
                         const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc) {
-    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, rev, N, Lx, Ly, Lz, rank16, rc_ptr, col_rc, geom, rev_rc);
+    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, rev, N, Lx, Ly, Lz, rank16, rc_ptr, col_rc, geom, rev_rc, ctx.skip);
 }
 void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip) {
     const int64_t work = (n_ext - N) * (nphip / 4);
-    if (work > 0) LAUNCH(ctx, k_ghost_gather, div_up(work, 256), 256, 0, c_ext, xrec, N, n_ext, nphip);
+    if (work > 0) LAUNCH(ctx, k_ghost_gather, div_up(work, 256), 256, 0, c_ext, xrec, N, n_ext, nphip, ctx.skip);
 }
 
 template <int NPHIP, int NA>
 static int run_edge_fwd_mma(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
                             const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
     using C = FwdMma<NA>;
-    LAUNCH(ctx, (k_edge_fwd_mma<NPHIP, NA>), div_up(N, EW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    LAUNCH(ctx, (k_edge_fwd_mma<NPHIP, NA>), div_up(N, EW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b, ctx.skip);
     return REANN_OK;
 }
 
@@ -779,7 +787,7 @@ static int run_edge_fwd(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, 
             return REANN_ERR_CUDA;
         attr_set[dev] = true;
     }
-    LAUNCH(ctx, (k_edge_fwd<NPHIP, NA, PN, PA>), div_up(N, (int64_t)EW * C::APW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b);
+    LAUNCH(ctx, (k_edge_fwd<NPHIP, NA, PN, PA>), div_up(N, (int64_t)EW * C::APW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b, ctx.skip);
     return REANN_OK;
 }
 
@@ -827,10 +835,10 @@ int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 #define M(NP, NA_, PN_, PA_)                                                                                      \
     if (vir_part)                                                                                                 \
         LAUNCH(ctx, (k_edge_bwd<NP, NA_, true>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,            \
-               md.S, bbar, want_kappa, kappa, gst, vir_part, ch);                                                 \
+               md.S, bbar, want_kappa, kappa, gst, vir_part, ch, ctx.skip);                                       \
     else                                                                                                          \
         LAUNCH(ctx, (k_edge_bwd<NP, NA_, false>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,           \
-               md.S, bbar, want_kappa, kappa, gst, vir_part, ch);                                                 \
+               md.S, bbar, want_kappa, kappa, gst, vir_part, ch, ctx.skip);                                       \
     return REANN_OK;
     EDGE_DISPATCH(M)
 #undef M
@@ -842,10 +850,10 @@ void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, c
     if (N <= 0) return;
     const StashChunk ch{e_lo, e_hi, do_forces, accumulate};
     switch (nphip) {
-        case 4: LAUNCH(ctx, k_rev_gather<4>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch); break;
-        case 8: LAUNCH(ctx, k_rev_gather<8>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch); break;
-        case 12: LAUNCH(ctx, k_rev_gather<12>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch); break;
-        default: LAUNCH(ctx, k_rev_gather<16>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch); break;
+        case 4: LAUNCH(ctx, k_rev_gather<4>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        case 8: LAUNCH(ctx, k_rev_gather<8>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        case 12: LAUNCH(ctx, k_rev_gather<12>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        default: LAUNCH(ctx, k_rev_gather<16>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
     }
 }
 
@@ -853,8 +861,8 @@ void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, con
                    const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
                    double *Ei_caller, double *scratch) {
     const int nb = (int)div_up(N > 0 ? N : 1, OUT_TPB);
-    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, vir_part, n_vir_blocks, vir_out != nullptr, scratch);
-    LAUNCH(ctx, k_output_b, 1, OUT_TPB, 0, nb, (const double *)scratch, E_out, vir_out);
+    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, vir_part, n_vir_blocks, vir_out != nullptr, scratch, ctx.skip);
+    LAUNCH(ctx, k_output_b, 1, OUT_TPB, 0, nb, (const double *)scratch, E_out, vir_out, ctx.skip);
 }
 
 void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,

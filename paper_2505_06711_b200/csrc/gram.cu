@@ -72,7 +72,8 @@ template <int NPHIP, int NA>
 __global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *__restrict__ sp_list,
                                                       const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, float *__restrict__ Q, int nphi,
-                                                      int npairs, int NPp, int KQ) {
+                                                      int npairs, int NPp, int KQ, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     constexpr int NB = NPHIP * NA, LMAX = l_of(NA - 1);
     extern __shared__ __align__(16) float sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, QS = KQ + 4;
@@ -152,7 +153,8 @@ template <int NPHIP, int NA>
 __global__ void __launch_bounds__(GW * 32, 4) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
                                                       const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, const float *__restrict__ Qbar,
-                                                      float *__restrict__ bbar, int nphi, int NPp, int KQ) {
+                                                      float *__restrict__ bbar, int nphi, int NPp, int KQ, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
     using C = BwdCfg<NPHIP, NA>;
     constexpr int NB = NPHIP * NA;
     extern __shared__ __align__(16) float sm[];
@@ -256,7 +258,7 @@ int run_gram_fwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int
     static size_t attr = 48 * 1024;
     if (int rc = set_smem(k_gram_fwd<NPHIP, NA>, smem, attr)) return rc;
     const unsigned grid = tiles ? (unsigned)n_tiles * 16u : div_up(N, GW);
-    LAUNCH(ctx, (k_gram_fwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Q, md.nphi, md.npairs, md.NPp, KQ);
+    LAUNCH(ctx, (k_gram_fwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Q, md.nphi, md.npairs, md.NPp, KQ, ctx.skip);
     return REANN_OK;
 }
 template <int NPHIP, int NA>
@@ -268,7 +270,7 @@ int run_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int
     static size_t attr = 48 * 1024;
     if (int rc = set_smem(k_gram_bwd<NPHIP, NA>, smem, attr)) return rc;
     const unsigned grid = tiles ? (unsigned)n_tiles * 16u : div_up(N, GW);
-    LAUNCH(ctx, (k_gram_bwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Qbar, bbar, md.nphi, md.NPp, KQ);
+    LAUNCH(ctx, (k_gram_bwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Qbar, bbar, md.nphi, md.NPp, KQ, ctx.skip);
     return REANN_OK;
 }
 

@@ -6,7 +6,14 @@ struct reann {
     ModelDims md{};
     LayerDims ld[REANN_MAX_T]{};
     int64_t N = 0;
-    cudaStream_t stream = nullptr;
+    cudaStream_t stream = nullptr;      // the stream every kernel of the handle runs on (never the legacy default stream)
+    cudaStream_t own_stream = nullptr;  // used while the caller has set no stream of their own
+    // CUDA graph of the steady-state evaluation (api.cu): replayed while this key stays the same
+    struct GraphKey { const void *pos, *E, *F, *V; int64_t n_rebuilds, cap_rc; cudaStream_t stream; };
+    cudaGraphExec_t gexec = nullptr;
+    GraphKey gkey{};
+    int64_t g_kernels = 0;
+    bool use_graph = true;              // REANN_GRAPH=0 switches the graph off
     int64_t n_launches = 0;
     std::string err;
 
@@ -81,7 +88,7 @@ struct reann {
     std::vector<cudaEvent_t> ev;  // event pool
     size_t bytes_device = 0;
 
-    LaunchCtx ctx() { return LaunchCtx{stream, &n_launches}; }
+    LaunchCtx ctx() { return LaunchCtx{stream, &n_launches, nullptr}; }
 };
 
 // api.cu helpers used by neighbor.cu
