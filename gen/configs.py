@@ -32,6 +32,10 @@ CONFIGS = {
             L=3, n_gauss=16, H=(128, 128), nbar=90.7),
     4: dict(name="fcc-4M", kind="fcc", ncell=100, a=3.61, sigma=0.1, rc=5.0, skin=1.0, T=3, L=2,
             n_gauss=12, H=(64, 64), nbar=44.7),
+    # NEXT-4 of SURVEY.md 8(f): multi-element solid, the shape of the paper's HEA workload (Fig. 7b: 576
+    # atoms per GPU; :116: five elements): fcc with `S` randomly assigned species
+    6: dict(name="hea-fcc", kind="hea", ncell=6, a=3.6, sigma=0.08, S=5, rc=6.0, skin=1.0, T=2, L=2, n_gauss=8,
+            H=(64, 64), nbar=78.0),
     5: dict(name="water-slab-10M", kind="slab", n_mol=3333333, box=463.7, gap=30.0, rc=6.0, skin=2.0,
             T=3, L=2, n_gauss=16, H=(128, 128), nbar=90.7),
 }
@@ -109,7 +113,8 @@ def _calib_table() -> dict:
 
 
 def make_config(k: int, T: int | None = None, n_mol: int | None = None, ncell: int | None = None,
-                geometry_only: bool = False, gains: dict | None = None, radial_jitter: float = 0.0) -> dict:
+                geometry_only: bool = False, gains: dict | None = None, radial_jitter: float = 0.0,
+                n_species: int | None = None) -> dict:
     """Build config k. Overrides (T, n_mol, ncell) give same-density replicas / the T sweep.
 
     radial_jitter > 0 (tests only): per-(layer, species) radial tables, see make_weights.
@@ -141,7 +146,9 @@ def make_config(k: int, T: int | None = None, n_mol: int | None = None, ncell: i
         nc = ncell if ncell is not None else r["ncell"]
         pos, species = fcc_lattice(nc, r["a"], r["sigma"], seed_g)
         box = np.array([nc * r["a"]] * 3)
-        S = 1
+        S = int(r.get("S", 1)) if n_species is None else int(n_species)
+        if S > 1:
+            species = np.random.default_rng(seed_g + 500).integers(0, S, len(pos)).astype(np.int32)
         masses = np.full(len(pos), MASS["M"])
     out = dict(k=k, name=r["name"], pos=pos, species=species, box=np.diag(box).reshape(9).copy(),
                masses=masses, rc=r["rc"], skin=r["skin"], T=r["T"], L=r["L"], n_gauss=r["n_gauss"],

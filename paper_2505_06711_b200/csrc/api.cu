@@ -142,7 +142,7 @@ extern "C" int reann_create(reann_t **out, const void *weights, size_t weights_b
         cudaGetLastError();
         return set_err(nullptr, REANN_ERR_CUDA, "no CUDA device: this library has no CPU path");
     }
-    if (n_atoms >= ((int64_t)1 << 28)) return set_err(nullptr, REANN_ERR_UNSUPPORTED, "n_atoms >= 2^28");
+    if (n_atoms >= ((int64_t)1 << COL_SPECIES_SHIFT)) return set_err(nullptr, REANN_ERR_UNSUPPORTED, "n_atoms >= 2^27");
     // bring blob and species to the host
     std::vector<unsigned char> blob(weights_bytes);
     if (is_device_ptr(weights)) {

@@ -12,7 +12,7 @@
 
 #include "../../include/reann.h"
 
-#define REANN_MAX_S 16
+#define REANN_MAX_S 32
 #define REANN_MAX_T 8
 #define REANN_MAX_NA 20
 #define REANN_MAX_NPHI 16
@@ -33,9 +33,9 @@ static_assert(sizeof(XRec) == 32, "XRec must be 32 bytes");
 // shift code 0..26 = (sx+1)*9 + (sy+1)*3 + (sz+1); 13 = no shift; reverse code = 26 - code
 __host__ __device__ inline int shift_code(int sx, int sy, int sz) { return (sx + 1) * 9 + (sy + 1) * 3 + (sz + 1); }
 
-// col_rc entries carry the neighbour's species in the top 4 bits (N_ext < 2^28)
-#define COL_IDX_MASK 0x0FFFFFFFu
-#define COL_SPECIES_SHIFT 28
+// col_rc entries carry the neighbour's species in the top 5 bits (S <= 32, N_ext < 2^27)
+#define COL_IDX_MASK 0x07FFFFFFu
+#define COL_SPECIES_SHIFT 27
 
 struct DevBuf {
     void *p = nullptr;

@@ -364,7 +364,7 @@ int neighbor_build(reann *h, const double *d_pos) {
     CU(h, cudaMemcpyAsync(&G, goff + N, sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
     CU(h, cudaStreamSynchronize(h->stream));
     if (N + G >= ((int64_t)1 << COL_SPECIES_SHIFT))
-        return set_err(h, REANN_ERR_UNSUPPORTED, "N_ext = %lld exceeds 2^28", (long long)(N + G));
+        return set_err(h, REANN_ERR_UNSUPPORTED, "N_ext = %lld exceeds 2^27", (long long)(N + G));
     {   // grow xrec preserving the local records
         size_t need = sizeof(XRec) * (size_t)(N + G);
         if (h->xrec.bytes < need) {

@@ -78,7 +78,8 @@ def test_neighbor_pair_sets_exact(R, case):
 
 # ------------------------------------------------------------------ energy / forces / virial
 @pytest.mark.parametrize("case", ["cfg0", "cfg0j", "cfg1", "cfg2", "cfg2j", "cfg3r", "cfg3rj", "cfg4r_T1", "cfg4r_T3",
-                                  "cfg4r_T6", "cfg5r", "small_L3", "small_L0", "small_L1_S1", "small_n4", "small_n12"])
+                                  "cfg4r_T6", "cfg5r", "hea5", "hea25", "small_L3", "small_L0", "small_L1_S1", "small_n4",
+                                  "small_n12"])
 def test_energy_forces_virial_parity(R, case):
     """`j` cases: radial tables that differ per (layer, neighbour species) -- with identical rows (the BASELINE
     recipe) an indexing mistake in the edge kernels (s_j -> s_i, t -> 0) would be invisible."""
@@ -89,6 +90,8 @@ def test_energy_forces_virial_parity(R, case):
     elif case == "cfg3r": cfg = gen.make_config(3, n_mol=700)         # L=3, 16 Gaussians, ragged tiles
     elif case.startswith("cfg4r"): cfg = gen.make_config(4, ncell=7, T=int(case[-1]))
     elif case == "cfg5r": cfg = gen.make_config(5, n_mol=900)
+    elif case == "hea5": cfg = jitter_cfg(6, 0.1)                          # 5 elements, 864 atoms
+    elif case == "hea25": cfg = jitter_cfg(6, 0.1, n_species=25)           # 25 elements: ragged per-species tiles
     elif case == "small_L3": cfg = small_cfg()
     elif case == "small_L0": cfg = small_cfg(L=0, n_gauss=8, T=2)
     elif case == "small_L1_S1": cfg = small_cfg(L=1, S=1, n_gauss=16, T=2, H=(64, 32), Hc=(16, 128))
@@ -400,6 +403,37 @@ def test_non_default_kernel_variants_parity(env):
                        timeout=600)
     assert r.returncode == 0, r.stdout + r.stderr
     assert r.stdout.count("[parity] variant") == 2
+
+
+def test_cost_is_linear_in_T(R):
+    """PAPER.md:49, :88 (Fig. 5): one neighbour list reused by every layer makes the cost per step linear in T.
+    Config 4 geometry on a 40^3-cell replica (256 000 atoms), T = 1...6: device time of reann_energy_forces
+    (median of 5, CUDA events, no rebuild), least-squares line a + b T; the largest residual must stay below 3 %
+    of the slope b (full-size sweep: profiles/r02_config4_Tsweep.md)."""
+    import torch
+    ms = []
+    for T in range(1, 7):
+        cfg = gen.make_config(4, ncell=40, T=T)
+        m = R.Reann.from_config(cfg)
+        pos = torch.tensor(cfg["pos"], device="cuda")
+        E = torch.zeros(1, dtype=torch.float64, device="cuda"); F = torch.zeros((m.n, 3), dtype=torch.float64, device="cuda")
+        m.build_neighbors(pos, cfg["box"])
+        for _ in range(3):
+            m.energy_forces(pos, cfg["box"], E, F)
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); e0.record()
+            m.energy_forces(pos, cfg["box"], E, F)
+            e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ms.append(sorted(ts)[2])
+        m.close()
+    T = np.arange(1, 7, dtype=float)
+    b, a = np.polyfit(T, np.array(ms), 1)
+    res = np.abs(np.array(ms) - (a + b * T)).max()
+    print(f"[T sweep] ms = {[round(x, 3) for x in ms]}  fit {a:.3f} + {b:.3f} T  max residual {res:.4f} ms = {100 * res / b:.2f} % of the slope")
+    assert b > 0 and res <= 0.03 * b
 
 
 def test_fast_mlp_mode_tf32_restated_tolerance():
