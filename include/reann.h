@@ -135,6 +135,36 @@ int reann_set_stream(reann_t *h, void *cuda_stream);    /* e.g. torch.cuda.curre
 int reann_get_atomic_energies(reann_t *h, double *Ei);
 
 /*
+ * ---- One rank of a spatially decomposed run (the paper's scheme, Fig. 3-4; groundwork for NEXT-1) ----
+ * The handle is created over the rank's local atoms (LAs) AND copies of the other ranks' atoms that lie within
+ * rc + skin of its domain (ghost atoms, GAs); reann_set_halo flags the GAs (HOST array [n_atoms], 1 = GA; NULL
+ * clears). GAs serve as neighbours only: their E_i is not counted, they are not centres of edges on this rank
+ * ("local parts computed in place"). One evaluation, driven by the caller, all ranks in lock step:
+ *   reann_step_begin(pos, box, want_virial)      skin check / rebuild, compact edge list, c^0
+ *   for t = 0 .. T-1:                             forward (Fig. 4a)
+ *     [t >= 1] reann_coeff_set(t, GAs, rows)      c^t of the GAs, received from their owners (reann_coeff_get there)
+ *     reann_step_forward(t)                       rho^t and c^{t+1} (or E_i) of the LAs
+ *   for t = T-1 .. 0:                             reverse (Fig. 4b; vector-Jacobian products)
+ *     [t < T-1] reann_cbar_add(LAs, rows)         dE/dc^{t+1} contributions received from the ranks that hold the
+ *                                                 atom as a GA (reann_cbar_get there, after their step_backward(t+1))
+ *     reann_step_backward(t)                      this rank's edges: dE/dc^t rows (t >= 1), forces accumulate
+ *   reann_step_end(E, F, virial)                  E = sum over LAs; F[n_atoms][3]: the rows of GAs are this rank's
+ *                                                 contributions to forces on other ranks' atoms (to be sent and added
+ *                                                 there, Eq. 3); virial = this rank's edges
+ * Row arrays are HOST float arrays [n][n_gauss]; idx are caller indices (HOST int64, unique within a call).
+ * Every call synchronises the stream. Not available while the per-edge stash is held in chunks.
+ */
+int reann_set_halo(reann_t *h, const uint8_t *is_halo);
+int reann_step_begin(reann_t *h, const double *pos, const double *box9, int want_virial);
+int reann_step_forward(reann_t *h, int t);
+int reann_coeff_get(reann_t *h, int t, int64_t n, const int64_t *idx, float *out);
+int reann_coeff_set(reann_t *h, int t, int64_t n, const int64_t *idx, const float *in);
+int reann_step_backward(reann_t *h, int t);
+int reann_cbar_get(reann_t *h, int64_t n, const int64_t *idx, float *out);
+int reann_cbar_add(reann_t *h, int64_t n, const int64_t *idx, const float *in);
+int reann_step_end(reann_t *h, double *E, double *F, double *virial);
+
+/*
  * Harness support, outside the energy/force path: one velocity-Verlet step on device arrays
  * (all DEVICE pointers, caller order): v += dt/2 * F * acc_unit / m ; x += dt * v  (kick_drift),
  * or only the half kick. inv_mass[n_atoms] in 1/amu, acc_unit converts eV/(A amu) to A/fs^2.

@@ -22,7 +22,8 @@ REANN_OK, REANN_ERR_ARG, REANN_ERR_WEIGHTS, REANN_ERR_BOX, REANN_ERR_NO_NEIGHBOR
 
 EXPORTS = ["reann_create", "reann_build_neighbors", "reann_energy_forces", "reann_destroy", "reann_last_error",
            "reann_get_neighbors", "reann_get_neighbor_rows", "reann_get_stats", "reann_set_profiling", "reann_set_stream",
-           "reann_get_atomic_energies", "reann_verlet"]
+           "reann_get_atomic_energies", "reann_verlet", "reann_set_halo", "reann_step_begin", "reann_step_forward",
+           "reann_coeff_get", "reann_coeff_set", "reann_step_backward", "reann_cbar_get", "reann_cbar_add", "reann_step_end"]
 
 
 class ReannError(RuntimeError):
@@ -77,6 +78,13 @@ def lib() -> ctypes.CDLL:
         L.reann_set_stream.argtypes = [vp, vp]
         L.reann_get_atomic_energies.restype = ctypes.c_int
         L.reann_get_atomic_energies.argtypes = [vp, vp]
+        for name, args in (("reann_set_halo", [vp, vp]), ("reann_step_begin", [vp, vp, vp, ctypes.c_int]),
+                           ("reann_step_forward", [vp, ctypes.c_int]), ("reann_coeff_get", [vp, ctypes.c_int, i64, vp, vp]),
+                           ("reann_coeff_set", [vp, ctypes.c_int, i64, vp, vp]), ("reann_step_backward", [vp, ctypes.c_int]),
+                           ("reann_cbar_get", [vp, i64, vp, vp]), ("reann_cbar_add", [vp, i64, vp, vp]),
+                           ("reann_step_end", [vp, vp, vp, vp])):
+            getattr(L, name).restype = ctypes.c_int
+            getattr(L, name).argtypes = args
         L.reann_verlet.restype = ctypes.c_int
         L.reann_verlet.argtypes = [vp, vp, vp, vp, vp, dbl, dbl, ctypes.c_int]
         _lib = L
@@ -177,6 +185,7 @@ class Reann:
     def __init__(self, weights: bytes, species, rc, skin, T, L, n_gauss):
         self.species = np.ascontiguousarray(species, dtype=np.int32)
         self.n = int(self.species.shape[0])
+        self.n_gauss = int(n_gauss)
         self.h = reann_create(weights, self.species, rc, skin, T, L, n_gauss)
 
     @classmethod
@@ -214,6 +223,37 @@ class Reann:
 
     def set_stream(self, stream_ptr: int):
         _check(self.h, lib().reann_set_stream(self.h, ctypes.c_void_p(stream_ptr)))
+
+    # ---- one rank of a decomposed run (include/reann.h, reann_step_*; driver: decomp.energy_forces_decomposed) ----
+    def set_halo(self, is_halo):
+        a = None if is_halo is None else np.ascontiguousarray(is_halo, dtype=np.uint8)
+        _check(self.h, lib().reann_set_halo(self.h, _ptr(a)))
+
+    def step_begin(self, pos, box, want_virial=True):
+        _check(self.h, lib().reann_step_begin(self.h, _ptr(pos, np.float64), _ptr(_box(box)), int(want_virial)))
+
+    def step_forward(self, t: int):
+        _check(self.h, lib().reann_step_forward(self.h, int(t)))
+
+    def step_backward(self, t: int):
+        _check(self.h, lib().reann_step_backward(self.h, int(t)))
+
+    def _rows(self, fn, idx, rows=None, t=None):
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        out = np.zeros((len(idx), self.n_gauss), dtype=np.float32) if rows is None else np.ascontiguousarray(rows, dtype=np.float32)
+        args = (self.h,) + (() if t is None else (int(t),)) + (len(idx), _ptr(idx), _ptr(out))
+        _check(self.h, fn(*args))
+        return out
+
+    def coeff_get(self, t, idx): return self._rows(lib().reann_coeff_get, idx, None, t)
+    def coeff_set(self, t, idx, rows): self._rows(lib().reann_coeff_set, idx, rows, t)
+    def cbar_get(self, idx): return self._rows(lib().reann_cbar_get, idx)
+    def cbar_add(self, idx, rows): self._rows(lib().reann_cbar_add, idx, rows)
+
+    def step_end(self, want_virial=True):
+        E = np.zeros(1); F = np.zeros((self.n, 3)); vir = np.zeros(9) if want_virial else None
+        _check(self.h, lib().reann_step_end(self.h, _ptr(E), _ptr(F), _ptr(vir)))
+        return float(E[0]), F, (vir.reshape(3, 3) if want_virial else None)
 
     def verlet(self, pos, vel, F, inv_mass, dt, acc_unit, drift: bool):
         _check(self.h, lib().reann_verlet(self.h, _ptr(pos), _ptr(vel), _ptr(F), _ptr(inv_mass), float(dt),

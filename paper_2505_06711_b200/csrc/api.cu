@@ -356,7 +356,8 @@ extern "C" void reann_destroy(reann_t *h) {
                       &h->cell_rank, &h->row_ptr, &h->col, &h->rev, &h->sp_list, &h->scratch_a, &h->scratch_b,
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
                       &h->geom, &h->rev_rc, &h->c_ext, &h->b, &h->z_stash, &h->bbar, &h->cbar, &h->kappa, &h->gst,
-                      &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch, &h->Qbuf};
+                      &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch, &h->Qbuf,
+                      &h->halo_caller, &h->xch_idx, &h->xch_val};
     for (DevBuf *b : bufs) dev_free(h, *b);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
@@ -544,88 +545,141 @@ struct OutPtrs {      // where the kernels write (device), and what has to be co
     bool E_host, F_host, V_host;
 };
 
+// ---- the pieces of one evaluation (used by reann_energy_forces and by the layer-by-layer calls of a decomposed run) ----
+struct LayerPtrs {
+    size_t cstride, bstride, zstride;
+    float *c_ext, *b, *zst;
+    const DenseW *wtab;
+    const DenseWT *wttab;
+    const DenseTile *gram_tiles;
+};
+static LayerPtrs layer_ptrs(reann *h) {
+    const ModelDims &md = h->md;
+    LayerPtrs p;
+    p.cstride = (size_t)h->n_ext * md.nphip; p.bstride = (size_t)h->N * md.NB;
+    p.zstride = (h->dense_tc ? (size_t)h->n_tiles * DENSE_TC_TM : (size_t)h->N) * h->zs;
+    p.c_ext = (float *)h->c_ext.p; p.b = (float *)h->b.p; p.zst = (float *)h->z_stash.p;
+    p.wtab = (const DenseW *)h->w_tab.p; p.wttab = (const DenseWT *)h->wt_tab.p;
+    p.gram_tiles = h->dense_tc ? (const DenseTile *)h->tiles.p : nullptr;
+    return p;
+}
+
+static void enqueue_filter_fill(reann *h, const LaunchCtx &ctx) {
+    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
+    launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
+                       (const uint32_t *)h->rev.p, h->N, Lx, Ly, Lz, (const uint16_t *)h->rank16.p,
+                       (const int64_t *)h->rc_ptr.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
+}
+
+// layer t of the forward pass (Eq. 1, Eq. 2): b^t, rho^t (radial-pair form), c^{t+1} of the local atoms or E_i
+static int enqueue_forward_layer(reann *h, const LaunchCtx &ctx, Marks &mk, int t) {
+    const ModelDims &md = h->md;
+    const int64_t N = h->N;
+    const LayerPtrs p = layer_ptrs(h);
+    mk.mark(2);
+    int rcode = launch_edge_fwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
+                                (const float4 *)h->geom.p, p.c_ext + t * p.cstride, (const float *)h->rcen.p,
+                                (const float *)h->alpha.p, p.b + t * p.bstride, h->edge_fwd_mma);
+    if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
+    mk.mark(3);
+    const bool last = t == md.T - 1;
+    launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, p.gram_tiles, h->n_tiles, p.b + t * p.bstride, (float *)h->Qbuf.p);
+    rcode = h->dense_tc
+                ? launch_dense_tc_fwd(ctx, md, h->ld[t], p.wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                      (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, p.zst + t * p.zstride, h->zs,
+                                      last ? (float *)h->Ei.p : p.c_ext + (t + 1) * p.cstride, last ? 1 : md.nphip, h->mlp_tf32)
+                : launch_dense_fwd(ctx, md, h->ld[t], p.wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                   (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, p.zst + t * p.zstride, h->zs,
+                                   last ? (float *)h->Ei.p : p.c_ext + (t + 1) * p.cstride, last ? 1 : md.nphip);
+    if (rcode) return set_err(h, rcode, "dense forward: unsupported MLP shape or shared-memory size");
+    return REANN_OK;
+}
+// the forward LA -> GA message of layer t for the periodic images held by this handle
+static void enqueue_image_gather(reann *h, const LaunchCtx &ctx, Marks &mk, int t) {
+    const LayerPtrs p = layer_ptrs(h);
+    mk.mark(4);
+    launch_ghost_gather(ctx, p.c_ext + t * p.cstride, (const XRec *)h->xrec.p, h->N, h->n_ext, h->md.nphip);
+}
+
+__global__ void k_zero_halo_rows(float *__restrict__ bbar, int nb, int64_t N, const int32_t *__restrict__ perm,
+                                 const uint8_t *__restrict__ halo_caller) {
+    const int64_t k = blockIdx.x;                       // internal atom index
+    if (k >= N || !halo_caller[perm[k]]) return;
+    for (int q = threadIdx.x; q < nb; q += blockDim.x) bbar[k * nb + q] = 0.f;
+}
+
+// layer t of the reverse pass (Eqs. 3-5): bbar^t from dE/dc^{t+1} (or from E_i), per-edge g_e / kappa_e, reverse gather
+static int enqueue_backward_layer(reann *h, const LaunchCtx &ctx, Marks &mk, int t, bool want_vir,
+                                  const std::vector<int64_t> &ch_atom, const std::vector<int64_t> &ch_edge) {
+    const ModelDims &md = h->md;
+    const int64_t N = h->N;
+    const LayerPtrs p = layer_ptrs(h);
+    const int C = (int)ch_atom.size() - 1;
+    mk.mark(5);
+    const bool last = t == md.T - 1;
+    int rcode = h->dense_tc
+                    ? launch_dense_tc_bwd(ctx, md, h->ld[t], p.wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                          (const int32_t *)h->sp_list.p, p.zst + t * p.zstride, h->zs,
+                                          last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p, h->mlp_tf32)
+                    : launch_dense_bwd(ctx, md, h->ld[t], p.wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
+                                       (const int32_t *)h->sp_list.p, p.zst + t * p.zstride, h->zs,
+                                       last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);
+    if (rcode) return set_err(h, rcode, "dense backward: unsupported MLP shape or shared-memory size");
+    launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, p.gram_tiles, h->n_tiles, p.b + t * p.bstride, (const float *)h->Qbuf.p,
+                    (float *)h->bbar.p);
+    // ghost atoms of a decomposed run are not centres on this rank: their rows of bbar are zero (their edges belong
+    // to the owning rank, "local parts computed in place")
+    if (h->have_halo && N > 0)
+        LAUNCH(ctx, k_zero_halo_rows, (unsigned)N, 64, 0, (float *)h->bbar.p, md.NB, N, (const int32_t *)h->perm.p,
+               (const uint8_t *)h->halo_caller.p);
+    mk.mark(6);
+    for (int c = 0; c < C; ++c) {
+        if (c > 0) mk.mark(6);
+        rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
+                                (const float4 *)h->geom.p, p.c_ext + t * p.cstride, (const float *)h->rcen.p,
+                                (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
+                                (float4 *)h->gst.p, want_vir ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
+                                ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
+        if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
+        mk.mark(t >= 1 ? 7 : 9);
+        // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after
+        if (t >= 1 || c == C - 1)
+            launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
+                              (const float4 *)h->gst.p, md.nphip, t >= 1, (float *)h->cbar.p, (double *)h->Fc.p,
+                              ch_edge[(size_t)c], ch_edge[(size_t)c + 1], c == C - 1, c > 0);
+    }
+    return REANN_OK;
+}
+
+static int enqueue_zero_accumulators(reann *h) {
+    if (h->N > 0) {
+        CU(h, cudaMemsetAsync(h->Fc.p, 0, sizeof(double) * 3 * (size_t)h->N, h->stream));
+        CU(h, cudaMemsetAsync(h->vir_part.p, 0, sizeof(double) * 9 * (size_t)h->n_vir_blocks, h->stream));
+    }
+    return REANN_OK;
+}
+
+static void enqueue_output(reann *h, const LaunchCtx &ctx, Marks &mk, const OutPtrs &o) {
+    mk.mark(8);
+    launch_output(ctx, h->N, (const int32_t *)h->inv_perm.p, (const double *)h->Fc.p, (const float *)h->Ei.p,
+                  (const double *)h->vir_part.p, h->N > 0 ? h->n_vir_blocks : 0, o.dE, o.dF, o.dV, (double *)h->Ei_caller.p,
+                  (double *)h->red_scratch.p, h->have_halo ? (const uint8_t *)h->halo_caller.p : nullptr);
+}
+
 // everything after the prep: compact list, T forward layers, reverse pass, outputs. ch_atom / ch_edge: stash chunks.
 static int enqueue_layers(reann *h, Marks &mk, const OutPtrs &o, bool want_vir, const std::vector<int64_t> &ch_atom,
                           const std::vector<int64_t> &ch_edge, bool guarded) {
     const ModelDims &md = h->md;
-    const int64_t N = h->N;
     LaunchCtx ctx = h->ctx();
     if (guarded) ctx.skip = (const int32_t *)h->flags.p;
-    const int C = (int)ch_atom.size() - 1;
-    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
-    launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
-                       (const uint32_t *)h->rev.p, N, Lx, Ly, Lz, (const uint16_t *)h->rank16.p,
-                       (const int64_t *)h->rc_ptr.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
-
-    // ---- forward: T layers (Eq. 1, Eq. 2) ----
-    const size_t cstride = (size_t)h->n_ext * md.nphip, bstride = (size_t)N * md.NB, zstride = (h->dense_tc ? (size_t)h->n_tiles * DENSE_TC_TM : (size_t)N) * h->zs;
-    float *c_ext = (float *)h->c_ext.p, *b = (float *)h->b.p, *zst = (float *)h->z_stash.p;
-    const DenseW *wtab = (const DenseW *)h->w_tab.p;
-    const DenseWT *wttab = (const DenseWT *)h->wt_tab.p;
-    const DenseTile *gram_tiles = h->dense_tc ? (const DenseTile *)h->tiles.p : nullptr;
+    enqueue_filter_fill(h, ctx);
     for (int t = 0; t < md.T; ++t) {
-        mk.mark(2);
-        int rcode = launch_edge_fwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
-                                    (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
-                                    (const float *)h->alpha.p, b + t * bstride, h->edge_fwd_mma);
-        if (rcode) return set_err(h, rcode, "edge forward: unsupported (n_gauss, L) combination");
-        mk.mark(3);
-        const bool last = t == md.T - 1;
-        launch_gram_fwd(ctx, md, N, (const int32_t *)h->sp_list.p, gram_tiles, h->n_tiles, b + t * bstride,
-                        (float *)h->Qbuf.p);
-        rcode = h->dense_tc
-                    ? launch_dense_tc_fwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                          (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
-                                          last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip, h->mlp_tf32)
-                    : launch_dense_fwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                       (const int32_t *)h->sp_list.p, (const float *)h->Qbuf.p, zst + t * zstride, h->zs,
-                                       last ? (float *)h->Ei.p : c_ext + (t + 1) * cstride, last ? 1 : md.nphip);
-        if (rcode) return set_err(h, rcode, "dense forward: unsupported MLP shape or shared-memory size");
-        if (!last) {
-            mk.mark(4);
-            launch_ghost_gather(ctx, c_ext + (t + 1) * cstride, (const XRec *)h->xrec.p, N, h->n_ext, md.nphip);
-        }
+        RC(enqueue_forward_layer(h, ctx, mk, t));
+        if (t + 1 < md.T) enqueue_image_gather(h, ctx, mk, t + 1);
     }
-    // ---- reverse: T layers (Eqs. 3-5) ----
-    if (N > 0) {
-        CU(h, cudaMemsetAsync(h->Fc.p, 0, sizeof(double) * 3 * (size_t)N, h->stream));
-        CU(h, cudaMemsetAsync(h->vir_part.p, 0, sizeof(double) * 9 * (size_t)h->n_vir_blocks, h->stream));
-    }
-    for (int t = md.T - 1; t >= 0; --t) {
-        mk.mark(5);
-        const bool last = t == md.T - 1;
-        int rcode = h->dense_tc
-                        ? launch_dense_tc_bwd(ctx, md, h->ld[t], wttab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                              (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
-                                              last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p, h->mlp_tf32)
-                        : launch_dense_bwd(ctx, md, h->ld[t], wtab + (size_t)t * md.S, (const DenseTile *)h->tiles.p, h->n_tiles,
-                                           (const int32_t *)h->sp_list.p, zst + t * zstride, h->zs,
-                                           last ? nullptr : (const float *)h->cbar.p, md.nphip, (float *)h->Qbuf.p);
-        if (rcode) return set_err(h, rcode, "dense backward: unsupported MLP shape or shared-memory size");
-        launch_gram_bwd(ctx, md, N, (const int32_t *)h->sp_list.p, gram_tiles, h->n_tiles, b + t * bstride, (const float *)h->Qbuf.p,
-                        (float *)h->bbar.p);
-        mk.mark(6);
-        for (int c = 0; c < C; ++c) {
-            if (c > 0) mk.mark(6);
-            rcode = launch_edge_bwd(ctx, md, t, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->col_rc.p,
-                                    (const float4 *)h->geom.p, c_ext + t * cstride, (const float *)h->rcen.p,
-                                    (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
-                                    (float4 *)h->gst.p, want_vir ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
-                                    ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
-            if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
-            mk.mark(t >= 1 ? 7 : 9);
-            // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after
-            if (t >= 1 || c == C - 1)
-                launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
-                                  (const float4 *)h->gst.p, md.nphip, t >= 1, (float *)h->cbar.p, (double *)h->Fc.p,
-                                  ch_edge[(size_t)c], ch_edge[(size_t)c + 1], c == C - 1, c > 0);
-        }
-    }
-    // ---- outputs (A12) ----
-    mk.mark(8);
-    launch_output(ctx, N, (const int32_t *)h->inv_perm.p, (const double *)h->Fc.p, (const float *)h->Ei.p,
-                  (const double *)h->vir_part.p, N > 0 ? h->n_vir_blocks : 0, o.dE, o.dF, o.dV, (double *)h->Ei_caller.p,
-                  (double *)h->red_scratch.p);
+    RC(enqueue_zero_accumulators(h));
+    for (int t = md.T - 1; t >= 0; --t) RC(enqueue_backward_layer(h, ctx, mk, t, want_vir, ch_atom, ch_edge));
+    enqueue_output(h, ctx, mk, o);
     return REANN_OK;
 }
 
@@ -739,6 +793,154 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         break;
     }
     mk.finish();
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}
+
+// =============================================================================================
+// NEXT-1 groundwork: one rank of a spatially decomposed run (Fig. 3-4). The handle holds the rank's
+// local atoms and copies of the other ranks' atoms within rc + skin of its domain (ghost atoms, reann_set_halo); the
+// caller drives the layers and moves the two messages of the paper between ranks: forward, c^{t+1} of the ghost
+// atoms from their owners; backward, dE/dc^t of the ghost atoms to their owners.
+__global__ void k_rows_get(const float *__restrict__ base, int stride, int ncol, const int32_t *__restrict__ inv_perm,
+                           const int64_t *__restrict__ idx, int64_t n, float *__restrict__ out) {
+    const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n * ncol) return;
+    const int64_t r = q / ncol; const int c = (int)(q - r * ncol);
+    out[q] = base[(int64_t)inv_perm[idx[r]] * stride + c];
+}
+__global__ void k_rows_put(float *__restrict__ base, int stride, int ncol, const int32_t *__restrict__ inv_perm,
+                           const int64_t *__restrict__ idx, int64_t n, const float *__restrict__ in, int add) {
+    const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n * ncol) return;
+    const int64_t r = q / ncol; const int c = (int)(q - r * ncol);
+    float *dst = base + (int64_t)inv_perm[idx[r]] * stride + c;      // distinct rows: the caller's indices are unique
+    *dst = add ? *dst + in[q] : in[q];
+}
+
+static int rows_xfer(reann *h, float *base, int64_t n, const int64_t *idx, float *host, int mode /*0 get, 1 set, 2 add*/) {
+    if (n < 0 || (n > 0 && (!idx || !host))) return set_err(h, REANN_ERR_ARG, "bad argument");
+    if (n == 0) return REANN_OK;
+    for (int64_t k = 0; k < n; ++k)
+        if (idx[k] < 0 || idx[k] >= h->N) return set_err(h, REANN_ERR_ARG, "atom index out of range");
+    const int nphi = h->md.nphi, stride = h->md.nphip;
+    RC(dev_ensure(h, h->xch_idx, sizeof(int64_t) * (size_t)n));
+    RC(dev_ensure(h, h->xch_val, sizeof(float) * (size_t)n * nphi));
+    LaunchCtx ctx = h->ctx();
+    CU(h, cudaMemcpyAsync(h->xch_idx.p, idx, sizeof(int64_t) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+    if (mode == 0) {
+        LAUNCH(ctx, k_rows_get, div_up(n * nphi, 256), 256, 0, (const float *)base, stride, nphi, (const int32_t *)h->inv_perm.p,
+               (const int64_t *)h->xch_idx.p, n, (float *)h->xch_val.p);
+        CU(h, cudaMemcpyAsync(host, h->xch_val.p, sizeof(float) * (size_t)n * nphi, cudaMemcpyDeviceToHost, h->stream));
+    } else {
+        CU(h, cudaMemcpyAsync(h->xch_val.p, host, sizeof(float) * (size_t)n * nphi, cudaMemcpyHostToDevice, h->stream));
+        LAUNCH(ctx, k_rows_put, div_up(n * nphi, 256), 256, 0, base, stride, nphi, (const int32_t *)h->inv_perm.p,
+               (const int64_t *)h->xch_idx.p, n, (const float *)h->xch_val.p, mode == 2 ? 1 : 0);
+    }
+    CU(h, cudaStreamSynchronize(h->stream));
+    return REANN_OK;
+}
+
+extern "C" int reann_set_halo(reann_t *h, const uint8_t *is_halo) {
+    if (!h) return REANN_ERR_ARG;
+    if (!is_halo || h->N == 0) { h->have_halo = false; return REANN_OK; }
+    RC(dev_ensure(h, h->halo_caller, (size_t)h->N));
+    CU(h, cudaMemcpyAsync(h->halo_caller.p, is_halo, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    h->have_halo = true;
+    return REANN_OK;
+}
+
+extern "C" int reann_step_begin(reann_t *h, const double *pos, const double *box9, int want_virial) {
+    if (!h) return REANN_ERR_ARG;
+    if (!h->have_list) return set_err(h, REANN_ERR_NO_NEIGHBORS, "call reann_build_neighbors first");
+    RC(check_box(h, box9));
+    const double *d_pos = nullptr;
+    RC(device_positions(h, pos, &d_pos));
+    h->n_calls++;
+    h->step_state = 0;
+    if (memcmp(box9, h->box_build, sizeof(double) * 9) != 0 && h->N > 0) RC(do_build(h, d_pos, box9));
+    for (int attempt = 0; attempt < 3 && h->N > 0; ++attempt) {
+        RC(enqueue_prep(h, d_pos));
+        CU(h, cudaMemcpyAsync(h->h_flags, h->flags.p, 16, cudaMemcpyDeviceToHost, h->stream));
+        CU(h, cudaStreamSynchronize(h->stream));
+        if (h->h_flags[0] & FLAG_REBUILD) { RC(do_build(h, d_pos, box9)); continue; }
+        int64_t n_rc = 0;
+        memcpy(&n_rc, h->h_flags + 2, 8);
+        RC(ensure_rc_capacity(h, n_rc));
+        h->E_rc = n_rc;
+        break;
+    }
+    if (h->stash_chunks > 1) return set_err(h, REANN_ERR_UNSUPPORTED, "layer-by-layer calls need the whole per-edge stash in memory");
+    enqueue_filter_fill(h, h->ctx());
+    RC(enqueue_zero_accumulators(h));
+    h->step_state = 1;
+    h->step_vir = want_virial != 0;
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}
+
+extern "C" int reann_step_forward(reann_t *h, int t) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state != 1 || t < 0 || t >= h->md.T) return set_err(h, REANN_ERR_ARG, "reann_step_forward: out of sequence or bad layer");
+    Marks mk{h, {}};
+    const LaunchCtx ctx = h->ctx();
+    if (t >= 1) enqueue_image_gather(h, ctx, mk, t);      // periodic images follow the (possibly just received) c^t rows
+    RC(enqueue_forward_layer(h, ctx, mk, t));
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}
+
+extern "C" int reann_coeff_get(reann_t *h, int t, int64_t n, const int64_t *idx, float *out) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state == 0 || t < 0 || t >= h->md.T) return set_err(h, REANN_ERR_ARG, "reann_coeff_get: out of sequence or bad layer");
+    return rows_xfer(h, (float *)h->c_ext.p + (size_t)t * h->n_ext * h->md.nphip, n, idx, out, 0);
+}
+extern "C" int reann_coeff_set(reann_t *h, int t, int64_t n, const int64_t *idx, const float *in) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state != 1 || t < 1 || t >= h->md.T) return set_err(h, REANN_ERR_ARG, "reann_coeff_set: out of sequence or bad layer");
+    return rows_xfer(h, (float *)h->c_ext.p + (size_t)t * h->n_ext * h->md.nphip, n, idx, const_cast<float *>(in), 1);
+}
+
+extern "C" int reann_step_backward(reann_t *h, int t) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state == 0 || t < 0 || t >= h->md.T) return set_err(h, REANN_ERR_ARG, "reann_step_backward: out of sequence or bad layer");
+    h->step_state = 2;
+    Marks mk{h, {}};
+    const std::vector<int64_t> ca{0, h->N}, ce{0, INT64_MAX};
+    RC(enqueue_backward_layer(h, h->ctx(), mk, t, h->step_vir, ca, ce));
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}
+
+extern "C" int reann_cbar_get(reann_t *h, int64_t n, const int64_t *idx, float *out) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state != 2) return set_err(h, REANN_ERR_ARG, "reann_cbar_get: no reverse layer evaluated yet");
+    return rows_xfer(h, (float *)h->cbar.p, n, idx, out, 0);
+}
+extern "C" int reann_cbar_add(reann_t *h, int64_t n, const int64_t *idx, const float *in) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state != 2) return set_err(h, REANN_ERR_ARG, "reann_cbar_add: no reverse layer evaluated yet");
+    return rows_xfer(h, (float *)h->cbar.p, n, idx, const_cast<float *>(in), 2);
+}
+
+extern "C" int reann_step_end(reann_t *h, double *E, double *F, double *virial) {
+    if (!h) return REANN_ERR_ARG;
+    if (h->step_state == 0) return set_err(h, REANN_ERR_ARG, "reann_step_end: no evaluation in progress");
+    const int64_t N = h->N;
+    const bool E_dev = is_device_ptr(E), F_dev = is_device_ptr(F), V_dev = is_device_ptr(virial);
+    double *stage = (double *)h->out_stage.p;
+    OutPtrs o;
+    o.dE = E ? (E_dev ? E : stage) : stage;
+    o.dV = (virial && h->step_vir) ? (V_dev ? virial : stage + 1) : nullptr;
+    o.dF = F ? (F_dev ? F : stage + 16) : nullptr;
+    Marks mk{h, {}};
+    enqueue_output(h, h->ctx(), mk, o);
+    if (E && !E_dev) CU(h, cudaMemcpyAsync(E, stage, 8, cudaMemcpyDeviceToHost, h->stream));
+    if (o.dV && !V_dev) CU(h, cudaMemcpyAsync(virial, stage + 1, 72, cudaMemcpyDeviceToHost, h->stream));
+    if (F && !F_dev && N > 0) CU(h, cudaMemcpyAsync(F, stage + 16, sizeof(double) * 3 * (size_t)N, cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    h->step_state = 0;
     CU(h, cudaGetLastError());
     return REANN_OK;
 }

@@ -128,7 +128,7 @@ void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, c
                        int64_t e_lo, int64_t e_hi, int do_forces, int accumulate /* kappa holds edges [e_lo, e_hi) */);
 void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, const double *Fc, const float *Ei,
                    const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
-                   double *Ei_sorted, double *scratch);
+                   double *Ei_sorted, double *scratch, const uint8_t *halo_caller /* or nullptr */);
 void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
                    double dt, double acc_unit, int drift);
 

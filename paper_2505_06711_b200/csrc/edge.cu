@@ -671,14 +671,15 @@ __global__ void __launch_bounds__(OUT_TPB) k_output_a(int64_t N, const int32_t *
                                                       const double *__restrict__ Fc, const float *__restrict__ Ei,
                                                       double *__restrict__ F_out, double *__restrict__ Ei_caller,
                                                       const double *__restrict__ vir_part, int n_vir, int want_vir,
-                                                      double *__restrict__ partial, const int32_t *__restrict__ skip) {
+                                                      double *__restrict__ partial, const uint8_t *__restrict__ halo,
+                                                      const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
     __shared__ double red[OUT_TPB];
     const int64_t i = (int64_t)blockIdx.x * OUT_TPB + threadIdx.x; // caller index
     double e = 0.0;
     if (i < N) {
         const int64_t k = inv_perm[i];
-        e = (double)Ei[k];
+        e = (halo && halo[i]) ? 0.0 : (double)Ei[k];    // ghost atoms of a decomposed run: E_i belongs to the owning rank
         if (Ei_caller) Ei_caller[i] = e;
         if (F_out) { F_out[3 * i] = Fc[3 * k]; F_out[3 * i + 1] = Fc[3 * k + 1]; F_out[3 * i + 2] = Fc[3 * k + 2]; }
     }
@@ -859,9 +860,9 @@ void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, c
 
 void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, const double *Fc, const float *Ei,
                    const double *vir_part, int n_vir_blocks, double *E_out, double *F_out, double *vir_out,
-                   double *Ei_caller, double *scratch) {
+                   double *Ei_caller, double *scratch, const uint8_t *halo) {
     const int nb = (int)div_up(N > 0 ? N : 1, OUT_TPB);
-    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, vir_part, n_vir_blocks, vir_out != nullptr, scratch, ctx.skip);
+    LAUNCH(ctx, k_output_a, nb, OUT_TPB, 0, N, inv_perm, Fc, Ei, F_out, Ei_caller, vir_part, n_vir_blocks, vir_out != nullptr, scratch, halo, ctx.skip);
     LAUNCH(ctx, k_output_b, 1, OUT_TPB, 0, nb, (const double *)scratch, E_out, vir_out, ctx.skip);
 }
 

@@ -81,6 +81,13 @@ struct reann {
     DevBuf flags;                 // int32 [4] device flags
     int32_t *h_flags = nullptr;   // pinned mirror [8] (+ int64 n_rc)
 
+    // ---- decomposed runs (NEXT-1 groundwork): ghost atoms of other ranks, layer-by-layer state ----
+    bool have_halo = false;
+    DevBuf halo_caller;           // uint8 [N], caller order: 1 = ghost atom (copy of another rank's atom)
+    DevBuf xch_idx, xch_val;      // staging of reann_coeff_* / reann_cbar_* (int64 indices, float rows)
+    int step_state = 0;           // 0 = idle, 1 = after reann_step_begin (forward), 2 = reverse pass started
+    bool step_vir = false;
+
     // ---- stats / profiling ----
     int64_t n_rebuilds = 0, n_calls = 0, n_prof_calls = 0;
     bool profiling = false;
