@@ -15,6 +15,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
+
 #include "common.cuh"
 #include "edge_common.cuh"
 
@@ -441,15 +443,185 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
 }
 
 // ------------------------------------------------------------------------------------------ A10
-// Warp per atom, one edge per lane; bbar_i is broadcast from shared memory, S_n and P_a stay in the
-// lane's registers, so there is no cross-lane reduction per edge. Orbitals are recomputed (nothing
-// per-edge is kept from the forward pass). Writes the per-edge stash g_e (float4) and kappa_e; the forces are
-// gathered from the g_e stash by k_rev_gather.
-// The radial tables sit in shared memory; c_j and the next pass's edge record are prefetched one
-// step ahead so that no global-load latency is exposed inside the FMA loop. VIR: accumulate the
-// virial (only when the caller asked for it).
+// Warp per atom; bbar_i is broadcast from shared memory, S_n and P_a stay in the lane's registers, so there is no
+// cross-lane reduction per edge. Orbitals are recomputed (nothing per-edge is kept from the forward pass). Writes
+// the per-edge stash g_e (float4) and kappa_e; the forces are gathered from the g_e stash by k_rev_gather.
+// Shared memory delivers 128 B per clock to the lanes whether or not they read the same word, and every float of
+// bbar_i feeds only two FMAs per edge (S and P), so a lane takes NE = 2 edges per pass while more than 32 remain:
+// one 16-byte read then feeds 16 FMAs instead of 8 (the last <= 32 edges of a row go one per lane).
+// VIR: accumulate the virial (only when the caller asked for it).
+template <int NPHIP, int NA, bool VIR, int NE>
+__device__ __forceinline__ void edge_bwd_pass(int64_t e0, int64_t end, const uint32_t *__restrict__ col_rc,
+                                              const float4 *__restrict__ geom, const float *__restrict__ c_ext,
+                                              const float *__restrict__ tab_rc, const float *__restrict__ tab_al,
+                                              float inv_rc, const float *__restrict__ bb, int want_kappa,
+                                              float *__restrict__ kappa, float4 *__restrict__ gst, int64_t e_lo, float *aV,
+                                              const float4 *g_s, const uint32_t *cj_s /* prefetched records of the row's first 64 edges, or nullptr */) {
+    constexpr bool PAIRS = NA % 2 == 0;                   // (a, a+1) pairs never straddle a row of bbar_i
+    constexpr int NP2 = PAIRS ? NA / 2 : 1;
+    static_assert(PAIRS || NE == 1, "two edges per lane need an even number of monomials");
+    const float pi_rc = 3.14159265358979f * inv_rc;
+    int64_t e[NE];
+    bool have[NE];
+    float4 g[NE];
+    int sj[NE];
+    const float4 *cptr[NE];
+    float fc[NE], dfc[NE], radial[NE];
+    float A[NE][NA], P[NE][NA];
+    f32x2 A2[NE][NP2], P2[NE][NP2];
+#pragma unroll
+    for (int k = 0; k < NE; ++k) {
+        e[k] = e0 + 32 * k;
+        have[k] = e[k] < end;
+        g[k] = make_float4(0.f, 0.f, 0.f, 1.f);
+        uint32_t cj = 0;
+        if (have[k]) {
+            if (g_s) { g[k] = g_s[32 * k]; cj = cj_s[32 * k]; }
+            else { g[k] = geom[e[k]]; cj = col_rc[e[k]]; }
+        }
+        sj[k] = cj >> COL_SPECIES_SHIFT;
+        cptr[k] = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
+    }
+#pragma unroll
+    for (int k = 0; k < NE; ++k) {
+        float sn, cs;
+        sincospif(g[k].w * inv_rc, &sn, &cs);
+        fc[k] = 0.5f + 0.5f * cs; dfc[k] = -0.5f * pi_rc * sn;
+        monomials<NA>(g[k].x, g[k].y, g[k].z, A[k]);
+        radial[k] = 0.f;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) P[k][a] = 0.f;
+        if constexpr (PAIRS) {
+#pragma unroll
+            for (int a2 = 0; a2 < NP2; ++a2) { A2[k][a2] = pack2(A[k][2 * a2], A[k][2 * a2 + 1]); P2[k][a2] = pack2(0.f, 0.f); }
+        }
+    }
+    // four rows n of bbar_i per outer iteration (one float4 of c_j / r_n / alpha_n / kappa);
+    // the outer loop is kept rolled so that the shared-memory loads are not all hoisted. The gathered c_j quad of
+    // the next iteration is requested one iteration ahead (an L2 round trip).
+    float4 cvc[NE];
+#pragma unroll
+    for (int k = 0; k < NE; ++k) cvc[k] = cptr[k][0];
+#pragma unroll 1
+    for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
+        float Rn[NE][4], xn[NE][4], yn[NE][4], Sn[NE][4];
+        float4 cvn[NE];
+#pragma unroll
+        for (int k = 0; k < NE; ++k) cvn[k] = cptr[k][n4 + 1 < NPHIP / 4 ? n4 + 1 : n4];
+#pragma unroll
+        for (int k = 0; k < NE; ++k) {
+            const float4 cv = cvc[k];
+            const float4 rc4 = reinterpret_cast<const float4 *>(tab_rc + sj[k] * NPHIP)[n4];
+            const float4 al4 = reinterpret_cast<const float4 *>(tab_al + sj[k] * NPHIP)[n4];
+            const float cva[4] = {cv.x, cv.y, cv.z, cv.w}, rca[4] = {rc4.x, rc4.y, rc4.z, rc4.w},
+                        ala[4] = {al4.x, al4.y, al4.z, al4.w};
+            // alpha2 = alpha*log2(e): d/dr exp(-alpha d^2) = -2 ln2 alpha2 d ex; two n per packed operation
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const f32x2 al2 = pack2(ala[2 * h], ala[2 * h + 1]), c2 = pack2(cva[2 * h], cva[2 * h + 1]);
+                const f32x2 d2 = fmadd2(pack2(rca[2 * h], rca[2 * h + 1]), pack2(-1.f, -1.f), pack2(g[k].w, g[k].w));
+                const f32x2 ad2 = fmul2(al2, d2);
+                float a0, a1;
+                unpack2(fmul2(ad2, d2), a0, a1);
+                const f32x2 ex2 = pack2(exp2f(-a0), exp2f(-a1));
+                const f32x2 R2 = fmul2(ex2, pack2(fc[k], fc[k]));
+                const f32x2 y2 = fmul2(c2, fmul2(fmadd2(ad2, pack2(-1.3862943611198906f * fc[k], -1.3862943611198906f * fc[k]),
+                                                        pack2(dfc[k], dfc[k])), ex2));
+                unpack2(R2, Rn[k][2 * h], Rn[k][2 * h + 1]);
+                unpack2(fmul2(c2, R2), xn[k][2 * h], xn[k][2 * h + 1]);
+                unpack2(y2, yn[k][2 * h], yn[k][2 * h + 1]);
+                Sn[k][2 * h] = Sn[k][2 * h + 1] = 0.f;
+            }
+        }
+        const float4 *bb4 = reinterpret_cast<const float4 *>(bb + n4 * 4 * NA);
+        if constexpr (PAIRS) {
+            f32x2 S2[NE][4], x2[NE][4];
+#pragma unroll
+            for (int k = 0; k < NE; ++k)
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { S2[k][u] = pack2(0.f, 0.f); x2[k][u] = pack2(xn[k][u], xn[k][u]); }
+#pragma unroll
+            for (int f4 = 0; f4 < NA; ++f4) { // 4 rows x NA values = NA float4 = 2 NA pairs
+                const float4 v = bb4[f4];
+                const f32x2 v2[2] = {pack2(v.x, v.y), pack2(v.z, v.w)};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int f = f4 * 4 + 2 * h, nl = f / NA, a2 = (f % NA) / 2;
+#pragma unroll
+                    for (int k = 0; k < NE; ++k) {
+                        ffma2(S2[k][nl], v2[h], A2[k][a2]);
+                        ffma2(P2[k][a2], v2[h], x2[k][nl]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NE; ++k)
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { float lo, hi; unpack2(S2[k][u], lo, hi); Sn[k][u] = lo + hi; }
+        } else {
+#pragma unroll
+            for (int f4 = 0; f4 < NA; ++f4) {
+                const float4 v = bb4[f4];
+                const float va[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int f = f4 * 4 + u, nl = f / NA, a = f % NA;
+                    Sn[0][nl] = fmaf(va[u], A[0][a], Sn[0][nl]);
+                    P[0][a] = fmaf(va[u], xn[0][nl], P[0][a]);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NE; ++k) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) radial[k] = fmaf(yn[k][u], Sn[k][u], radial[k]);
+            if (want_kappa && have[k])
+                reinterpret_cast<float4 *>(kappa + (e[k] - e_lo) * (int64_t)NPHIP)[n4] =
+                    make_float4(Rn[k][0] * Sn[k][0], Rn[k][1] * Sn[k][1], Rn[k][2] * Sn[k][2], Rn[k][3] * Sn[k][3]);
+            cvc[k] = cvn[k];
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NE; ++k) {
+        if constexpr (PAIRS) {
+#pragma unroll
+            for (int a2 = 0; a2 < NP2; ++a2) unpack2(P2[k][a2], P[k][2 * a2], P[k][2 * a2 + 1]);
+        }
+        float gx, gy, gz;
+        monomial_vjp<NA>(A[k], P[k], gx, gy, gz);
+        const float rr = __fdividef(radial[k], g[k].w);
+        gx = fmaf(rr, g[k].x, gx); gy = fmaf(rr, g[k].y, gy); gz = fmaf(rr, g[k].z, gz);
+        if (have[k]) {
+            gst[e[k]] = make_float4(gx, gy, gz, 0.f);
+            if constexpr (VIR) {
+                aV[0] -= g[k].x * gx; aV[1] -= g[k].x * gy; aV[2] -= g[k].x * gz;
+                aV[3] -= g[k].y * gx; aV[4] -= g[k].y * gy; aV[5] -= g[k].y * gz;
+                aV[6] -= g[k].z * gx; aV[7] -= g[k].z * gy; aV[8] -= g[k].z * gz;
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *dst_smem, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
+
+// Persistent warps: a warp walks over atoms (stride = warps of the grid); bbar_i and the records of the row's first
+// 64 edges of the NEXT atom arrive by cp.async while the current atom is processed (double-buffered in shared
+// memory, no registers held), so an atom starts without waiting on DRAM.
+// two edges per lane where the registers allow three blocks per SM with it (N_a <= 10); at N_a = 20 the pair of edges
+// costs a quarter of the resident warps and measured slower (1.09 vs 1.03 ms on config 3)
+template <int NA>
+struct BwdShape { static constexpr int NE = (NA % 2 == 0 && NA <= 10) ? 2 : 1, MINB = NE == 2 ? 3 : 4; };
+
 template <int NPHIP, int NA, bool VIR>
-__global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
+__global__ void __launch_bounds__(EW * 32, BwdShape<NA>::MINB) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                       const uint32_t *__restrict__ col_rc,
                                                       const float4 *__restrict__ geom,
                                                       const float *__restrict__ c_ext, RadialTab rt, int S,
@@ -458,141 +630,73 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
                                                       double *__restrict__ vir_part, AtomChunk ch, const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
     constexpr int NB = NPHIP * NA;
-    __shared__ __align__(16) float bb_s[EW][NB];
+    __shared__ __align__(16) float bb_s[EW][2][NB];
+    __shared__ __align__(16) float4 g_s[EW][2][64];
+    __shared__ uint32_t cj_s[EW][2][64];
     __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
     __shared__ float vir_s[VIR ? EW : 1][9];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t i0 = ch.a0 + (int64_t)blockIdx.x * EW + warp;
-    const int64_t i = i0 < ch.a1 ? i0 : N;              // atoms [a0, a1) of this launch
     for (int k = threadIdx.x; k < S * NPHIP; k += EW * 32) { tab_s[0][k] = rt.rcen[k]; tab_s[1][k] = rt.alpha2[k]; }
+    __syncthreads();
     float aV[VIR ? 9 : 1];
 #pragma unroll
     for (int k = 0; k < (VIR ? 9 : 1); ++k) aV[k] = 0.f;
-    if (i < N) {
-        const float4 *src = reinterpret_cast<const float4 *>(bbar + i * (int64_t)NB);
-        for (int k = lane; k < NB / 4; k += 32) reinterpret_cast<float4 *>(bb_s[warp])[k] = src[k];
-    }
-    __syncthreads();
-    if (i < N) {
-        const int64_t beg = rc_ptr[i], end = rc_ptr[i + 1];
-        const float pi_rc = 3.14159265358979f * rt.inv_rc;
-        int64_t e = beg + lane;
-        float4 g = make_float4(0.f, 0.f, 0.f, 1.f);
-        uint32_t cj = 0;
-        if (e < end) { g = geom[e]; cj = col_rc[e]; }
-        while (e < end) {
-            const int sj = cj >> COL_SPECIES_SHIFT;
-            const float4 *cptr = reinterpret_cast<const float4 *>(c_ext + (int64_t)(cj & COL_IDX_MASK) * NPHIP);
-            float4 cv = cptr[0];
-            // next pass's edge record
-            const int64_t e_next = e + 32;
-            float4 g_next = g;
-            uint32_t cj_next = cj;
-            if (e_next < end) { g_next = geom[e_next]; cj_next = col_rc[e_next]; }
-            float sn, cs;
-            sincospif(g.w * rt.inv_rc, &sn, &cs);
-            const float fc = 0.5f + 0.5f * cs, dfc = -0.5f * pi_rc * sn;
-            constexpr bool PAIRS = NA % 2 == 0;                   // (a, a+1) pairs never straddle a row of bbar_i
-            constexpr int NP2 = PAIRS ? NA / 2 : 1;
-            float A[NA], P[NA];
-            monomials<NA>(g.x, g.y, g.z, A);
+    const int64_t stride = (int64_t)gridDim.x * EW;
+    int64_t i = ch.a0 + (int64_t)blockIdx.x * EW + warp;
+    // request bbar and the first-pass records of atom `a` (row [b0, b1)) into buffer `buf`
+    auto request = [&](int64_t a, int64_t b0, int64_t b1, int buf) {
+        const float4 *src = reinterpret_cast<const float4 *>(bbar + a * (int64_t)NB);
+        for (int k = lane; k < NB / 4; k += 32) cp_async16(reinterpret_cast<float4 *>(bb_s[warp][buf]) + k, src + k);
 #pragma unroll
-            for (int a = 0; a < NA; ++a) P[a] = 0.f;
-            f32x2 A2[NP2], P2[NP2];
-            if constexpr (PAIRS) {
-#pragma unroll
-                for (int a2 = 0; a2 < NP2; ++a2) { A2[a2] = pack2(A[2 * a2], A[2 * a2 + 1]); P2[a2] = pack2(0.f, 0.f); }
-            }
-            // four rows n of bbar_i per outer iteration (one float4 of c_j / r_n / alpha_n / kappa);
-            // the outer loop is kept rolled so that the shared-memory loads are not all hoisted.
-            float radial = 0.f;
-            float4 *kp = reinterpret_cast<float4 *>(kappa + (e - ch.e_lo) * (int64_t)NPHIP);
-#pragma unroll 1
-            for (int n4 = 0; n4 < NPHIP / 4; ++n4) {
-                const float4 cvn = cptr[n4 + 1 < NPHIP / 4 ? n4 + 1 : n4];
-                const float4 rc4 = reinterpret_cast<const float4 *>(tab_s[0] + sj * NPHIP)[n4];
-                const float4 al4 = reinterpret_cast<const float4 *>(tab_s[1] + sj * NPHIP)[n4];
-                const float cva[4] = {cv.x, cv.y, cv.z, cv.w}, rca[4] = {rc4.x, rc4.y, rc4.z, rc4.w},
-                            ala[4] = {al4.x, al4.y, al4.z, al4.w};
-                float Rn[4], xn[4], yn[4], Sn[4];
-                // alpha2 = alpha*log2(e): d/dr exp(-alpha d^2) = -2 ln2 alpha2 d ex; two n per packed operation
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const f32x2 al2 = pack2(ala[2 * h], ala[2 * h + 1]), c2 = pack2(cva[2 * h], cva[2 * h + 1]);
-                    const f32x2 d2 = fmadd2(pack2(rca[2 * h], rca[2 * h + 1]), pack2(-1.f, -1.f), pack2(g.w, g.w));
-                    const f32x2 ad2 = fmul2(al2, d2);
-                    float a0, a1;
-                    unpack2(fmul2(ad2, d2), a0, a1);
-                    const f32x2 ex2 = pack2(exp2f(-a0), exp2f(-a1));
-                    const f32x2 R2 = fmul2(ex2, pack2(fc, fc));
-                    const f32x2 y2 = fmul2(c2, fmul2(fmadd2(ad2, pack2(-1.3862943611198906f * fc, -1.3862943611198906f * fc),
-                                                            pack2(dfc, dfc)), ex2));
-                    unpack2(R2, Rn[2 * h], Rn[2 * h + 1]);
-                    unpack2(fmul2(c2, R2), xn[2 * h], xn[2 * h + 1]);
-                    unpack2(y2, yn[2 * h], yn[2 * h + 1]);
-                    Sn[2 * h] = Sn[2 * h + 1] = 0.f;
-                }
-                const float4 *bb4 = reinterpret_cast<const float4 *>(bb_s[warp] + n4 * 4 * NA);
-                if constexpr (PAIRS) {
-                    f32x2 S2[4], x2[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) { S2[u] = pack2(0.f, 0.f); x2[u] = pack2(xn[u], xn[u]); }
-#pragma unroll
-                    for (int f4 = 0; f4 < NA; ++f4) { // 4 rows x NA values = NA float4 = 2 NA pairs
-                        const float4 v = bb4[f4];
-                        const f32x2 v2[2] = {pack2(v.x, v.y), pack2(v.z, v.w)};
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const int f = f4 * 4 + 2 * h, nl = f / NA, a2 = (f % NA) / 2;
-                            ffma2(S2[nl], v2[h], A2[a2]);
-                            ffma2(P2[a2], v2[h], x2[nl]);
-                        }
-                    }
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) { float lo, hi; unpack2(S2[u], lo, hi); Sn[u] = lo + hi; }
-                } else {
-#pragma unroll
-                    for (int f4 = 0; f4 < NA; ++f4) {
-                        const float4 v = bb4[f4];
-                        const float va[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const int f = f4 * 4 + u, nl = f / NA, a = f % NA;
-                            Sn[nl] = fmaf(va[u], A[a], Sn[nl]);
-                            P[a] = fmaf(va[u], xn[nl], P[a]);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) radial = fmaf(yn[u], Sn[u], radial);
-                if (want_kappa) kp[n4] = make_float4(Rn[0] * Sn[0], Rn[1] * Sn[1], Rn[2] * Sn[2], Rn[3] * Sn[3]);
-                cv = cvn;
-            }
-            if constexpr (PAIRS) {
-#pragma unroll
-                for (int a2 = 0; a2 < NP2; ++a2) unpack2(P2[a2], P[2 * a2], P[2 * a2 + 1]);
-            }
-            float gx, gy, gz;
-            monomial_vjp<NA>(A, P, gx, gy, gz);
-            const float rr = __fdividef(radial, g.w);
-            gx = fmaf(rr, g.x, gx); gy = fmaf(rr, g.y, gy); gz = fmaf(rr, g.z, gz);
-            gst[e] = make_float4(gx, gy, gz, 0.f);
-            if constexpr (VIR) {
-                aV[0] -= g.x * gx; aV[1] -= g.x * gy; aV[2] -= g.x * gz;
-                aV[3] -= g.y * gx; aV[4] -= g.y * gy; aV[5] -= g.y * gz;
-                aV[6] -= g.z * gx; aV[7] -= g.z * gy; aV[8] -= g.z * gz;
-            }
-            e = e_next; g = g_next; cj = cj_next;
+        for (int k = 0; k < 2; ++k) {
+            const int64_t e = b0 + lane + 32 * k;
+            if (e < b1) { cp_async16(&g_s[warp][buf][lane + 32 * k], geom + e); cp_async4(&cj_s[warp][buf][lane + 32 * k], col_rc + e); }
         }
+    };
+    int64_t beg = 0, end = 0, beg_n = 0, end_n = 0;
+    int buf = 0;
+    if (i < ch.a1) {
+        beg = rc_ptr[i]; end = rc_ptr[i + 1];
+        request(i, beg, end, 0);
+        if (i + stride < ch.a1) { beg_n = rc_ptr[i + stride]; end_n = rc_ptr[i + stride + 1]; }
     }
+    cp_async_commit();
+    for (; i < ch.a1; i += stride) {
+        const int64_t i_n = i + stride;
+        if (i_n < ch.a1) request(i_n, beg_n, end_n, buf ^ 1);
+        cp_async_commit();
+        int64_t beg_nn = 0, end_nn = 0;
+        if (i_n + stride < ch.a1) { beg_nn = rc_ptr[i_n + stride]; end_nn = rc_ptr[i_n + stride + 1]; }
+        cp_async_wait<1>();                                  // this atom's group (the one committed an iteration ago)
+        __syncwarp();
+        int64_t p0 = beg;                                    // first edge of the pass (warp-uniform)
+        while (p0 < end) {
+            const bool first = p0 == beg;
+            const float4 *gp = first ? &g_s[warp][buf][lane] : nullptr;
+            const uint32_t *cp = first ? &cj_s[warp][buf][lane] : nullptr;
+            if constexpr (BwdShape<NA>::NE == 2) {
+                if (end - p0 > 32) {
+                    edge_bwd_pass<NPHIP, NA, VIR, 2>(p0 + lane, end, col_rc, geom, c_ext, tab_s[0], tab_s[1], rt.inv_rc,
+                                                     bb_s[warp][buf], want_kappa, kappa, gst, ch.e_lo, aV, gp, cp);
+                    p0 += 64;
+                    continue;
+                }
+            }
+            edge_bwd_pass<NPHIP, NA, VIR, 1>(p0 + lane, end, col_rc, geom, c_ext, tab_s[0], tab_s[1], rt.inv_rc,
+                                             bb_s[warp][buf], want_kappa, kappa, gst, ch.e_lo, aV, gp, cp);
+            p0 += 32;
+        }
+        __syncwarp();                                        // every lane is done with bb_s[buf] before it is refilled
+        buf ^= 1;
+        beg = beg_n; end = end_n; beg_n = beg_nn; end_n = end_nn;
+    }
+    cp_async_wait<0>();
     // fixed-order reductions: lanes (butterfly, FP32), then FP64 accumulation across layers / warps
     if constexpr (VIR) {
 #pragma unroll
         for (int d = 16; d >= 1; d >>= 1)
 #pragma unroll
             for (int k = 0; k < 9; ++k) aV[k] += __shfl_xor_sync(0xffffffffu, aV[k], d);
-    }
-    if constexpr (VIR) {
         if (lane == 0) {
 #pragma unroll
             for (int k = 0; k < 9; ++k) vir_s[warp][k] = aV[k];
@@ -602,7 +706,7 @@ __global__ void __launch_bounds__(EW * 32, 4) k_edge_bwd(int64_t N, const int64_
             double s = 0.0;
 #pragma unroll
             for (int w = 0; w < EW; ++w) s += (double)vir_s[w][threadIdx.x];
-            vir_part[(ch.a0 / EW + (int64_t)blockIdx.x) * 9 + threadIdx.x] += s;
+            vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x] += s;
         }
     }
 }
@@ -822,7 +926,17 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 #undef M
 }
 
-int edge_bwd_blocks(int64_t N) { return (int)div_up(N, EW); }
+// upper bound of the grid of the edge backward kernel (= entries of the virial partial array)
+int edge_bwd_blocks(int64_t N) { return (int)div_up(std::max<int64_t>(N, 1), EW); }
+static int sm_count() {
+    static int n_sm[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) dev = 0;
+    if (!n_sm[dev] && (cudaDeviceGetAttribute(&n_sm[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm[dev] <= 0))
+        n_sm[dev] = 148;
+    return n_sm[dev];
+}
 
 int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
@@ -830,17 +944,19 @@ int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
                     int64_t a0, int64_t a1, int64_t e_lo) {
     if (N <= 0 || a1 <= a0) return REANN_OK;
     const AtomChunk ch{a0, a1, e_lo};
-    const unsigned nblk = div_up(a1 - a0, EW);
+    const unsigned nblk_all = div_up(a1 - a0, EW);
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
     const int want_kappa = t >= 1;
-#define M(NP, NA_, PN_, PA_)                                                                                      \
+#define M(NP, NA_, PN_, PA_) {                                                                                    \
+    /* two edges per lane: persistent warps, one wave of resident blocks; else one atom per warp (measured faster) */ \
+    const unsigned nblk = BwdShape<NA_>::NE == 2 ? std::min(nblk_all, (unsigned)(BwdShape<NA_>::MINB * sm_count())) : nblk_all; \
     if (vir_part)                                                                                                 \
         LAUNCH(ctx, (k_edge_bwd<NP, NA_, true>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,            \
                md.S, bbar, want_kappa, kappa, gst, vir_part, ch, ctx.skip);                                       \
     else                                                                                                          \
         LAUNCH(ctx, (k_edge_bwd<NP, NA_, false>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,           \
                md.S, bbar, want_kappa, kappa, gst, vir_part, ch, ctx.skip);                                       \
-    return REANN_OK;
+    return REANN_OK; }
     EDGE_DISPATCH(M)
 #undef M
 }
