@@ -251,10 +251,10 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
                     const float4 al4 = reinterpret_cast<const float4 *>(rt.alpha2 + sj * NPHIP)[part];
                     float4 xv;
                     float d;
-                    d = we - rc4.x; xv.x = cv.x * (exp2f(-al4.x * d * d) * fce);
-                    d = we - rc4.y; xv.y = cv.y * (exp2f(-al4.y * d * d) * fce);
-                    d = we - rc4.z; xv.z = cv.z * (exp2f(-al4.z * d * d) * fce);
-                    d = we - rc4.w; xv.w = cv.w * (exp2f(-al4.w * d * d) * fce);
+                    d = we - rc4.x; xv.x = cv.x * (ex2_ftz(-al4.x * d * d) * fce);
+                    d = we - rc4.y; xv.y = cv.y * (ex2_ftz(-al4.y * d * d) * fce);
+                    d = we - rc4.z; xv.z = cv.z * (ex2_ftz(-al4.z * d * d) * fce);
+                    d = we - rc4.w; xv.w = cv.w * (ex2_ftz(-al4.w * d * d) * fce);
                     reinterpret_cast<float4 *>(stage + (size_t)rr * C::ROW)[part] = xv;
                 }
             }
@@ -400,8 +400,8 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
                     float a0, a1, a2, a3;
                     unpack2(fmul2(fmul2(pack2(al4.x, al4.y), da), da), a0, a1);
                     unpack2(fmul2(fmul2(pack2(al4.z, al4.w), db), db), a2, a3);
-                    unpack2(fmul2(pack2(cv.x, cv.y), fmul2(pack2(exp2f(-a0), exp2f(-a1)), f2)), xv.x, xv.y);
-                    unpack2(fmul2(pack2(cv.z, cv.w), fmul2(pack2(exp2f(-a2), exp2f(-a3)), f2)), xv.z, xv.w);
+                    unpack2(fmul2(pack2(cv.x, cv.y), fmul2(pack2(ex2_ftz(-a0), ex2_ftz(-a1)), f2)), xv.x, xv.y);
+                    unpack2(fmul2(pack2(cv.z, cv.w), fmul2(pack2(ex2_ftz(-a2), ex2_ftz(-a3)), f2)), xv.z, xv.w);
                 }
                 float *dst = XT + (part * 4) * TS + rr;
                 dst[0] = xv.x; dst[TS] = xv.y; dst[2 * TS] = xv.z; dst[3 * TS] = xv.w;
@@ -523,7 +523,7 @@ __device__ __forceinline__ void edge_bwd_pass(int64_t e0, int64_t end, const uin
                 const f32x2 ad2 = fmul2(al2, d2);
                 float a0, a1;
                 unpack2(fmul2(ad2, d2), a0, a1);
-                const f32x2 ex2 = pack2(exp2f(-a0), exp2f(-a1));
+                const f32x2 ex2 = pack2(ex2_ftz(-a0), ex2_ftz(-a1));
                 const f32x2 R2 = fmul2(ex2, pack2(fc[k], fc[k]));
                 const f32x2 y2 = fmul2(c2, fmul2(fmadd2(ad2, pack2(-1.3862943611198906f * fc[k], -1.3862943611198906f * fc[k]),
                                                         pack2(dfc[k], dfc[k])), ex2));

@@ -35,6 +35,9 @@ __device__ __forceinline__ void monomial_vjp(const float *A, const float *P, flo
     }
 }
 
+// 2^x as one MUFU.EX2 (exp2f() wraps it in a range check for denormal results, six more instructions per call)
+__device__ __forceinline__ float ex2_ftz(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 // Packed FP32 pairs: Blackwell's fma.rn.f32x2 (SASS FFMA2) does two FP32 FMAs per issue slot at the same FLOP
 // rate (measured 74 TFLOP/s either way), which halves the instruction count of the FMA loops below.
 typedef unsigned long long f32x2;
