@@ -172,6 +172,34 @@ int reann_step_end(reann_t *h, double *E, double *F, double *virial);
 int reann_verlet(reann_t *h, double *pos, double *vel, const double *F, const double *inv_mass,
                  double dt, double acc_unit, int drift);
 
+/*
+ * ---- Device-resident molecular dynamics ----
+ * The paper drives its potentials in NVT molecular dynamics at 300 K (MD driver of
+ * section 4.2). reann_md_run advances n_steps of velocity Verlet, optionally with a Nose-Hoover
+ * thermostat (one thermostat variable; half step before and after every velocity-Verlet step; g = 3 n_atoms degrees of
+ * freedom; Q = g kT tau^2 -- the integrator is written out in DESIGN.md section 2, B-7, and in oracle/md.py):
+ *   pos, vel [n_atoms][3], inv_mass [n_atoms] (1/amu), F [n_atoms][3], virial [9] or NULL: DEVICE pointers, caller
+ *     order; pos and vel are advanced in place, F and virial hold the values at the final positions on return
+ *     (F need not be initialised: the forces at the initial positions are evaluated first, unless st->forces_valid
+ *     says that F already holds them, e.g. from the previous reann_md_run of the same trajectory);
+ *   dt in fs, acc_unit converts eV/(A amu) to A/fs^2, kT = kB T in eV (kT <= 0: no thermostat, NVE), tau in fs;
+ *   st: in  xi, vxi (0, 0 to start; pass the values a previous call returned to continue a run), forces_valid,
+ *       out xi, vxi, kinetic and potential energy (eV) after the last step, the conserved quantity
+ *           KE + PE + Q vxi^2 / 2 + g kT xi, steps done, rebuilds of the neighbour list during the run.
+ * Nothing but the thermostat scalars and E crosses to the host; every step is one reann_energy_forces (skin check on
+ * the device, CUDA graph of the evaluation) plus three small kernels. Builds the list first if there is none.
+ * Errors: as reann_energy_forces; REANN_ERR_ARG for host pointers or non-positive dt / acc_unit / tau.
+ */
+typedef struct {
+    double xi, vxi;
+    int64_t forces_valid;            /* in: non-zero = F holds the forces at pos (skip the initial evaluation; then
+                                        `potential` / `conserved` are only defined when n_steps > 0) */
+    double kinetic, potential, conserved;
+    int64_t n_steps_done, n_rebuilds;
+} reann_md_state_t;
+int reann_md_run(reann_t *h, double *pos, double *vel, const double *inv_mass, const double *box9, int64_t n_steps,
+                 double dt, double acc_unit, double kT, double tau, double *F, double *virial, reann_md_state_t *st);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,13 +23,20 @@ REANN_OK, REANN_ERR_ARG, REANN_ERR_WEIGHTS, REANN_ERR_BOX, REANN_ERR_NO_NEIGHBOR
 EXPORTS = ["reann_create", "reann_build_neighbors", "reann_energy_forces", "reann_destroy", "reann_last_error",
            "reann_get_neighbors", "reann_get_neighbor_rows", "reann_get_stats", "reann_set_profiling", "reann_set_stream",
            "reann_get_atomic_energies", "reann_verlet", "reann_set_halo", "reann_step_begin", "reann_step_forward",
-           "reann_coeff_get", "reann_coeff_set", "reann_step_backward", "reann_cbar_get", "reann_cbar_add", "reann_step_end"]
+           "reann_coeff_get", "reann_coeff_set", "reann_step_backward", "reann_cbar_get", "reann_cbar_add", "reann_step_end",
+           "reann_md_run"]
 
 
 class ReannError(RuntimeError):
     def __init__(self, code: int, text: str):
         super().__init__(f"reann error {code}: {text}")
         self.code = code
+
+
+class MdState(ctypes.Structure):
+    _fields_ = [("xi", ctypes.c_double), ("vxi", ctypes.c_double), ("forces_valid", ctypes.c_int64), ("kinetic", ctypes.c_double),
+                ("potential", ctypes.c_double), ("conserved", ctypes.c_double), ("n_steps_done", ctypes.c_int64),
+                ("n_rebuilds", ctypes.c_int64)]
 
 
 class Stats(ctypes.Structure):
@@ -87,6 +94,8 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = args
         L.reann_verlet.restype = ctypes.c_int
         L.reann_verlet.argtypes = [vp, vp, vp, vp, vp, dbl, dbl, ctypes.c_int]
+        L.reann_md_run.restype = ctypes.c_int
+        L.reann_md_run.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, vp, vp, ctypes.POINTER(MdState)]
         _lib = L
     return _lib
 
@@ -258,6 +267,15 @@ class Reann:
     def verlet(self, pos, vel, F, inv_mass, dt, acc_unit, drift: bool):
         _check(self.h, lib().reann_verlet(self.h, _ptr(pos), _ptr(vel), _ptr(F), _ptr(inv_mass), float(dt),
                                           float(acc_unit), int(drift)))
+
+    def md_run(self, pos, vel, inv_mass, box, n_steps, dt, acc_unit, kT=0.0, tau=100.0, F=None, virial=None, xi=0.0, vxi=0.0,
+               forces_valid=False):
+        """reann_md_run on device tensors (pos, vel advanced in place); returns the thermostat / energy record."""
+        st = MdState(xi=float(xi), vxi=float(vxi), forces_valid=int(bool(forces_valid)))
+        _check(self.h, lib().reann_md_run(self.h, _ptr(pos), _ptr(vel), _ptr(inv_mass), _ptr(_box(box)), int(n_steps),
+                                          float(dt), float(acc_unit), float(kT), float(tau), _ptr(F), _ptr(virial),
+                                          ctypes.byref(st)))
+        return {k: getattr(st, k) for k, _ in MdState._fields_}
 
     def close(self):
         if self.h is not None:

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libreann_b200.so")
-SOURCES = ["api.cu", "scan.cu", "neighbor.cu", "edge.cu", "gram.cu", "dense.cu", "dense_tc.cu"]
+SOURCES = ["api.cu", "scan.cu", "neighbor.cu", "edge.cu", "gram.cu", "dense.cu", "dense_tc.cu", "md.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -357,7 +357,7 @@ extern "C" void reann_destroy(reann_t *h) {
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
                       &h->geom, &h->rev_rc, &h->c_ext, &h->b, &h->z_stash, &h->bbar, &h->cbar, &h->kappa, &h->gst,
                       &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch, &h->Qbuf,
-                      &h->halo_caller, &h->xch_idx, &h->xch_val};
+                      &h->halo_caller, &h->xch_idx, &h->xch_val, &h->md_state, &h->md_partial, &h->md_E};
     for (DevBuf *b : bufs) dev_free(h, *b);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
@@ -985,6 +985,51 @@ extern "C" int reann_verlet(reann_t *h, double *pos, double *vel, const double *
     if (!is_device_ptr(pos) || !is_device_ptr(vel) || !is_device_ptr(F) || !is_device_ptr(inv_mass))
         return set_err(h, REANN_ERR_ARG, "reann_verlet takes device pointers");
     launch_verlet(h->ctx(), h->N, pos, vel, F, inv_mass, dt, acc_unit, drift);
+    CU(h, cudaGetLastError());
+    return REANN_OK;
+}
+
+// NEXT-3 (SURVEY.md 8(f); PAPER.md:110-116 NVT MD, :122): n_steps of velocity Verlet (+ Nose-Hoover thermostat) with
+// positions, velocities, forces and the thermostat state on the device throughout; see md.cu for the scheme.
+extern "C" int reann_md_run(reann_t *h, double *pos, double *vel, const double *inv_mass, const double *box9,
+                            int64_t n_steps, double dt, double acc_unit, double kT, double tau, double *F, double *virial,
+                            reann_md_state_t *st) {
+    if (!h || !st || !pos || !vel || !inv_mass || !F || n_steps < 0 || !(dt > 0.0) || !(acc_unit > 0.0)) return REANN_ERR_ARG;
+    if (!is_device_ptr(pos) || !is_device_ptr(vel) || !is_device_ptr(inv_mass) || !is_device_ptr(F) ||
+        (virial && !is_device_ptr(virial)))
+        return set_err(h, REANN_ERR_ARG, "reann_md_run takes device pointers (pos, vel, inv_mass, F, virial)");
+    const bool nvt = kT > 0.0;
+    if (nvt && !(tau > 0.0)) return set_err(h, REANN_ERR_ARG, "thermostat time constant tau must be > 0");
+    const int64_t N = h->N;
+    const double g = 3.0 * (double)N, g_kT = g * kT, Q = nvt ? g_kT * tau * tau : 1.0;
+    RC(dev_ensure(h, h->md_state, sizeof(double) * 8));
+    RC(dev_ensure(h, h->md_partial, sizeof(double) * (size_t)(md_blocks(N) + 1)));
+    RC(dev_ensure(h, h->md_E, sizeof(double)));
+    double *state = (double *)h->md_state.p, *part = (double *)h->md_partial.p, *dE = (double *)h->md_E.p;
+    const double init[8] = {st->xi, st->vxi, 1.0, 0.0, 1.0, 0.0, 0.0, 0.0};
+    CU(h, cudaMemcpyAsync(state, init, sizeof(init), cudaMemcpyHostToDevice, h->stream));
+    const int64_t rebuilds0 = h->n_rebuilds;
+    if (!h->have_list) RC(reann_build_neighbors(h, pos, box9));
+    if (!st->forces_valid) RC(reann_energy_forces(h, pos, box9, dE, F, virial));   // forces at the initial positions
+    LaunchCtx ctx = h->ctx();
+    launch_md_kick(ctx, N, pos, vel, F, inv_mass, 0.0, acc_unit, 0, nullptr, part);      // sum m v^2 of the initial velocities
+    launch_nh_update(ctx, N, part, state, 0.5 * dt, g_kT, Q, acc_unit, n_steps > 0 ? 0 : 2, nvt && n_steps > 0);
+    for (int64_t k = 0; k < n_steps; ++k) {
+        launch_md_kick(ctx, N, pos, vel, F, inv_mass, dt, acc_unit, 1, state, nullptr);  // (pending scale) half kick + drift
+        RC(reann_energy_forces(h, pos, box9, dE, F, virial));
+        launch_md_kick(ctx, N, pos, vel, F, inv_mass, dt, acc_unit, 0, nullptr, part);   // half kick + sum m v^2
+        launch_nh_update(ctx, N, part, state, 0.5 * dt, g_kT, Q, acc_unit, k + 1 < n_steps ? 1 : 2, nvt);
+    }
+    launch_md_scale(ctx, N, vel, state);
+    double hs[8], pe = 0.0;
+    CU(h, cudaMemcpyAsync(hs, state, sizeof(hs), cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaMemcpyAsync(&pe, dE, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    st->xi = hs[0]; st->vxi = hs[1];
+    st->kinetic = 0.5 * hs[3]; st->potential = pe;
+    st->conserved = st->kinetic + pe + (nvt ? 0.5 * Q * hs[1] * hs[1] + g_kT * hs[0] : 0.0);
+    st->n_steps_done = n_steps;
+    st->n_rebuilds = h->n_rebuilds - rebuilds0;
     CU(h, cudaGetLastError());
     return REANN_OK;
 }

@@ -132,6 +132,14 @@ void launch_output(const LaunchCtx &ctx, int64_t N, const int32_t *inv_perm, con
 void launch_verlet(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
                    double dt, double acc_unit, int drift);
 
+// ---- md.cu ----
+int md_blocks(int64_t N);
+void launch_md_kick(const LaunchCtx &ctx, int64_t N, double *pos, double *vel, const double *F, const double *inv_mass,
+                    double dt, double acc_unit, int drift, const double *state /* or nullptr */, double *ke_partial /* or nullptr */);
+void launch_nh_update(const LaunchCtx &ctx, int64_t N, const double *ke_partial, double *state, double h, double g_kT,
+                      double Q, double acc_unit, int mode, int nvt);
+void launch_md_scale(const LaunchCtx &ctx, int64_t N, double *vel, const double *state);
+
 // ---- gram.cu / dense.cu ----
 struct DenseTile {
     int32_t species, start, count; // atoms sp_list[start .. start+count) all of `species`

@@ -88,6 +88,11 @@ struct reann {
     int step_state = 0;           // 0 = idle, 1 = after reann_step_begin (forward), 2 = reverse pass started
     bool step_vir = false;
 
+    // ---- device-resident MD (reann_md_run, md.cu) ----
+    DevBuf md_state;              // double [8]: xi, vxi, pending scale, 2 KE, final scale
+    DevBuf md_partial;            // double [N/256 + 1] block partials of sum m v^2
+    DevBuf md_E;                  // double [1] potential energy of the last step
+
     // ---- stats / profiling ----
     int64_t n_rebuilds = 0, n_calls = 0, n_prof_calls = 0;
     bool profiling = false;
