@@ -177,7 +177,7 @@ int reann_verlet(reann_t *h, double *pos, double *vel, const double *F, const do
  * The paper drives its potentials in NVT molecular dynamics at 300 K (MD driver of
  * section 4.2). reann_md_run advances n_steps of velocity Verlet, optionally with a Nose-Hoover
  * thermostat (one thermostat variable; half step before and after every velocity-Verlet step; g = 3 n_atoms degrees of
- * freedom; Q = g kT tau^2 -- the integrator is written out in DESIGN.md section 2, B-7, and in oracle/md.py):
+ * freedom; Q = g kT tau^2 -- the integrator is written out in DESIGN.md section 2, B-8, and in oracle/md.py):
  *   pos, vel [n_atoms][3], inv_mass [n_atoms] (1/amu), F [n_atoms][3], virial [9] or NULL: DEVICE pointers, caller
  *     order; pos and vel are advanced in place, F and virial hold the values at the final positions on return
  *     (F need not be initialised: the forces at the initial positions are evaluated first, unless st->forces_valid

@@ -3,7 +3,7 @@
 Plain NumPy float64 molecular dynamics driver used to check `reann_md_run` (the
 paper runs its potentials in NVT molecular dynamics at 300 K, with the MD
 driver of section 4.2). The paper does not print the integrator (it uses LAMMPS), so the
-reading taken here (B-7) is the textbook one:
+reading taken here (B-8) is the textbook one:
 
   * velocity Verlet:            v += dt/2 a(x);  x += dt v;  a = F(x)/m;  v += dt/2 a(x)
   * Nose-Hoover thermostat (one thermostat variable xi with "velocity" vxi), applied as a half step

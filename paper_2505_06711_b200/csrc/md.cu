@@ -1,6 +1,6 @@
 // md.cu -- device-resident molecular dynamics around the energy/force path: velocity Verlet
 // with a Nose-Hoover thermostat (the paper runs its potentials in NVT MD at 300 K; MD driver
-// of section 4.2). The integrator is the one stated in DESIGN.md section 2, reading B-7:
+// of section 4.2). The integrator is the one stated in DESIGN.md section 2, reading B-8:
 //     thermostat half step,  v += dt/2 a,  x += dt v,  a = F(x) / m,  v += dt/2 a,  thermostat half step
 //     thermostat: dv/dt = -vxi v,  dvxi/dt = (2 KE - g kB T) / Q,  dxi/dt = vxi,  Q = g kB T tau^2,  g = 3 N
 //     half step h = dt/2:  vxi += h/2 G;  v *= exp(-h vxi);  xi += h vxi;  vxi += h/2 G   (G from the current KE)
