@@ -309,19 +309,6 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
     }
 }
 
-// ---- warp-level tensor-core helpers (mma.sync TF32, 3xTF32 splitting) ----
-__device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void split_bits(float x, uint32_t &hi, uint32_t &lo) {
-    // hi rounded to nearest TF32, lo = x - hi exact (<= 13 significant bits, of which the MMA reads the top 11):
-    // |x - hi - lo_read| <= 2^-22 |x|
-    hi = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;
-    lo = __float_as_uint(x - __uint_as_float(hi));
-}
-
 // ------------------------------------------------------------------------------------------ A5 (MMA)
 // Edge forward with the neighbour sum on the tensor cores: b_i[n,a] = sum_e X[e,n] A[e,a] is a
 // (N_phi x edges) x (edges x N_a) product with K = the edges of atom i. Warp per atom, rounds of 32 edges:

@@ -53,6 +53,19 @@ __device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.
 
 __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 
+// ---- warp-level tensor-core helpers (mma.sync TF32, 3xTF32 splitting) ----
+__device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void split_bits(float x, uint32_t &hi, uint32_t &lo) {
+    // hi rounded to nearest TF32, lo = x - hi exact (<= 13 significant bits, of which the MMA reads the top 11):
+    // |x - hi - lo_read| <= 2^-22 |x|
+    hi = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;
+    lo = __float_as_uint(x - __uint_as_float(hi));
+}
+
 struct StashChunk { // reverse gather: kappa holds the edges [e_lo, e_hi); forces once; cbar = or +=
     int64_t e_lo, e_hi;
     int do_forces, accumulate;

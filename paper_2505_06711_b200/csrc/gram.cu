@@ -10,6 +10,7 @@
 // Column q = l * NPp + pair(n, n'), pair(n, n') = n nphi - n (n - 1) / 2 + (n' - n); columns that
 // are padding are written as zeros.
 #include "common.cuh"
+#include "edge_common.cuh"
 
 namespace {
 
@@ -22,6 +23,12 @@ __host__ __device__ constexpr float mu_of(int a) { // l! / (lx! ly! lz!) in the 
 }
 __host__ __device__ constexpr int l_of(int a) { return a >= 10 ? 3 : a >= 4 ? 2 : a >= 1 ? 1 : 0; }
 __constant__ float c_mu[20] = {1, 1, 1, 1, 1, 2, 2, 1, 2, 1, 1, 3, 3, 3, 6, 3, 1, 3, 3, 1};
+
+// hi = x rounded to TF32, lo = (x - hi) rounded to TF32 (nearest; split_bits() leaves lo's low bits to the MMA's truncation)
+__device__ __forceinline__ void split_rn(float x, uint32_t &hi, uint32_t &lo) {
+    hi = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;
+    lo = (__float_as_uint(x - __uint_as_float(hi)) + 0x1000u) & 0xFFFFE000u;
+}
 
 template <int NA>
 __device__ __forceinline__ void load_row(const float *__restrict__ src, float *x) {
@@ -85,37 +92,87 @@ __global__ void __launch_bounds__(GW * 32) k_gram_fwd(int64_t N, const int32_t *
 #pragma unroll
         for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
         __syncwarp();
-        // 2 x 2 blocks of row pairs: block (I <= J) = rows {2I, 2I+1} x {2J, 2J+1}; four rows loaded for (up to)
-        // four products -- half the shared-memory operand traffic of one pair per lane
-        constexpr int NBK = NPHIP / 2, NBLOCKS = NBK * (NBK + 1) / 2;
+        if constexpr (NA == 20) {
+            // Q_l = B_l diag(mu) B_l^T per l on the tensor cores: M = N = rows n (16), K = the monomials of degree l in steps
+            // of 8 (l = 0: 1 of 8 used, l = 1: 3, l = 2: 6, l = 3: 8 + 2). mma.sync m16n8k8 TF32, operands split hi + lo; the
+            // chains are at most two steps long. The B fragments (K = a, N = n') are the A fragment's own registers times
+            // mu_a: column tile j = 0 is rows n' = g (a0, a2), j = 1 rows n' = g + 8 (a1, a3). Shared-memory traffic: four
+            // LDS.32 per K step instead of 80 LDS.128 per atom in the FP32 ALU form this replaces.
+            const int g8 = lane >> 2, t4 = lane & 3;
+            constexpr int NKS = NA == 20 ? 5 : NA == 10 ? 3 : NA == 4 ? 2 : 1;
+            constexpr int KS_A0[5] = {0, 1, 4, 10, 18}, KS_CNT[5] = {1, 3, 6, 8, 2}, KS_L[5] = {0, 1, 2, 3, 3};
+            float acc[LMAX + 1][2][4];
 #pragma unroll
-        for (int j = 0; j < (NBLOCKS + 31) / 32; ++j) {
-            const int bi = lane + 32 * j;
-            if (bi < NBLOCKS) {
-                int I = 0, rem = bi;
-                while (rem >= NBK - I) { rem -= NBK - I; ++I; }
-                const int J = I + rem, n0 = 2 * I, m0 = 2 * J;
-                float s[4][LMAX + 1];                       // (n0,m0) (n0,m1) (n1,m0) (n1,m1)
+            for (int l = 0; l <= LMAX; ++l)
 #pragma unroll
-                for (int k = 0; k < 4; ++k)
+                for (int j = 0; j < 2; ++j) acc[l][j][0] = acc[l][j][1] = acc[l][j][2] = acc[l][j][3] = 0.f;
 #pragma unroll
-                    for (int l = 0; l <= LMAX; ++l) s[k][l] = 0.f;
-                float x0[NA], x1[NA], y0[NA], y1[NA];
-                load_row<NA>(bs + n0 * NA, x0); load_row<NA>(bs + (n0 + 1) * NA, x1);
-                load_row<NA>(bs + m0 * NA, y0); load_row<NA>(bs + (m0 + 1) * NA, y1);
+            for (int ks = 0; ks < NKS; ++ks) {
+                const int a0 = KS_A0[ks] + t4, a1 = a0 + 4;
+                const bool v0 = t4 < KS_CNT[ks], v1 = t4 + 4 < KS_CNT[ks];
+                const bool r0 = g8 < NPHIP, r1 = g8 + 8 < NPHIP;
+                const float x00 = (v0 && r0) ? bs[g8 * NA + a0] : 0.f, x10 = (v0 && r1) ? bs[(g8 + 8) * NA + a0] : 0.f;
+                const float x01 = (v1 && r0) ? bs[g8 * NA + a1] : 0.f, x11 = (v1 && r1) ? bs[(g8 + 8) * NA + a1] : 0.f;
+                const float m0 = v0 ? c_mu[a0] : 0.f, m1 = v1 ? c_mu[a1] : 0.f;
+                uint32_t ah[4], al[4], bh[2][2], bl[2][2];
+                split_rn(x00, ah[0], al[0]); split_rn(x10, ah[1], al[1]);
+                split_rn(x01, ah[2], al[2]); split_rn(x11, ah[3], al[3]);
+                split_rn(m0 * x00, bh[0][0], bl[0][0]); split_rn(m1 * x01, bh[0][1], bl[0][1]);
+                split_rn(m0 * x10, bh[1][0], bl[1][0]); split_rn(m1 * x11, bh[1][1], bl[1][1]);
 #pragma unroll
-                for (int a = 0; a < NA; ++a) {
-                    const float u0 = mu_of(a) * x0[a], u1 = mu_of(a) * x1[a];
-                    s[0][l_of(a)] = fmaf(u0, y0[a], s[0][l_of(a)]); s[1][l_of(a)] = fmaf(u0, y1[a], s[1][l_of(a)]);
-                    s[2][l_of(a)] = fmaf(u1, y0[a], s[2][l_of(a)]); s[3][l_of(a)] = fmaf(u1, y1[a], s[3][l_of(a)]);
+                for (int j = 0; j < 2; ++j) {
+                    if (j == 1 && NPHIP <= 8) continue;
+                    edge::mma_tf32(acc[KS_L[ks]][j], al, bl[j][0], bl[j][1]);      // Q is quadratic in b and feeds E_i: all four
+                    edge::mma_tf32(acc[KS_L[ks]][j], al, bh[j][0], bh[j][1]);      // partial products, smallest first
+                    edge::mma_tf32(acc[KS_L[ks]][j], ah, bl[j][0], bl[j][1]);
+                    edge::mma_tf32(acc[KS_L[ks]][j], ah, bh[j][0], bh[j][1]);
                 }
+            }
+            // C fragment: rows n = g, g + 8; columns n' = 8 j + 2 t, + 1; kept where n <= n' < nphi
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int n = n0 + (k >> 1), m = m0 + (k & 1);
-                    if (n <= m && m < nphi) {                // diagonal block: (n1, m0) is the mirror of (n0, m1)
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int n = g8 + 8 * (c >> 1), m = 8 * j + 2 * t4 + (c & 1);
+                    if (n <= m && m < nphi) {
                         const int pi = n * nphi - (n * (n - 1)) / 2 + (m - n);
 #pragma unroll
-                        for (int l = 0; l <= LMAX; ++l) qs[l * NPp + pi] = s[k][l];
+                        for (int l = 0; l <= LMAX; ++l) qs[l * NPp + pi] = acc[l][j][c];
+                    }
+                }
+        } else {
+            // 2 x 2 blocks of row pairs: block (I <= J) = rows {2I, 2I+1} x {2J, 2J+1}; four rows loaded for (up to)
+            // four products -- half the shared-memory operand traffic of one pair per lane
+            constexpr int NBK = NPHIP / 2, NBLOCKS = NBK * (NBK + 1) / 2;
+#pragma unroll
+            for (int j = 0; j < (NBLOCKS + 31) / 32; ++j) {
+                const int bi = lane + 32 * j;
+                if (bi < NBLOCKS) {
+                    int I = 0, rem = bi;
+                    while (rem >= NBK - I) { rem -= NBK - I; ++I; }
+                    const int J = I + rem, n0 = 2 * I, m0 = 2 * J;
+                    float s[4][LMAX + 1];                       // (n0,m0) (n0,m1) (n1,m0) (n1,m1)
+#pragma unroll
+                    for (int k = 0; k < 4; ++k)
+#pragma unroll
+                        for (int l = 0; l <= LMAX; ++l) s[k][l] = 0.f;
+                    float x0[NA], x1[NA], y0[NA], y1[NA];
+                    load_row<NA>(bs + n0 * NA, x0); load_row<NA>(bs + (n0 + 1) * NA, x1);
+                    load_row<NA>(bs + m0 * NA, y0); load_row<NA>(bs + (m0 + 1) * NA, y1);
+#pragma unroll
+                    for (int a = 0; a < NA; ++a) {
+                        const float u0 = mu_of(a) * x0[a], u1 = mu_of(a) * x1[a];
+                        s[0][l_of(a)] = fmaf(u0, y0[a], s[0][l_of(a)]); s[1][l_of(a)] = fmaf(u0, y1[a], s[1][l_of(a)]);
+                        s[2][l_of(a)] = fmaf(u1, y0[a], s[2][l_of(a)]); s[3][l_of(a)] = fmaf(u1, y1[a], s[3][l_of(a)]);
+                    }
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int n = n0 + (k >> 1), m = m0 + (k & 1);
+                        if (n <= m && m < nphi) {                // diagonal block: (n1, m0) is the mirror of (n0, m1)
+                            const int pi = n * nphi - (n * (n - 1)) / 2 + (m - n);
+#pragma unroll
+                            for (int l = 0; l <= LMAX; ++l) qs[l * NPp + pi] = s[k][l];
+                        }
                     }
                 }
             }
@@ -180,55 +237,123 @@ __global__ void __launch_bounds__(GW * 32, 4) k_gram_bwd(int64_t N, const int32_
         }
     }
     int64_t atom = 0;
-    if (row.p >= 0) {
-        atom = sp_list[row.p];
-        const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
+    if constexpr (NA == 20) {
+        // bbar_l = mu . (G_l B_l) per l on the tensor cores: M = n (16), K = n' (two steps of 8), N = the monomials of degree l
+        // in tiles of 8 (l = 0: 1 of 8 columns used, l = 1: 3, l = 2: 6, l = 3: 8 + 2). A fragments = G_l gathered from the
+        // triangular Qbar row, B fragments = b (row-major in shared memory, no transposed copy), 3xTF32.
+        float *bs = bT;                                  // row-major b_i [n][a] in the first NB floats of the warp's area
+        if (row.p >= 0) {
+            atom = sp_list[row.p];
+            const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
 #pragma unroll
-        for (int f = lane; f < NB / 4; f += 32) {
-            const float4 v = __ldg(bi + f);
-            const float va[4] = {v.x, v.y, v.z, v.w};
+            for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
+        }
+        __syncthreads();
+        if (row.p < 0) return;
+        const int g8 = lane >> 2, t4 = lane & 3;
+        int gi[2][4];
+        float gf[2][4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int e = f * 4 + u;
-                bT[(e % NA) * C::TS + e / NA] = va[u];
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int n = g8 + 8 * (c & 1), m = 8 * k + t4 + 4 * (c >> 1);       // a0 (g, t), a1 (g+8, t), a2 (g, t+4), a3 (g+8, t+4)
+                const int lo = min(n, m), hi = max(n, m);
+                const bool ok = n < nphi && m < nphi;
+                gi[k][c] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
+                gf[k][c] = ok ? (n == m ? 2.0f : 1.0f) : 0.0f;
+            }
+        constexpr int NTL = 5;
+        constexpr int NT_A0[NTL] = {0, 1, 4, 10, 18}, NT_CNT[NTL] = {1, 3, 6, 8, 2}, NT_L[NTL] = {0, 1, 2, 3, 3};
+        uint32_t ah[2][4], al[2][4];
+#pragma unroll
+        for (int nt = 0; nt < NTL; ++nt) {
+            if (nt == 0 || NT_L[nt] != NT_L[nt - 1]) {
+                const float *ql = qs + NT_L[nt] * NPp;
+#pragma unroll
+                for (int k = 0; k < 2; ++k)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) edge::split_bits(ql[gi[k][c]] * gf[k][c], ah[k][c], al[k][c]);
+            }
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+            const int a = NT_A0[nt] + g8;
+            const bool va = g8 < NT_CNT[nt];
+            uint32_t bh[2][2], bl[2][2];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const int r0 = 8 * k + t4, r1 = r0 + 4;
+                edge::split_bits((va && r0 < NPHIP) ? bs[r0 * NA + a] : 0.f, bh[k][0], bl[k][0]);
+                edge::split_bits((va && r1 < NPHIP) ? bs[r1 * NA + a] : 0.f, bh[k][1], bl[k][1]);
+            }
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                if (k == 1 && NPHIP <= 8) continue;
+                edge::mma_tf32(acc, al[k], bh[k][0], bh[k][1]);
+                edge::mma_tf32(acc, ah[k], bl[k][0], bl[k][1]);
+            }
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                if (k == 1 && NPHIP <= 8) continue;
+                edge::mma_tf32(acc, ah[k], bh[k][0], bh[k][1]);
+            }
+            // C fragment: rows n = g, g + 8; columns a = a0 + 2t, + 1
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int n = g8 + 8 * (c >> 1), col = 2 * t4 + (c & 1);
+                if (col < NT_CNT[nt] && n < NPHIP) outs[n * NA + NT_A0[nt] + col] = c_mu[NT_A0[nt] + col] * acc[c];
             }
         }
-    }
-    __syncthreads();
-    if (row.p < 0) return;
-    const int n = lane / C::PARTS, a0 = (lane % C::PARTS) * C::CNT;
-    if (n < NPHIP) {
-        // triangular offsets of G[n, k] and the (1 + delta) factor; 0 for padded rows / columns
-        int idx[NPHIP];
-        float fac[NPHIP];
+    } else {
+        if (row.p >= 0) {
+            atom = sp_list[row.p];
+            const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
 #pragma unroll
-        for (int k = 0; k < NPHIP; ++k) {
-            const int lo = min(n, k), hi = max(n, k);
-            const bool ok = n < nphi && k < nphi;
-            idx[k] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
-            fac[k] = ok ? (k == n ? 2.0f : 1.0f) : 0.0f;
+            for (int f = lane; f < NB / 4; f += 32) {
+                const float4 v = __ldg(bi + f);
+                const float va[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int e = f * 4 + u;
+                    bT[(e % NA) * C::TS + e / NA] = va[u];
+                }
+            }
         }
-        float G[NPHIP];
-        int lcur = -1;
+        __syncthreads();
+        if (row.p < 0) return;
+        const int n = lane / C::PARTS, a0 = (lane % C::PARTS) * C::CNT;
+        if (n < NPHIP) {
+            // triangular offsets of G[n, k] and the (1 + delta) factor; 0 for padded rows / columns
+            int idx[NPHIP];
+            float fac[NPHIP];
 #pragma unroll
-        for (int ai = 0; ai < C::CNT; ++ai) {
-            const int a = a0 + ai;
-            if (a < NA) {
-                const int l = l_of(a);
-                if (l != lcur) {
-                    const float *ql = qs + l * NPp;
+            for (int k = 0; k < NPHIP; ++k) {
+                const int lo = min(n, k), hi = max(n, k);
+                const bool ok = n < nphi && k < nphi;
+                idx[k] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
+                fac[k] = ok ? (k == n ? 2.0f : 1.0f) : 0.0f;
+            }
+            float G[NPHIP];
+            int lcur = -1;
 #pragma unroll
-                    for (int k = 0; k < NPHIP; ++k) G[k] = ql[idx[k]] * fac[k];
-                    lcur = l;
+            for (int ai = 0; ai < C::CNT; ++ai) {
+                const int a = a0 + ai;
+                if (a < NA) {
+                    const int l = l_of(a);
+                    if (l != lcur) {
+                        const float *ql = qs + l * NPp;
+#pragma unroll
+                        for (int k = 0; k < NPHIP; ++k) G[k] = ql[idx[k]] * fac[k];
+                        lcur = l;
+                    }
+                    float s = 0.f;
+#pragma unroll
+                    for (int k4 = 0; k4 < NPHIP / 4; ++k4) {
+                        const float4 v = *reinterpret_cast<const float4 *>(bT + a * C::TS + 4 * k4);
+                        s = fmaf(G[4 * k4], v.x, s); s = fmaf(G[4 * k4 + 1], v.y, s);
+                        s = fmaf(G[4 * k4 + 2], v.z, s); s = fmaf(G[4 * k4 + 3], v.w, s);
+                    }
+                    outs[n * NA + a] = c_mu[a] * s;
                 }
-                float s = 0.f;
-#pragma unroll
-                for (int k4 = 0; k4 < NPHIP / 4; ++k4) {
-                    const float4 v = *reinterpret_cast<const float4 *>(bT + a * C::TS + 4 * k4);
-                    s = fmaf(G[4 * k4], v.x, s); s = fmaf(G[4 * k4 + 1], v.y, s);
-                    s = fmaf(G[4 * k4 + 2], v.z, s); s = fmaf(G[4 * k4 + 3], v.w, s);
-                }
-                outs[n * NA + a] = c_mu[a] * s;
             }
         }
     }
