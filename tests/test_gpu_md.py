@@ -20,10 +20,10 @@ def R():
     return R
 
 
-def setup(cfg, speed):
+def setup(cfg, speed, fscale=1e-3):
     # forces enter the integrator scaled by 1e-3 (the random-weight potential has close contacts with |F| of
     # hundreds of eV/A; see test_md_trajectory_config2) -- the same acc_unit on both sides
-    acc = 1e-3 * gen.configs.ACC_UNIT
+    acc = fscale * gen.configs.ACC_UNIT
     vel = gen.maxwell_boltzmann(cfg["masses"], 300.0, cfg["seed_vel"]) * speed
     force_fn = lambda p: (lambda r: (r["E"], r["F"]))(oracle.energy_forces(cfg["blob"], cfg["species"], p, cfg["box"]))
     return acc, vel, force_fn
@@ -62,6 +62,32 @@ def test_md_run_matches_oracle_driver(R, mode):
         assert ref["KE"] < 0.9 * ke0          # the thermostat did act
     else:
         assert st["xi"] == 0.0 and st["vxi"] == 0.0
+    m.close()
+
+
+def test_config2_protocol_100_steps_300K(R):
+    """BASELINE.json config 2: 1024 H2O, 100 velocity-Verlet steps of 0.5 fs from a seeded Maxwell-Boltzmann start at
+    300 K, skin-triggered rebuilds inside the run; the whole trajectory against the oracle driver (same scaled
+    acc_unit on both sides, see setup())."""
+    import torch
+    cfg = gen.make_config(2)
+    n = len(cfg["pos"])
+    # forces scaled by 1e-4 as in bench.py: displacements stay thermal (with 1e-3 the close contacts of the random-weight
+    # potential fling atoms 4 A within 50 fs and the trajectory is no longer comparable)
+    acc, vel0, force_fn = setup(cfg, 1.0, 1e-4)
+    ref = omd.md_run(force_fn, cfg["pos"], vel0, cfg["masses"], 100, 0.5, acc)
+    m = R.Reann.from_config(cfg)
+    pos = torch.tensor(cfg["pos"], device="cuda"); vel = torch.tensor(vel0, device="cuda")
+    inv_m = torch.tensor(1.0 / cfg["masses"], device="cuda")
+    F = torch.zeros((n, 3), dtype=torch.float64, device="cuda")
+    st = m.md_run(pos, vel, inv_m, cfg["box"], 100, 0.5, acc, F=F)
+    disp = np.sqrt(((ref["pos"] - cfg["pos"]) ** 2).sum(1)).max()
+    dp = np.abs(pos.cpu().numpy() - ref["pos"]).max(); dv = np.abs(vel.cpu().numpy() - ref["vel"]).max()
+    dF = np.abs(F.cpu().numpy() - ref["F"]).max()
+    print(f"[md cfg2] 100 steps: max displacement {disp:.2f} A, rebuilds {st['n_rebuilds']}, max|dpos|={dp:.2e} max|dvel|={dv:.2e} max|dF|={dF:.2e}")
+    assert disp > 0.5 * cfg["skin"] and st["n_rebuilds"] >= 2       # the initial build and at least one triggered by the skin rule
+    assert dp < 1e-5 and dv < 1e-6 and dF < 5e-4
+    assert abs(st["potential"] - ref["PE"]) < 1e-6 * n * max(1.0, abs(ref["PE"]) / n)
     m.close()
 
 
