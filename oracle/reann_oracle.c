@@ -118,69 +118,96 @@ static int model_parse(model_t *m, const void *blob, size_t nbytes) {
 /* ------------------------------------------------------------------------------------------
  * Edges (readings A-12, A-13, A-15)
  *   E = {(i, j, S): S in Z^3, (j,S) != (i,0), |r_j + S o box - r_i| < R}, strict "<" on d^2,
- *   arithmetic: wrap x <- x - floor(x/L) L; d = (x_j - x_i) + S L; d2 = (dx dx + dy dy) + dz dz.
+ *   arithmetic: wrap x <- x - floor(x/L) L; d = (x_j - x_i) + S L; d2 = (dx dx + dy dy) + dz dz (orthorhombic box;
+ *   the triclinic form is written out at wrap_all() and pair_test()).
  * ---------------------------------------------------------------------------------------- */
 typedef struct { int32_t j; int32_t S[3]; double d[3]; } edge_t;
 typedef struct { int64_t n; int64_t *off; edge_t *e; double *xw; int32_t *w; } edges_t;
 
 static void edges_free(edges_t *E) { free(E->off); free(E->e); free(E->xw); free(E->w); memset(E, 0, sizeof(*E)); }
 
-static int box_lengths(const double *box9, double Lb[3]) {
-    for (int r = 0; r < 3; ++r)
-        for (int c = 0; c < 3; ++c)
-            if (r != c && box9[3 * r + c] != 0.0) return ORC_ERR_UNSUPPORTED; /* orthorhombic only */
-    for (int d = 0; d < 3; ++d) { Lb[d] = box9[4 * d]; if (!(Lb[d] > 0)) return ORC_ERR_BOX; }
+/* Box: row-major lattice vectors a = box9[0..2], b = box9[3..5], c = box9[6..8] in the lower-triangular form
+ * a = (ax, 0, 0), b = (bx, by, 0), c = (cx, cy, cz) with ax, by, cz > 0 (orthorhombic: bx = cx = cy = 0; any cell can be
+ * brought to this form by a rotation). H = {ax, bx, by, cx, cy, cz}; wd[d] = distance between the two faces of the cell
+ * that are spanned by the other two lattice vectors: images with S in {-1,0,1}^3 of WRAPPED atoms are enough when
+ * every wd[d] >= R (a point within R of the cell is less than one period away in every fractional coordinate). */
+static int box_params(const double *box9, double H[6], double wd[3]) {
+    if (box9[1] != 0.0 || box9[2] != 0.0 || box9[5] != 0.0) return ORC_ERR_UNSUPPORTED; /* not lower-triangular */
+    H[0] = box9[0]; H[1] = box9[3]; H[2] = box9[4]; H[3] = box9[6]; H[4] = box9[7]; H[5] = box9[8];
+    if (!(H[0] > 0) || !(H[2] > 0) || !(H[5] > 0)) return ORC_ERR_BOX;
+    const double ax = H[0], bx = H[1], by = H[2], cx = H[3], cy = H[4], cz = H[5];
+    const double n0 = by * cz, n1 = -bx * cz, n2 = bx * cy - by * cx;       /* b x c */
+    wd[0] = ax * by * cz / sqrt(n0 * n0 + n1 * n1 + n2 * n2);
+    wd[1] = by * cz / sqrt(cy * cy + cz * cz);                                /* a x c = (0, -ax cz, ax cy) */
+    wd[2] = cz;
     return ORC_OK;
 }
 
-static void wrap_all(const double *pos, int64_t N, const double Lb[3], double *xw, int32_t *w) {
-    for (int64_t i = 0; i < N; ++i)
-        for (int d = 0; d < 3; ++d) {
-            double f = floor(pos[3 * i + d] / Lb[d]);
-            w[3 * i + d] = (int32_t)f;
-            xw[3 * i + d] = pos[3 * i + d] - f * Lb[d];
-        }
+/* Wrapping (reading A-15, extended to a triclinic cell in DESIGN.md B-9): fractional coordinates by back substitution,
+ *   sc = z / cz;  sb = (y - sc cy) / by;  sa = ((x - sb bx) - sc cx) / ax;   w = floor(s)  (whole periods, per lattice vector)
+ * and the wrapped position is x - ((wa ax + wb bx) + wc cx), y - (wb by + wc cy), z - wc cz. For an orthorhombic box
+ * this is x - floor(x / L) L, bit for bit. */
+static void wrap_all(const double *pos, int64_t N, const double H[6], double *xw, int32_t *w) {
+    const double ax = H[0], bx = H[1], by = H[2], cx = H[3], cy = H[4], cz = H[5];
+    for (int64_t i = 0; i < N; ++i) {
+        const double x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+        const double sc = z / cz;
+        const double sb = (y - sc * cy) / by;
+        const double sa = ((x - sb * bx) - sc * cx) / ax;
+        const double fa = floor(sa), fb = floor(sb), fc = floor(sc);
+        w[3 * i] = (int32_t)fa; w[3 * i + 1] = (int32_t)fb; w[3 * i + 2] = (int32_t)fc;
+        xw[3 * i] = x - ((fa * ax + fb * bx) + fc * cx);
+        xw[3 * i + 1] = y - (fb * by + fc * cy);
+        xw[3 * i + 2] = z - fc * cz;
+    }
 }
 
-static inline int pair_test(const double *xi, const double *xj, const int S[3], const double Lb[3],
+/* d = (x_j - x_i) + S . box with S . box = ((S0 ax + S1 bx) + S2 cx, S1 by + S2 cy, S2 cz) */
+static inline int pair_test(const double *xi, const double *xj, const int S[3], const double H[6],
                             double R2, double d[3]) {
-    d[0] = (xj[0] - xi[0]) + S[0] * Lb[0];
-    d[1] = (xj[1] - xi[1]) + S[1] * Lb[1];
-    d[2] = (xj[2] - xi[2]) + S[2] * Lb[2];
+    d[0] = (xj[0] - xi[0]) + ((S[0] * H[0] + S[1] * H[1]) + S[2] * H[3]);
+    d[1] = (xj[1] - xi[1]) + (S[1] * H[2] + S[2] * H[4]);
+    d[2] = (xj[2] - xi[2]) + S[2] * H[5];
     double d2 = (d[0] * d[0] + d[1] * d[1]) + d[2] * d[2];
     return d2 < R2;
 }
 
-/* mode 0: O(N^2 * 27) brute force over S in {-1,0,1}^3; mode 1: cell list. Both need L_d >= R.
+/* mode 0: O(N^2 * 27) brute force over S in {-1,0,1}^3; mode 1: cell list (cells in fractional coordinates, at least R
+ * wide between their faces). Both need wd[d] >= R.
  * sel == NULL: rows of all N atoms (row k = atom k); else rows of the n_sel atoms sel[k] only (row k = atom
  * sel[k]; the same pair test over the same candidates -- used for sampled pair-set parity on systems whose
  * full list would not fit the host). */
 static int build_edges_sel(const double *pos, int64_t N, const double *box9, double R, int mode, edges_t *E,
                            const int64_t *sel, int64_t n_sel) {
     memset(E, 0, sizeof(*E));
-    double Lb[3];
-    int rc_ = box_lengths(box9, Lb);
+    double H[6], wd[3];
+    int rc_ = box_params(box9, H, wd);
     if (rc_) return rc_;
-    for (int d = 0; d < 3; ++d) if (Lb[d] < R) return ORC_ERR_BOX;
+    for (int d = 0; d < 3; ++d) if (wd[d] < R) return ORC_ERR_BOX;
     const double R2 = R * R;
     E->xw = malloc(sizeof(double) * 3 * (size_t)(N > 0 ? N : 1));
     E->w = malloc(sizeof(int32_t) * 3 * (size_t)(N > 0 ? N : 1));
     const int64_t n_rows = sel ? n_sel : N;
     E->off = calloc((size_t)n_rows + 1, sizeof(int64_t));
     if (!E->xw || !E->w || !E->off) return ORC_ERR_MEM;
-    wrap_all(pos, N, Lb, E->xw, E->w);
+    wrap_all(pos, N, H, E->xw, E->w);
     int nc[3]; int64_t ncell = 1;
     int32_t *cell_of = NULL; int64_t *cstart = NULL; int32_t *catoms = NULL;
     if (mode == 1) {
-        for (int d = 0; d < 3; ++d) { nc[d] = (int)floor(Lb[d] / R); if (nc[d] < 1) nc[d] = 1; ncell *= nc[d]; }
+        for (int d = 0; d < 3; ++d) { nc[d] = (int)floor(wd[d] / R); if (nc[d] < 1) nc[d] = 1; ncell *= nc[d]; }
         cell_of = malloc(sizeof(int32_t) * 3 * (size_t)(N > 0 ? N : 1));
         cstart = calloc((size_t)ncell + 1, sizeof(int64_t));
         catoms = malloc(sizeof(int32_t) * (size_t)(N > 0 ? N : 1));
         if (!cell_of || !cstart || !catoms) return ORC_ERR_MEM;
         for (int64_t i = 0; i < N; ++i) {
             int64_t lin = 0;
+            /* fractional coordinates of the wrapped position: x = sa a + sb b + sc c */
+            double sf[3];
+            sf[2] = E->xw[3 * i + 2] / H[5];
+            sf[1] = (E->xw[3 * i + 1] - sf[2] * H[4]) / H[2];
+            sf[0] = ((E->xw[3 * i] - sf[1] * H[1]) - sf[2] * H[3]) / H[0];
             for (int d = 0; d < 3; ++d) {
-                int c = (int)(E->xw[3 * i + d] / (Lb[d] / nc[d]));
+                int c = (int)floor(sf[d] * nc[d]);
                 if (c >= nc[d]) c = nc[d] - 1;
                 if (c < 0) c = 0;
                 cell_of[3 * i + d] = c;
@@ -219,7 +246,7 @@ static int build_edges_sel(const double *pos, int64_t N, const double *box9, dou
                     for (int sx = -1; sx <= 1; ++sx) for (int sy = -1; sy <= 1; ++sy) for (int sz = -1; sz <= 1; ++sz) {
                         if (j == i && sx == 0 && sy == 0 && sz == 0) continue;
                         int S[3] = {sx, sy, sz};
-                        if (pair_test(xi, E->xw + 3 * j, S, Lb, R2, d)) {
+                        if (pair_test(xi, E->xw + 3 * j, S, H, R2, d)) {
                             if (pass == 1) { edge_t *e = &E->e[base + cnt]; e->j = (int32_t)j;
                                 e->S[0] = sx; e->S[1] = sy; e->S[2] = sz; e->d[0] = d[0]; e->d[1] = d[1]; e->d[2] = d[2]; }
                             ++cnt;
@@ -237,7 +264,7 @@ static int build_edges_sel(const double *pos, int64_t N, const double *box9, dou
                     for (int64_t q = cstart[lin]; q < cstart[lin + 1]; ++q) {
                         int64_t j = catoms[q];
                         if (j == i && S[0] == 0 && S[1] == 0 && S[2] == 0) continue;
-                        if (pair_test(xi, E->xw + 3 * j, S, Lb, R2, d)) {
+                        if (pair_test(xi, E->xw + 3 * j, S, H, R2, d)) {
                             if (pass == 1) { edge_t *e = &E->e[base + cnt]; e->j = (int32_t)j;
                                 e->S[0] = S[0]; e->S[1] = S[1]; e->S[2] = S[2]; e->d[0] = d[0]; e->d[1] = d[1]; e->d[2] = d[2]; }
                             ++cnt;
