@@ -114,8 +114,13 @@ def _calib_table() -> dict:
 
 def make_config(k: int, T: int | None = None, n_mol: int | None = None, ncell: int | None = None,
                 geometry_only: bool = False, gains: dict | None = None, radial_jitter: float = 0.0,
-                n_species: int | None = None) -> dict:
+                n_species: int | None = None, tilt: tuple | None = None) -> dict:
     """Build config k. Overrides (T, n_mol, ncell) give same-density replicas / the T sweep.
+
+    tilt = (xy, xz, yz) in Angstrom (tests of the triclinic path, NEXT-4): lattice vectors a = (Lx, 0, 0),
+    b = (xy, Ly, 0), c = (xz, yz, Lz). Water: the molecules' fractional coordinates are kept, so the density is that of
+    the orthorhombic recipe; fcc: the Cartesian positions are kept (choose tilts that are multiples of the lattice
+    constant to describe the same crystal).
 
     radial_jitter > 0 (tests only): per-(layer, species) radial tables, see make_weights.
 
@@ -150,7 +155,14 @@ def make_config(k: int, T: int | None = None, n_mol: int | None = None, ncell: i
         if S > 1:
             species = np.random.default_rng(seed_g + 500).integers(0, S, len(pos)).astype(np.int32)
         masses = np.full(len(pos), MASS["M"])
-    out = dict(k=k, name=r["name"], pos=pos, species=species, box=np.diag(box).reshape(9).copy(),
+    box9 = np.diag(box).reshape(9).copy()
+    if tilt is not None:
+        box9[3], box9[6], box9[7] = float(tilt[0]), float(tilt[1]), float(tilt[2])
+        if r["kind"] in ("water", "slab"):
+            centre = pos.reshape(-1, 3, 3)[:, :1, :]                   # the O site carries the molecule
+            moved = (centre / box) @ box9.reshape(3, 3)
+            pos = (pos.reshape(-1, 3, 3) - centre + moved).reshape(-1, 3)
+    out = dict(k=k, name=r["name"], pos=pos, species=species, box=box9,
                masses=masses, rc=r["rc"], skin=r["skin"], T=r["T"], L=r["L"], n_gauss=r["n_gauss"],
                H=r["H"], S=S, nbar=r["nbar"], n_orb=n_orb_default(r["n_gauss"], r["L"]),
                seed_vel=3000 + k)

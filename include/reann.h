@@ -10,9 +10,12 @@
  *  - Units: Angstrom, eV, eV/Angstrom.
  *  - `pos`, `E`, `F`, `virial`, `species`, `weights` may each be HOST or DEVICE pointers
  *    (detected with cudaPointerGetAttributes). `box` is always a HOST pointer to 9 doubles:
- *    row-major lattice vectors; only orthorhombic boxes (off-diagonals exactly 0) are
- *    supported and every box length must be >= rc + skin (so only images -1,0,+1 occur).
- *    Positions need not be wrapped into the box.
+ *    row-major lattice vectors a = box[0..2], b = box[3..5], c = box[6..8] in lower-triangular form,
+ *    a = (ax, 0, 0), b = (bx, by, 0), c = (cx, cy, cz) with ax, by, cz > 0 (orthorhombic: bx = cx = cy = 0;
+ *    any triclinic cell can be rotated into this form). The distance between opposite faces of the cell
+ *    must be >= rc + skin in all three directions (so only images -1,0,+1 of the wrapped atoms occur);
+ *    entries box[1], box[2], box[5] other than 0 give REANN_ERR_UNSUPPORTED. Positions need not be
+ *    wrapped into the cell. The pair test is FP64 with the operation order of DESIGN.md A-15 / B-9.
  *  - Ownership: the caller owns every array it passes; the library copies what it keeps
  *    (weights, species) and never retains caller pointers past the call.
  *  - Synchronisation: reann_energy_forces enqueues the whole evaluation on the handle's stream
@@ -58,7 +61,7 @@ enum {
     REANN_ERR_NO_NEIGHBORS = 4, /* reann_energy_forces before any reann_build_neighbors */
     REANN_ERR_CUDA = 5,         /* a CUDA runtime call failed (text in last_error)      */
     REANN_ERR_OOM = 6,          /* device allocation failed                             */
-    REANN_ERR_UNSUPPORTED = 7   /* triclinic box, n_gauss > 16, L > 3, row too long ... */
+    REANN_ERR_UNSUPPORTED = 7   /* lattice not lower-triangular, n_gauss > 16, L > 3, row too long ... */
 };
 
 /*

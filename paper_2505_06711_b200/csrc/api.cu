@@ -388,12 +388,15 @@ extern "C" int reann_set_profiling(reann_t *h, int on) {
 
 static int check_box(reann *h, const double *box9) {
     if (!box9) return set_err(h, REANN_ERR_ARG, "box is NULL");
-    for (int r = 0; r < 3; ++r)
-        for (int c = 0; c < 3; ++c)
-            if (r != c && box9[3 * r + c] != 0.0) return set_err(h, REANN_ERR_UNSUPPORTED, "only orthorhombic boxes are supported");
-    const double R = h->md.rc + h->md.skin;
+    if (box9[1] != 0.0 || box9[2] != 0.0 || box9[5] != 0.0)
+        return set_err(h, REANN_ERR_UNSUPPORTED, "lattice vectors must be in lower-triangular form: a = (ax,0,0), b = (bx,by,0), c = (cx,cy,cz)");
+    if (!(box9[0] > 0.0) || !(box9[4] > 0.0) || !(box9[8] > 0.0)) return set_err(h, REANN_ERR_BOX, "ax, by, cz must be positive");
+    if (h->have_halo && (box9[3] != 0.0 || box9[6] != 0.0 || box9[7] != 0.0))
+        return set_err(h, REANN_ERR_UNSUPPORTED, "decomposed runs (reann_set_halo) take orthorhombic boxes only");
+    const BoxP B = make_boxp(box9);
+    const double R = h->md.rc + h->md.skin, wd[3] = {B.wa, B.wb, B.wc};
     for (int d = 0; d < 3; ++d)
-        if (!(box9[4 * d] >= R)) return set_err(h, REANN_ERR_BOX, "box length %g < rc + skin = %g", box9[4 * d], R);
+        if (!(wd[d] >= R)) return set_err(h, REANN_ERR_BOX, "distance %g between the cell faces along lattice vector %d < rc + skin = %g", wd[d], d, R);
     return REANN_OK;
 }
 
@@ -501,15 +504,15 @@ __global__ void k_cap_check(const int64_t *__restrict__ n_rc, int64_t cap, int32
 static int enqueue_prep(reann *h, const double *d_pos) {
     LaunchCtx ctx = h->ctx();
     const int64_t N = h->N;
-    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
+    const BoxP B = make_boxp(h->box_build);
     int32_t *flags = (int32_t *)h->flags.p;
     CU(h, cudaMemsetAsync(flags, 0, 16, h->stream));
     const double thr = 0.5 * h->md.skin;
     launch_skin_check(ctx, d_pos, (const double *)h->pos_build.p, N, thr * thr, flags);
     launch_refresh(ctx, (XRec *)h->xrec.p, h->n_ext, (const int32_t *)h->perm.p, (const int32_t *)h->wshift.p, d_pos,
-                   Lx, Ly, Lz, (float *)h->c_ext.p, (const float *)h->c0.p, h->md.nphip);
-    launch_filter_count(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p, N, Lx,
-                        Ly, Lz, h->md.rc * h->md.rc, (uint16_t *)h->rank16.p, (int32_t *)h->rc_cnt.p);
+                   B, (float *)h->c_ext.p, (const float *)h->c0.p, h->md.nphip);
+    launch_filter_count(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p, N, B,
+                        h->md.rc * h->md.rc, (uint16_t *)h->rank16.p, (int32_t *)h->rc_cnt.p);
     exclusive_scan_i32_to_i64(ctx, (const int32_t *)h->rc_cnt.p, (int64_t *)h->rc_ptr.p, N, h->scan_ws.p);
     LAUNCH(ctx, k_cap_check, 1, 1, 0, (const int64_t *)h->rc_ptr.p + N, h->cap_rc, flags, (int64_t *)(flags + 2));
     return REANN_OK;
@@ -565,9 +568,9 @@ static LayerPtrs layer_ptrs(reann *h) {
 }
 
 static void enqueue_filter_fill(reann *h, const LaunchCtx &ctx) {
-    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
+    const BoxP B = make_boxp(h->box_build);
     launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
-                       (const uint32_t *)h->rev.p, h->N, Lx, Ly, Lz, (const uint16_t *)h->rank16.p,
+                       (const uint32_t *)h->rev.p, h->N, B, (const uint16_t *)h->rank16.p,
                        (const int64_t *)h->rc_ptr.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
 }
 

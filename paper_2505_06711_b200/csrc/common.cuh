@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <math.h>
 
 #include <string>
 #include <vector>
@@ -32,6 +33,38 @@ static_assert(sizeof(XRec) == 32, "XRec must be 32 bytes");
 
 // shift code 0..26 = (sx+1)*9 + (sy+1)*3 + (sz+1); 13 = no shift; reverse code = 26 - code
 __host__ __device__ inline int shift_code(int sx, int sy, int sz) { return (sx + 1) * 9 + (sy + 1) * 3 + (sz + 1); }
+
+// Periodic cell in the lower-triangular form of include/reann.h: a = (ax, 0, 0), b = (bx, by, 0), c = (cx, cy, cz);
+// orthorhombic: bx = cx = cy = 0. wa / wb / wc = distance between the two faces spanned by the other two vectors.
+// The arithmetic below is the reading B-9 of DESIGN.md (A-15 extended): FP64, round to nearest, no contraction, in
+// exactly this order -- the r < R decisions of the neighbour list depend on it bit for bit. For an orthorhombic cell
+// every expression reduces to the x - floor(x / L) L and (x_j - x_i) + S L of A-15 with the same bits.
+struct BoxP {
+    double ax, bx, by, cx, cy, cz;
+    double wa, wb, wc;
+};
+inline BoxP make_boxp(const double *box9) {
+    BoxP B{box9[0], box9[3], box9[4], box9[6], box9[7], box9[8], 0, 0, 0};
+    const double n0 = B.by * B.cz, n1 = -B.bx * B.cz, n2 = B.bx * B.cy - B.by * B.cx;      // b x c
+    B.wa = B.ax * B.by * B.cz / sqrt(n0 * n0 + n1 * n1 + n2 * n2);
+    B.wb = B.by * B.cz / sqrt(B.cy * B.cy + B.cz * B.cz);
+    B.wc = B.cz;
+    return B;
+}
+#ifdef __CUDACC__
+// fractional coordinates by back substitution: x = sa a + sb b + sc c
+__device__ __forceinline__ void box_frac(const BoxP &B, double x, double y, double z, double &sa, double &sb, double &sc) {
+    sc = __ddiv_rn(z, B.cz);
+    sb = __ddiv_rn(__dsub_rn(y, __dmul_rn(sc, B.cy)), B.by);
+    sa = __ddiv_rn(__dsub_rn(__dsub_rn(x, __dmul_rn(sb, B.bx)), __dmul_rn(sc, B.cx)), B.ax);
+}
+// S . box for whole periods (sa, sb, sc): ((sa ax + sb bx) + sc cx, sb by + sc cy, sc cz)
+__device__ __forceinline__ void box_shift(const BoxP &B, double sa, double sb, double sc, double &hx, double &hy, double &hz) {
+    hx = __dadd_rn(__dadd_rn(__dmul_rn(sa, B.ax), __dmul_rn(sb, B.bx)), __dmul_rn(sc, B.cx));
+    hy = __dadd_rn(__dmul_rn(sb, B.by), __dmul_rn(sc, B.cy));
+    hz = __dmul_rn(sc, B.cz);
+}
+#endif
 
 // col_rc entries carry the neighbour's species in the top 5 bits (S <= 32, N_ext < 2^27)
 #define COL_IDX_MASK 0x07FFFFFFu
@@ -108,11 +141,11 @@ int neighbor_export_rows(reann *h, int64_t n_sel, const int64_t *atoms, int64_t 
 void launch_skin_check(const LaunchCtx &ctx, const double *pos, const double *pos_build, int64_t N, double thr2,
                        int32_t *flag);
 void launch_refresh(const LaunchCtx &ctx, XRec *xrec, int64_t n_ext, const int32_t *perm, const int32_t *wshift,
-                    const double *pos, double Lx, double Ly, double Lz, float *c_ext0, const float *c0, int nphip);
+                    const double *pos, const BoxP &box, float *c_ext0, const float *c0, int nphip);
 void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
-                         int64_t N, double Lx, double Ly, double Lz, double rc2, uint16_t *rank16, int32_t *rc_cnt);
+                         int64_t N, const BoxP &box, double rc2, uint16_t *rank16, int32_t *rc_cnt);
 void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
-                        const uint32_t *rev, int64_t N, double Lx, double Ly, double Lz, const uint16_t *rank16,
+                        const uint32_t *rev, int64_t N, const BoxP &box, const uint16_t *rank16,
                         const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc);
 void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip);
 int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,

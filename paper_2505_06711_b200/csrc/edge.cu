@@ -40,32 +40,34 @@ __global__ void k_skin_check(const double *__restrict__ pos, const double *__res
 
 // positions of all ext atoms in the build-time wrapped frame; layer-0 coefficients c^0 = c0[species]
 __global__ void k_refresh(XRec *__restrict__ xrec, int64_t n_ext, const int32_t *__restrict__ perm,
-                          const int32_t *__restrict__ wshift, const double *__restrict__ pos, double Lx, double Ly,
-                          double Lz, float *__restrict__ c_ext0, const float *__restrict__ c0, int nphip) {
+                          const int32_t *__restrict__ wshift, const double *__restrict__ pos, BoxP B,
+                          float *__restrict__ c_ext0, const float *__restrict__ c0, int nphip) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_ext) return;
     XRec r = xrec[k];
     const int64_t i = perm[r.owner];
-    r.x = __dsub_rn(pos[3 * i], __dmul_rn((double)wshift[3 * i], Lx));
-    r.y = __dsub_rn(pos[3 * i + 1], __dmul_rn((double)wshift[3 * i + 1], Ly));
-    r.z = __dsub_rn(pos[3 * i + 2], __dmul_rn((double)wshift[3 * i + 2], Lz));
+    double hx, hy, hz;
+    box_shift(B, (double)wshift[3 * i], (double)wshift[3 * i + 1], (double)wshift[3 * i + 2], hx, hy, hz);
+    r.x = __dsub_rn(pos[3 * i], hx);
+    r.y = __dsub_rn(pos[3 * i + 1], hy);
+    r.z = __dsub_rn(pos[3 * i + 2], hz);
     xrec[k] = r;
     for (int n = 0; n < nphip; ++n) c_ext0[k * nphip + n] = c0[r.species * nphip + n];
 }
 
-__device__ __forceinline__ double edge_d2(const XRec &me, const XRec &o, double Lx, double Ly, double Lz, double *dx,
-                                          double *dy, double *dz) {
-    *dx = __dadd_rn(__dsub_rn(o.x, me.x), __dmul_rn((double)o.sx, Lx));
-    *dy = __dadd_rn(__dsub_rn(o.y, me.y), __dmul_rn((double)o.sy, Ly));
-    *dz = __dadd_rn(__dsub_rn(o.z, me.z), __dmul_rn((double)o.sz, Lz));
+__device__ __forceinline__ double edge_d2(const XRec &me, const XRec &o, const BoxP &B, double *dx, double *dy, double *dz) {
+    double hx, hy, hz;
+    box_shift(B, (double)o.sx, (double)o.sy, (double)o.sz, hx, hy, hz);
+    *dx = __dadd_rn(__dsub_rn(o.x, me.x), hx);
+    *dy = __dadd_rn(__dsub_rn(o.y, me.y), hy);
+    *dz = __dadd_rn(__dsub_rn(o.z, me.z), hz);
     return __dadd_rn(__dadd_rn(__dmul_rn(*dx, *dx), __dmul_rn(*dy, *dy)), __dmul_rn(*dz, *dz));
 }
 
 // rc-filter, pass 1: rank of every accepted list entry inside its row (0xFFFF = rejected)
 __global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict__ xrec,
                                                           const int64_t *__restrict__ row_ptr,
-                                                          const int32_t *__restrict__ col, int64_t N, double Lx,
-                                                          double Ly, double Lz, double rc2,
+                                                          const int32_t *__restrict__ col, int64_t N, BoxP B, double rc2,
                                                           uint16_t *__restrict__ rank16, int32_t *__restrict__ rc_cnt) {
     const int lane = threadIdx.x & 31;
     const int64_t i = (int64_t)blockIdx.x * EW + (threadIdx.x >> 5);
@@ -83,8 +85,8 @@ __global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict
         if (e0 < r1) o0 = xrec[j0];
         if (e1 < r1) o1 = xrec[j1];
         double dx, dy, dz;
-        const bool in0 = e0 < r1 && edge_d2(me, o0, Lx, Ly, Lz, &dx, &dy, &dz) < rc2;
-        const bool in1 = e1 < r1 && edge_d2(me, o1, Lx, Ly, Lz, &dx, &dy, &dz) < rc2;
+        const bool in0 = e0 < r1 && edge_d2(me, o0, B, &dx, &dy, &dz) < rc2;
+        const bool in1 = e1 < r1 && edge_d2(me, o1, B, &dx, &dy, &dz) < rc2;
         const unsigned m0 = __ballot_sync(0xffffffffu, in0), m1 = __ballot_sync(0xffffffffu, in1);
         if (e0 < r1) rank16[e0] = in0 ? (uint16_t)(cnt + __popc(m0 & ((1u << lane) - 1))) : (uint16_t)0xFFFF;
         cnt += __popc(m0);
@@ -99,8 +101,8 @@ __global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict
 __global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict__ xrec,
                                                          const int64_t *__restrict__ row_ptr,
                                                          const int32_t *__restrict__ col,
-                                                         const uint32_t *__restrict__ rev, int64_t N, double Lx,
-                                                         double Ly, double Lz, const uint16_t *__restrict__ rank16,
+                                                         const uint32_t *__restrict__ rev, int64_t N, BoxP B,
+                                                         const uint16_t *__restrict__ rank16,
                                                          const int64_t *__restrict__ rc_ptr,
                                                          uint32_t *__restrict__ col_rc, float4 *__restrict__ geom,
                                                          uint32_t *__restrict__ rev_rc, const int32_t *__restrict__ skip) {
@@ -137,7 +139,7 @@ __global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict_
         for (int u = 0; u < U; ++u)
             if (rk[u] != 0xFFFF) {
                 double dx, dy, dz;
-                const double d2 = edge_d2(me, o[u], Lx, Ly, Lz, &dx, &dy, &dz);
+                const double d2 = edge_d2(me, o[u], B, &dx, &dy, &dz);
                 const int64_t ce = c0 + rk[u];
                 col_rc[ce] = (uint32_t)j[u] | ((uint32_t)o[u].species << COL_SPECIES_SHIFT);
                 geom[ce] = make_float4((float)dx, (float)dy, (float)dz, (float)sqrt(d2));
@@ -841,17 +843,17 @@ void launch_skin_check(const LaunchCtx &ctx, const double *pos, const double *po
     if (N > 0) LAUNCH(ctx, k_skin_check, div_up(N, 256), 256, 0, pos, pos_build, 3 * N, thr2, flag);
 }
 void launch_refresh(const LaunchCtx &ctx, XRec *xrec, int64_t n_ext, const int32_t *perm, const int32_t *wshift,
-                    const double *pos, double Lx, double Ly, double Lz, float *c_ext0, const float *c0, int nphip) {
-    if (n_ext > 0) LAUNCH(ctx, k_refresh, div_up(n_ext, 256), 256, 0, xrec, n_ext, perm, wshift, pos, Lx, Ly, Lz, c_ext0, c0, nphip);
+                    const double *pos, const BoxP &box, float *c_ext0, const float *c0, int nphip) {
+    if (n_ext > 0) LAUNCH(ctx, k_refresh, div_up(n_ext, 256), 256, 0, xrec, n_ext, perm, wshift, pos, box, c_ext0, c0, nphip);
 }
 void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
-                         int64_t N, double Lx, double Ly, double Lz, double rc2, uint16_t *rank16, int32_t *rc_cnt) {
-    if (N > 0) LAUNCH(ctx, k_filter_count, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, N, Lx, Ly, Lz, rc2, rank16, rc_cnt);
+                         int64_t N, const BoxP &box, double rc2, uint16_t *rank16, int32_t *rc_cnt) {
+    if (N > 0) LAUNCH(ctx, k_filter_count, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, N, box, rc2, rank16, rc_cnt);
 }
 void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
-                        const uint32_t *rev, int64_t N, double Lx, double Ly, double Lz, const uint16_t *rank16,
+                        const uint32_t *rev, int64_t N, const BoxP &box, const uint16_t *rank16,
                         const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc) {
-    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, rev, N, Lx, Ly, Lz, rank16, rc_ptr, col_rc, geom, rev_rc, ctx.skip);
+    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, rev, N, box, rank16, rc_ptr, col_rc, geom, rev_rc, ctx.skip);
 }
 void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip) {
     const int64_t work = (n_ext - N) * (nphip / 4);

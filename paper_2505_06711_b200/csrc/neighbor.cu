@@ -9,6 +9,8 @@
 //
 // Pair test: FP64, round-to-nearest, no FMA contraction:
 //   x_w = x - floor(x/L) L;  d = (x_w[j] - x_w[i]) + S L;  d2 = (dx dx + dy dy) + dz dz;  d2 < (rc+skin)^2
+// and for a triclinic cell (lower-triangular lattice, reading B-9) the same with fractional coordinates by
+// back substitution and S . box = ((S0 ax + S1 bx) + S2 cx, S1 by + S2 cy, S2 cz): box_frac / box_shift of common.cuh.
 // Integer atomics (cell histogram, scatter slots, counters) are used; their effect on ordering is
 // removed by sorting each cell by caller index and each CSR row by ext index, so the list is
 // bitwise deterministic.
@@ -22,25 +24,38 @@ namespace {
 constexpr int ROWCAP = 1024; // max list entries per atom (smem row buffer per warp)
 constexpr int NB_WARPS = 4;  // warps per block in the row kernels
 
-__device__ __forceinline__ double wrap_coord(double x, double L, int32_t *w) {
-    double f = floor(__ddiv_rn(x, L));
-    *w = (int32_t)f;
-    return __dsub_rn(x, __dmul_rn(f, L));
+// whole periods w = floor(fractional coordinates) and the wrapped position x - w . box (reading B-9)
+__device__ __forceinline__ void wrap_pos(const BoxP &B, double x, double y, double z, int32_t *w, double *xw, double *yw,
+                                         double *zw) {
+    double sa, sb, sc;
+    box_frac(B, x, y, z, sa, sb, sc);
+    const double fa = floor(sa), fb = floor(sb), fc = floor(sc);
+    w[0] = (int32_t)fa; w[1] = (int32_t)fb; w[2] = (int32_t)fc;
+    double hx, hy, hz;
+    box_shift(B, fa, fb, fc, hx, hy, hz);
+    *xw = __dsub_rn(x, hx); *yw = __dsub_rn(y, hy); *zw = __dsub_rn(z, hz);
+}
+// cell of a wrapped position: cells are equal slices of the fractional coordinates
+__device__ __forceinline__ void cell_of(const BoxP &B, double xw, double yw, double zw, int ncx, int ncy, int ncz, int *cx,
+                                        int *cy, int *cz) {
+    double sa, sb, sc;
+    box_frac(B, xw, yw, zw, sa, sb, sc);
+    *cx = min(ncx - 1, max(0, (int)floor(sa * ncx)));
+    *cy = min(ncy - 1, max(0, (int)floor(sb * ncy)));
+    *cz = min(ncz - 1, max(0, (int)floor(sc * ncz)));
 }
 
-__global__ void k_wrap_cell(const double *__restrict__ pos, int64_t N, double Lx, double Ly, double Lz, int ncx,
+__global__ void k_wrap_cell(const double *__restrict__ pos, int64_t N, BoxP B, int ncx,
                             int ncy, int ncz, const int32_t *__restrict__ cell_rank, int32_t *__restrict__ wshift,
                             int32_t *__restrict__ cellkey, int32_t *__restrict__ cell_count) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     int32_t w[3];
-    double x = wrap_coord(pos[3 * i], Lx, &w[0]);
-    double y = wrap_coord(pos[3 * i + 1], Ly, &w[1]);
-    double z = wrap_coord(pos[3 * i + 2], Lz, &w[2]);
+    double x, y, z;
+    wrap_pos(B, pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], w, &x, &y, &z);
     wshift[3 * i] = w[0]; wshift[3 * i + 1] = w[1]; wshift[3 * i + 2] = w[2];
-    int cx = min(ncx - 1, max(0, (int)(x * (ncx / Lx))));
-    int cy = min(ncy - 1, max(0, (int)(y * (ncy / Ly))));
-    int cz = min(ncz - 1, max(0, (int)(z * (ncz / Lz))));
+    int cx, cy, cz;
+    cell_of(B, x, y, z, ncx, ncy, ncz, &cx, &cy, &cz);
     int key = cell_rank[(cx * ncy + cy) * ncz + cz];
     cellkey[i] = key;
     atomicAdd(&cell_count[key], 1);
@@ -70,45 +85,56 @@ __global__ void k_sort_cells(int32_t *__restrict__ perm, const int64_t *__restri
 
 __global__ void k_local_records(const int32_t *__restrict__ perm, const double *__restrict__ pos,
                                 const int32_t *__restrict__ wshift, const int32_t *__restrict__ species_caller,
-                                int64_t N, double Lx, double Ly, double Lz, XRec *__restrict__ xrec,
+                                int64_t N, BoxP B, XRec *__restrict__ xrec,
                                 int32_t *__restrict__ inv_perm, double *__restrict__ pos_build) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     int64_t i = perm[k];
     XRec r;
-    r.x = __dsub_rn(pos[3 * i], __dmul_rn((double)wshift[3 * i], Lx));
-    r.y = __dsub_rn(pos[3 * i + 1], __dmul_rn((double)wshift[3 * i + 1], Ly));
-    r.z = __dsub_rn(pos[3 * i + 2], __dmul_rn((double)wshift[3 * i + 2], Lz));
+    double hx, hy, hz;
+    box_shift(B, (double)wshift[3 * i], (double)wshift[3 * i + 1], (double)wshift[3 * i + 2], hx, hy, hz);
+    r.x = __dsub_rn(pos[3 * i], hx);
+    r.y = __dsub_rn(pos[3 * i + 1], hy);
+    r.z = __dsub_rn(pos[3 * i + 2], hz);
     r.owner = (int32_t)k; r.sx = r.sy = r.sz = 0; r.species = (uint8_t)species_caller[i];
     xrec[k] = r;
     inv_perm[i] = (int32_t)k;
     pos_build[3 * i] = pos[3 * i]; pos_build[3 * i + 1] = pos[3 * i + 1]; pos_build[3 * i + 2] = pos[3 * i + 2];
 }
 
-// A2: images of atom k that can lie within R of some wrapped local atom: shift s_d = +1 needs
-// x_d < R (+margin), s_d = -1 needs x_d >= L_d - R (-margin). Superset of the images referenced.
-__device__ __forceinline__ int allowed_mask(double x, double L, double Rm) {
+// A2: images of atom k that can lie within R of some wrapped local atom. In the direction of lattice vector d the atom
+// is s_d w_d away from the low face and (1 - s_d) w_d from the high one (s = fractional coordinate, w = distance between
+// the faces): shift +1 needs s_d w_d < R (+margin), shift -1 needs (1 - s_d) w_d <= R (+margin). Superset of the images
+// referenced.
+__device__ __forceinline__ int allowed_mask(double s, double w, double Rm) {
     int m = 2; // bit1: s=0
-    if (x < Rm) m |= 4;         // s=+1
-    if (x >= L - Rm) m |= 1;    // s=-1
+    if (s * w < Rm) m |= 4;             // s=+1
+    if ((1.0 - s) * w <= Rm) m |= 1;    // s=-1
     return m;
 }
+__device__ __forceinline__ void image_masks(const BoxP &B, const XRec &r, double Rm, int *mx, int *my, int *mz) {
+    double sa, sb, sc;
+    box_frac(B, r.x, r.y, r.z, sa, sb, sc);
+    *mx = allowed_mask(sa, B.wa, Rm); *my = allowed_mask(sb, B.wb, Rm); *mz = allowed_mask(sc, B.wc, Rm);
+}
 
-__global__ void k_ghost_count(const XRec *__restrict__ xrec, int64_t N, double Lx, double Ly, double Lz, double Rm,
+__global__ void k_ghost_count(const XRec *__restrict__ xrec, int64_t N, BoxP B, double Rm,
                               int32_t *__restrict__ gcnt) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     XRec r = xrec[k];
-    int mx = allowed_mask(r.x, Lx, Rm), my = allowed_mask(r.y, Ly, Rm), mz = allowed_mask(r.z, Lz, Rm);
+    int mx, my, mz;
+    image_masks(B, r, Rm, &mx, &my, &mz);
     gcnt[k] = __popc(mx) * __popc(my) * __popc(mz) - 1;
 }
 
-__global__ void k_ghost_fill(XRec *__restrict__ xrec, int64_t N, double Lx, double Ly, double Lz, double Rm,
+__global__ void k_ghost_fill(XRec *__restrict__ xrec, int64_t N, BoxP B, double Rm,
                              const int64_t *__restrict__ goff, int32_t *__restrict__ img_index) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     XRec r = xrec[k];
-    int mx = allowed_mask(r.x, Lx, Rm), my = allowed_mask(r.y, Ly, Rm), mz = allowed_mask(r.z, Lz, Rm);
+    int mx, my, mz;
+    image_masks(B, r, Rm, &mx, &my, &mz);
     int64_t g = N + goff[k];
     for (int sx = -1; sx <= 1; ++sx)
         for (int sy = -1; sy <= 1; ++sy)
@@ -125,7 +151,7 @@ __global__ void k_ghost_fill(XRec *__restrict__ xrec, int64_t N, double Lx, doub
 }
 
 struct Grid {
-    double Lx, Ly, Lz;
+    BoxP B;
     int ncx, ncy, ncz;
     double R2, rc2;
 };
@@ -156,9 +182,8 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
     const int64_t i = (int64_t)blockIdx.x * NB_WARPS + warp;
     if (i >= N) return;
     const XRec me = xrec[i];
-    int cx = min(g.ncx - 1, max(0, (int)(me.x * (g.ncx / g.Lx))));
-    int cy = min(g.ncy - 1, max(0, (int)(me.y * (g.ncy / g.Ly))));
-    int cz = min(g.ncz - 1, max(0, (int)(me.z * (g.ncz / g.Lz))));
+    int cx, cy, cz;
+    cell_of(g.B, me.x, me.y, me.z, g.ncx, g.ncy, g.ncz, &cx, &cy, &cz);
     int cnt = 0, cnt_rc = 0;
     int32_t *buf = rowbuf + (FILL ? warp * ROWCAP : 0);
     for (int o = 0; o < 27; ++o) {
@@ -169,8 +194,8 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
         if (az < 0) { az += g.ncz; sz = -1; } else if (az >= g.ncz) { az -= g.ncz; sz = 1; }
         const int key = cell_rank[(ax * g.ncy + ay) * g.ncz + az];
         const int64_t c0 = cell_start[key], c1 = cell_start[key + 1];
-        const double shx = __dmul_rn((double)sx, g.Lx), shy = __dmul_rn((double)sy, g.Ly),
-                     shz = __dmul_rn((double)sz, g.Lz);
+        double shx, shy, shz;
+        box_shift(g.B, (double)sx, (double)sy, (double)sz, shx, shy, shz);
         const int code = shift_code(sx, sy, sz);
         for (int64_t jb = c0; jb < c1; jb += 32) {
             const int64_t j = jb + lane;
@@ -297,9 +322,10 @@ int neighbor_build(reann *h, const double *d_pos) {
     const ModelDims &md = h->md;
     LaunchCtx ctx = h->ctx();
     const double R = md.rc + md.skin;
-    const double Lx = h->box_build[0], Ly = h->box_build[4], Lz = h->box_build[8];
-    Grid g{Lx, Ly, Lz, std::max(1, (int)floor(Lx / R)), std::max(1, (int)floor(Ly / R)),
-           std::max(1, (int)floor(Lz / R)), R * R, md.rc * md.rc};
+    const BoxP B = make_boxp(h->box_build);
+    // cells: equal slices of the fractional coordinates, at least R between their faces
+    Grid g{B, std::max(1, (int)floor(B.wa / R)), std::max(1, (int)floor(B.wb / R)),
+           std::max(1, (int)floor(B.wc / R)), R * R, md.rc * md.rc};
     const int64_t ncell = (int64_t)g.ncx * g.ncy * g.ncz;
     if (ncell > (int64_t)1 << 30) return set_err(h, REANN_ERR_UNSUPPORTED, "too many cells");
 
@@ -344,21 +370,21 @@ int neighbor_build(reann *h, const double *d_pos) {
     CU(h, cudaMemsetAsync(flags, 0, sizeof(int32_t) * 8, h->stream));
 
     // A1: wrap, cell key, counting sort in Morton cell order, deterministic inside each cell
-    LAUNCH(ctx, k_wrap_cell, div_up(N, TPB), TPB, 0, d_pos, N, Lx, Ly, Lz, g.ncx, g.ncy, g.ncz,
+    LAUNCH(ctx, k_wrap_cell, div_up(N, TPB), TPB, 0, d_pos, N, B, g.ncx, g.ncy, g.ncz,
            (const int32_t *)h->cell_rank.p, (int32_t *)h->wshift.p, cellkey, cell_count);
     exclusive_scan_i32_to_i64(ctx, cell_count, (int64_t *)h->cell_start.p, ncell, h->scan_ws.p);
     LAUNCH(ctx, k_scatter, div_up(N, TPB), TPB, 0, cellkey, N, (const int64_t *)h->cell_start.p, cell_fill,
            (int32_t *)h->perm.p);
     LAUNCH(ctx, k_sort_cells, div_up(ncell, 64), 64, 0, (int32_t *)h->perm.p, (const int64_t *)h->cell_start.p, ncell);
     LAUNCH(ctx, k_local_records, div_up(N, TPB), TPB, 0, (const int32_t *)h->perm.p, d_pos,
-           (const int32_t *)h->wshift.p, (const int32_t *)h->species_caller.p, N, Lx, Ly, Lz, (XRec *)h->xrec.p,
+           (const int32_t *)h->wshift.p, (const int32_t *)h->species_caller.p, N, B, (XRec *)h->xrec.p,
            (int32_t *)h->inv_perm.p, (double *)h->pos_build.p);
 
     // A2: ghost / image map
-    const double Rm = R + 1e-6 * std::max(Lx, std::max(Ly, Lz)) + 1e-9;
+    const double Rm = R + 1e-6 * std::max(B.ax, std::max(B.by, B.cz)) + 1e-9;
     int32_t *gcnt = (int32_t *)h->scratch_a.p;
     int64_t *goff = (int64_t *)h->scratch_c.p;
-    LAUNCH(ctx, k_ghost_count, div_up(N, TPB), TPB, 0, (const XRec *)h->xrec.p, N, Lx, Ly, Lz, Rm, gcnt);
+    LAUNCH(ctx, k_ghost_count, div_up(N, TPB), TPB, 0, (const XRec *)h->xrec.p, N, B, Rm, gcnt);
     exclusive_scan_i32_to_i64(ctx, gcnt, goff, N, h->scan_ws.p);
     int64_t G = 0;
     CU(h, cudaMemcpyAsync(&G, goff + N, sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
@@ -378,7 +404,7 @@ int neighbor_build(reann *h, const double *d_pos) {
         }
     }
     h->G = G; h->n_ext = N + G;
-    LAUNCH(ctx, k_ghost_fill, div_up(N, TPB), TPB, 0, (XRec *)h->xrec.p, N, Lx, Ly, Lz, Rm, (const int64_t *)goff,
+    LAUNCH(ctx, k_ghost_fill, div_up(N, TPB), TPB, 0, (XRec *)h->xrec.p, N, B, Rm, (const int64_t *)goff,
            (int32_t *)h->img_index.p);
 
     // A3: count -> scan -> fill (+ row sort) -> reverse index
