@@ -24,6 +24,7 @@ namespace {
 using namespace edge;
 
 constexpr int EW = 4; // warps per block in the edge kernels
+constexpr int RW = 2; // warps per block of the row-streaming kernels (rc-filter, reverse gather): a warp takes one row
 
 // ------------------------------------------------------------------------------------------ A4
 __global__ void k_skin_check(const double *__restrict__ pos, const double *__restrict__ pos_build, int64_t n3,
@@ -65,12 +66,12 @@ __device__ __forceinline__ double edge_d2(const XRec &me, const XRec &o, const B
 }
 
 // rc-filter, pass 1: rank of every accepted list entry inside its row (0xFFFF = rejected)
-__global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict__ xrec,
+__global__ void __launch_bounds__(RW * 32) k_filter_count(const XRec *__restrict__ xrec,
                                                           const int64_t *__restrict__ row_ptr,
                                                           const int32_t *__restrict__ col, int64_t N, BoxP B, double rc2,
                                                           uint16_t *__restrict__ rank16, int32_t *__restrict__ rc_cnt) {
     const int lane = threadIdx.x & 31;
-    const int64_t i = (int64_t)blockIdx.x * EW + (threadIdx.x >> 5);
+    const int64_t i = (int64_t)blockIdx.x * RW + (threadIdx.x >> 5);
     if (i >= N) return;
     const XRec me = xrec[i];
     const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1];
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(EW * 32) k_filter_count(const XRec *__restrict
 
 // rc-filter, pass 2: compact rows (neighbour ext index | species<<28, edge vector + length in FP32
 // rounded once from the FP64 difference, index of the reverse compact edge)
-__global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict__ xrec,
+__global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict__ xrec,
                                                          const int64_t *__restrict__ row_ptr,
                                                          const int32_t *__restrict__ col,
                                                          const uint32_t *__restrict__ rev, int64_t N, BoxP B,
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(EW * 32) k_filter_fill(const XRec *__restrict_
                                                          uint32_t *__restrict__ rev_rc, const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
     const int lane = threadIdx.x & 31;
-    const int64_t i = (int64_t)blockIdx.x * EW + (threadIdx.x >> 5);
+    const int64_t i = (int64_t)blockIdx.x * RW + (threadIdx.x >> 5);
     if (i >= N) return;
     const XRec me = xrec[i];
     const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1], c0 = rc_ptr[i];
@@ -321,14 +322,15 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd(int64_t N, const int64_t *
 // registers: accumulating the ~36 steps of an atom inside the MMA truncates like tcgen05 does and was measured
 // to cost 1.4e-6 eV/atom on config 2, above the 1e-6 gate). N_phi (padded to 4) in {8, 12, 16}: the M = 16 rows
 // beyond N_phi are zero.
+constexpr int FW = 1; // warps per block of the mma.sync edge forward kernel: a warp takes one atom and leaves
 template <int NA>
 struct FwdMma {
     static constexpr int NAP = (NA + 7) & ~7, AT = NAP / 8, TS = 36;
-    static constexpr int ROWS = 16 + NAP, SMEM = EW * ROWS * TS * 4;
+    static constexpr int ROWS = 16 + NAP, SMEM = FW * ROWS * TS * 4;
 };
 
 template <int NPHIP, int NA>
-__global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64_t *__restrict__ rc_ptr,
+__global__ void __launch_bounds__(FW * 32) k_edge_fwd_mma(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                           const uint32_t *__restrict__ col_rc,
                                                           const float4 *__restrict__ geom,
                                                           const float *__restrict__ c_ext, RadialTab rt,
@@ -340,7 +342,7 @@ __global__ void __launch_bounds__(EW * 32) k_edge_fwd_mma(int64_t N, const int64
     extern __shared__ __align__(16) float smem_f[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g8 = lane >> 2, t4 = lane & 3;
     float *XT = smem_f + (size_t)warp * C::ROWS * TS, *AT_s = XT + 16 * TS;
-    const int64_t i = (int64_t)blockIdx.x * EW + warp;
+    const int64_t i = (int64_t)blockIdx.x * FW + warp;
     if (i >= N) return;
     const int64_t beg = rc_ptr[i], end = rc_ptr[i + 1];
     float acc[AT][4];
@@ -607,10 +609,14 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // two edges per lane where the registers allow three blocks per SM with it (N_a <= 10); at N_a = 20 the pair of edges
 // costs a quarter of the resident warps and measured slower (1.09 vs 1.03 ms on config 3)
 template <int NA>
-struct BwdShape { static constexpr int NE = (NA % 2 == 0 && NA <= 10) ? 2 : 1, MINB = NE == 2 ? 3 : 4; };
+struct BwdShape {
+    static constexpr int NE = (NA % 2 == 0 && NA <= 10) ? 2 : 1;
+    static constexpr int WPB = NE == 2 ? EW : 1;        // warps per block: one where a warp takes one atom and leaves (no waiting for block mates)
+    static constexpr int MINB = NE == 2 ? 3 : 16;
+};
 
 template <int NPHIP, int NA, bool VIR>
-__global__ void __launch_bounds__(EW * 32, BwdShape<NA>::MINB) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
+__global__ void __launch_bounds__(BwdShape<NA>::WPB * 32, BwdShape<NA>::MINB) k_edge_bwd(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                       const uint32_t *__restrict__ col_rc,
                                                       const float4 *__restrict__ geom,
                                                       const float *__restrict__ c_ext, RadialTab rt, int S,
@@ -618,20 +624,20 @@ __global__ void __launch_bounds__(EW * 32, BwdShape<NA>::MINB) k_edge_bwd(int64_
                                                       float *__restrict__ kappa, float4 *__restrict__ gst,
                                                       double *__restrict__ vir_part, AtomChunk ch, const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
-    constexpr int NB = NPHIP * NA;
-    __shared__ __align__(16) float bb_s[EW][2][NB];
-    __shared__ __align__(16) float4 g_s[EW][2][64];
-    __shared__ uint32_t cj_s[EW][2][64];
+    constexpr int NB = NPHIP * NA, WPB = BwdShape<NA>::WPB;
+    __shared__ __align__(16) float bb_s[WPB][2][NB];
+    __shared__ __align__(16) float4 g_s[WPB][2][64];
+    __shared__ uint32_t cj_s[WPB][2][64];
     __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
-    __shared__ float vir_s[VIR ? EW : 1][9];
+    __shared__ float vir_s[VIR ? WPB : 1][9];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int k = threadIdx.x; k < S * NPHIP; k += EW * 32) { tab_s[0][k] = rt.rcen[k]; tab_s[1][k] = rt.alpha2[k]; }
+    for (int k = threadIdx.x; k < S * NPHIP; k += WPB * 32) { tab_s[0][k] = rt.rcen[k]; tab_s[1][k] = rt.alpha2[k]; }
     __syncthreads();
     float aV[VIR ? 9 : 1];
 #pragma unroll
     for (int k = 0; k < (VIR ? 9 : 1); ++k) aV[k] = 0.f;
-    const int64_t stride = (int64_t)gridDim.x * EW;
-    int64_t i = ch.a0 + (int64_t)blockIdx.x * EW + warp;
+    const int64_t stride = (int64_t)gridDim.x * WPB;
+    int64_t i = ch.a0 + (int64_t)blockIdx.x * WPB + warp;
     // request bbar and the first-pass records of atom `a` (row [b0, b1)) into buffer `buf`
     auto request = [&](int64_t a, int64_t b0, int64_t b1, int buf) {
         const float4 *src = reinterpret_cast<const float4 *>(bbar + a * (int64_t)NB);
@@ -694,7 +700,7 @@ __global__ void __launch_bounds__(EW * 32, BwdShape<NA>::MINB) k_edge_bwd(int64_
         if (threadIdx.x < 9) {
             double s = 0.0;
 #pragma unroll
-            for (int w = 0; w < EW; ++w) s += (double)vir_s[w][threadIdx.x];
+            for (int w = 0; w < WPB; ++w) s += (double)vir_s[w][threadIdx.x];
             vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x] += s;
         }
     }
@@ -705,7 +711,7 @@ __global__ void __launch_bounds__(EW * 32, BwdShape<NA>::MINB) k_edge_bwd(int64_
 // edge): cbar_k[n] = sum_{e in row(k)} kappa[rev(e)][n];  F_k += sum_{e in row(k)} (g_e - g_rev(e))
 // (Eq. 3).
 template <int NPHIP>
-__global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t *__restrict__ rc_ptr,
+__global__ void __launch_bounds__(RW * 32) k_rev_gather(int64_t N, const int64_t *__restrict__ rc_ptr,
                                                         const uint32_t *__restrict__ rev_rc,
                                                         const float *__restrict__ kappa,
                                                         const float4 *__restrict__ gst, int want_cbar,
@@ -713,9 +719,9 @@ __global__ void __launch_bounds__(EW * 32) k_rev_gather(int64_t N, const int64_t
                                                         StashChunk ch, const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
     constexpr int PARTS = NPHIP / 4, EPS = 32 / PARTS; // float4 parts per edge, edges per warp step
-    __shared__ float4 red_s[EW][32];
+    __shared__ float4 red_s[RW][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t k = (int64_t)blockIdx.x * EW + warp;
+    const int64_t k = (int64_t)blockIdx.x * RW + warp;
     if (k >= N) return;
     const int64_t beg = rc_ptr[k], end = rc_ptr[k + 1];
     if (ch.do_forces) {
@@ -848,12 +854,12 @@ void launch_refresh(const LaunchCtx &ctx, XRec *xrec, int64_t n_ext, const int32
 }
 void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
                          int64_t N, const BoxP &box, double rc2, uint16_t *rank16, int32_t *rc_cnt) {
-    if (N > 0) LAUNCH(ctx, k_filter_count, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, N, box, rc2, rank16, rc_cnt);
+    if (N > 0) LAUNCH(ctx, k_filter_count, div_up(N, RW), RW * 32, 0, xrec, row_ptr, col, N, box, rc2, rank16, rc_cnt);
 }
 void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
                         const uint32_t *rev, int64_t N, const BoxP &box, const uint16_t *rank16,
                         const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc) {
-    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, EW), EW * 32, 0, xrec, row_ptr, col, rev, N, box, rank16, rc_ptr, col_rc, geom, rev_rc, ctx.skip);
+    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, RW), RW * 32, 0, xrec, row_ptr, col, rev, N, box, rank16, rc_ptr, col_rc, geom, rev_rc, ctx.skip);
 }
 void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip) {
     const int64_t work = (n_ext - N) * (nphip / 4);
@@ -864,7 +870,7 @@ template <int NPHIP, int NA>
 static int run_edge_fwd_mma(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *col_rc,
                             const float4 *geom, const float *c_ext, RadialTab rt, float *b) {
     using C = FwdMma<NA>;
-    LAUNCH(ctx, (k_edge_fwd_mma<NPHIP, NA>), div_up(N, EW), EW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b, ctx.skip);
+    LAUNCH(ctx, (k_edge_fwd_mma<NPHIP, NA>), div_up(N, FW), FW * 32, C::SMEM, N, rc_ptr, col_rc, geom, c_ext, rt, b, ctx.skip);
     return REANN_OK;
 }
 
@@ -916,7 +922,7 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 }
 
 // upper bound of the grid of the edge backward kernel (= entries of the virial partial array)
-int edge_bwd_blocks(int64_t N) { return (int)div_up(std::max<int64_t>(N, 1), EW); }
+int edge_bwd_blocks(int64_t N) { return (int)std::max<int64_t>(N, 1); }   // one-warp blocks in the one-edge-per-lane shape
 static int sm_count() {
     static int n_sm[64] = {};
     int dev = 0;
@@ -933,17 +939,17 @@ int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
                     int64_t a0, int64_t a1, int64_t e_lo) {
     if (N <= 0 || a1 <= a0) return REANN_OK;
     const AtomChunk ch{a0, a1, e_lo};
-    const unsigned nblk_all = div_up(a1 - a0, EW);
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
     const int want_kappa = t >= 1;
 #define M(NP, NA_, PN_, PA_) {                                                                                    \
     /* two edges per lane: persistent warps, one wave of resident blocks; else one atom per warp (measured faster) */ \
+    const unsigned nblk_all = div_up(a1 - a0, BwdShape<NA_>::WPB);                                                \
     const unsigned nblk = BwdShape<NA_>::NE == 2 ? std::min(nblk_all, (unsigned)(BwdShape<NA_>::MINB * sm_count())) : nblk_all; \
     if (vir_part)                                                                                                 \
-        LAUNCH(ctx, (k_edge_bwd<NP, NA_, true>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,            \
+        LAUNCH(ctx, (k_edge_bwd<NP, NA_, true>), nblk, BwdShape<NA_>::WPB * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,            \
                md.S, bbar, want_kappa, kappa, gst, vir_part, ch, ctx.skip);                                       \
     else                                                                                                          \
-        LAUNCH(ctx, (k_edge_bwd<NP, NA_, false>), nblk, EW * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,           \
+        LAUNCH(ctx, (k_edge_bwd<NP, NA_, false>), nblk, BwdShape<NA_>::WPB * 32, 0, N, rc_ptr, col_rc, geom, c_ext, rt,           \
                md.S, bbar, want_kappa, kappa, gst, vir_part, ch, ctx.skip);                                       \
     return REANN_OK; }
     EDGE_DISPATCH(M)
@@ -956,10 +962,10 @@ void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, c
     if (N <= 0) return;
     const StashChunk ch{e_lo, e_hi, do_forces, accumulate};
     switch (nphip) {
-        case 4: LAUNCH(ctx, k_rev_gather<4>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
-        case 8: LAUNCH(ctx, k_rev_gather<8>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
-        case 12: LAUNCH(ctx, k_rev_gather<12>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
-        default: LAUNCH(ctx, k_rev_gather<16>, div_up(N, EW), EW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        case 4: LAUNCH(ctx, k_rev_gather<4>, div_up(N, RW), RW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        case 8: LAUNCH(ctx, k_rev_gather<8>, div_up(N, RW), RW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        case 12: LAUNCH(ctx, k_rev_gather<12>, div_up(N, RW), RW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
+        default: LAUNCH(ctx, k_rev_gather<16>, div_up(N, RW), RW * 32, 0, N, rc_ptr, rev_rc, kappa, gst, want_cbar, cbar, Fc, ch, ctx.skip); break;
     }
 }
 
