@@ -58,6 +58,8 @@ constexpr int NCOMPUTE = 256, NTHREADS = NCOMPUTE + 32, CTL_WARP = 8;
 constexpr uint32_t COL_BUF = 128;      // TMEM columns per group buffer
 constexpr int NBUF = 3;                // group buffers: one filling, one complete, one being drained
 constexpr uint32_t TMEM_COLS = 512;    // allocation (power of two >= NBUF * COL_BUF)
+constexpr uint32_t COL_A = NBUF * COL_BUF; // forward GEMM 1: A operand (hi | lo images of a Q chunk) in TMEM, two slots of 64 columns
+constexpr uint32_t A_TSLOT = 2 * KC;
 
 // barrier slots (8 bytes each) in the barrier area
 enum { BAR_BFULL = 0, BAR_MMA = 3, BAR_AFULL = 6, BAR_AH = 9, BAR_QFULL = 13, BAR_QEMPTY = 15, BAR_DFULL = 17,
@@ -182,6 +184,53 @@ struct Ctl {
             if (last) tc_commit(bar(BAR_DFULL + d));
         }
         __syncwarp();
+    }
+    // The same two with the A operand in tensor memory (TS form: `a_col` = first column of the hi image, lo image KC
+    // columns further): the MMAs then read only B from shared memory
+    __device__ __forceinline__ void mma_chunk_ts(int i_loc, uint32_t a_col, int n_rows, int g_loc) const {
+        const int i = sb + i_loc, g = gb + g_loc;
+        const int s = i % NSTAGE, d = g % NBUF;
+        if (g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
+        mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
+        tc_fence_after();
+        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
+        if (elect_one()) {
+            issue_ts(i, a_col, n_rows, dm, true, false, true);
+            issue_ts(i, a_col, n_rows, dm, false, true, false);
+            tc_commit(bar(BAR_MMA + s));
+            tc_commit(bar(BAR_DFULL + d));
+        }
+        __syncwarp();
+    }
+    __device__ __forceinline__ void mma_chunk_1x_ts(int i_loc, uint32_t a_col, int n_rows, int g_loc, bool first, bool last) const {
+        const int i = sb + i_loc, g = gb + g_loc;
+        const int s = i % NSTAGE, d = g % NBUF;
+        if (first && g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
+        mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
+        tc_fence_after();
+        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
+        if (elect_one()) {
+            issue_ts(i, a_col, n_rows, dm, false, true, first);
+            tc_commit(bar(BAR_MMA + s));
+            if (last) tc_commit(bar(BAR_DFULL + d));
+        }
+        __syncwarp();
+    }
+    __device__ __forceinline__ void issue_ts(int i, uint32_t a_col, int n_rows, uint32_t dm, bool corr, bool main, bool fresh) const {
+        const int s = i % NSTAGE;
+        const uint32_t idesc = make_idesc(n_rows);
+        const uint32_t a_hi = tmem + a_col, a_lo = a_hi + KC;
+        const uint32_t b_lbo = (uint32_t)n_rows * 16;
+        const uint32_t b_hi = b0 + (uint32_t)s * B_SLOT, b_lo = b_hi + (uint32_t)n_rows * KC * 4;
+#pragma unroll
+        for (int kk = 0; kk < KC / 8; ++kk) {
+            const uint64_t bh = make_desc(b_hi + kk * 2 * b_lbo, b_lbo), bl = make_desc(b_lo + kk * 2 * b_lbo, b_lbo);
+            if (corr) {
+                umma_tf32_ts(dm, a_lo + kk * 8, bh, idesc, (fresh && kk == 0) ? 0u : 1u);
+                umma_tf32_ts(dm, a_hi + kk * 8, bl, idesc, 1u);
+            }
+            if (main) umma_tf32_ts(dm, a_hi + kk * 8, bh, idesc, (fresh && !corr && kk == 0) ? 0u : 1u);
+        }
     }
     // Two K chunks (steps i, i+1) = one accumulation group of K = 64: all corrections first, then hi.hi of both
     __device__ __forceinline__ void mma_pair(int i_loc, int a_slot0, int a_slot1, int n_rows, int g_loc) const {
@@ -328,8 +377,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                         mbar_wait(c.bar(BAR_AFULL + sa), (uint32_t)((j / NSTAGE) & 1));
                         if (i + 2 < n1) issue_q(i + 2);
                         TC_TRACE(0, 0, 2 * i);
-                        if (A.tf32) c.mma_chunk_1x(i, sa, H1p, 0, i == 0, i == n1 - 1);
-                        else c.mma_chunk(i, sa, H1p, i);
+                        const uint32_t a_col = COL_A + A_TSLOT * (uint32_t)(i & 1);
+                        if (A.tf32) c.mma_chunk_1x_ts(i, a_col, H1p, 0, i == 0, i == n1 - 1);
+                        else c.mma_chunk_ts(i, a_col, H1p, i);
                     } else {
                         mbar_wait(c.bar(BAR_AH + (i - n1)), (uint32_t)(it & 1));
                         TC_TRACE(0, 0, 2 * i);
@@ -356,27 +406,32 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
             float acc1[CW1];
 #pragma unroll
             for (int c = 0; c < CW1; ++c) acc1[c] = 0.f;
-            const int crow = warp * 16 + (lane & 7), ckq = lane >> 3;
 #pragma unroll 1
             for (int i = 0; i < n1; ++i) {
                 const int j = qb + i, sa = j % NSTAGE, qs = j & 1;
                 mbar_wait(bar0 + 8 * (BAR_QFULL + qs), (uint32_t)((j >> 1) & 1));
-                wait_stage_free(bar0, sb + i);       // MMAs of step - 3 (they read A slot sa when they belong to this tile)
+                // TMEM operand slot i & 1: the MMAs of chunk i - 2 (this tile) must have read it
+                if (i >= 2) { const int st = sb + i - 2; mbar_wait(bar0 + 8 * (BAR_MMA + st % NSTAGE), (uint32_t)((st / NSTAGE) & 1)); }
+                tc_fence_after();
+                // my row of the raw chunk, K columns [16 hf, 16 hf + 16): hi / lo images straight into tensor memory
                 const unsigned char *stg = smem + SM_A + 3 * A_SLOT + qs * A_HALF;
-                float4 v[4];
+                uint32_t hi[16], lo[16];
 #pragma unroll
-                for (int rb = 0; rb < 2; ++rb)
+                for (int q = 0; q < 4; ++q) {
+                    const float4 v = *reinterpret_cast<const float4 *>(stg + (4 * hf + q) * (int)A_LBO + m * 16);
+                    const float x[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-                    for (int jj = 0; jj < 2; ++jj)
-                        v[rb * 2 + jj] = *reinterpret_cast<const float4 *>(stg + (ckq + 4 * jj) * (int)A_LBO + (crow + rb * 8) * 16);
-#pragma unroll
-                for (int rb = 0; rb < 2; ++rb)
-#pragma unroll
-                    for (int jj = 0; jj < 2; ++jj) {
-                        const float x[4] = {v[rb * 2 + jj].x, v[rb * 2 + jj].y, v[rb * 2 + jj].z, v[rb * 2 + jj].w};
-                        store_split4(a_base + sa * A_SLOT, ckq + 4 * jj, crow + rb * 8, x);
+                    for (int u = 0; u < 4; ++u) {
+                        float h, l;
+                        split_tf32(x[u], h, l);
+                        hi[4 * q + u] = __float_as_uint(h); lo[4 * q + u] = __float_as_uint(l);
                     }
-                fence_async_smem();
+                }
+                const uint32_t ta = tl + COL_A + A_TSLOT * (uint32_t)(i & 1) + 16u * (uint32_t)hf;
+                tmem_st16(ta, hi);
+                if (!A.tf32) tmem_st16(ta + KC, lo);
+                tmem_wait_st();
+                tc_fence_before();
                 mbar_arrive(bar0 + 8 * (BAR_AFULL + sa));
                 mbar_arrive(bar0 + 8 * (BAR_QEMPTY + qs));
                 if (tid == 0) TC_TRACE(0, 1, 2 * i);
