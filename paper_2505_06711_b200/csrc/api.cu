@@ -444,7 +444,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->Ei, sizeof(float) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Ei_caller, sizeof(double) * (size_t)std::max<int64_t>(N, 1)));
         RC(dev_ensure(h, h->Fc, sizeof(double) * 3 * (size_t)std::max<int64_t>(N, 1)));
-        h->n_vir_blocks = edge_bwd_blocks(std::max<int64_t>(N, 1));
+        h->n_vir_blocks = edge_bwd_blocks(std::max<int64_t>(N, 1), md.Na);
         RC(dev_ensure(h, h->vir_part, sizeof(double) * 9 * (size_t)h->n_vir_blocks));
         RC(dev_ensure(h, h->red_scratch, sizeof(double) * 10 * ((size_t)N / 256 + 2)));
         RC(dev_ensure(h, h->out_stage, sizeof(double) * (16 + 3 * (size_t)N)));

@@ -155,7 +155,7 @@ int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
                     const float *alpha, const float *bbar, float *kappa, float4 *gst, double *vir_part,
                     int64_t a0, int64_t a1, int64_t e_lo /* atoms [a0, a1), a0 % 4 == 0; kappa holds edges from e_lo on */);
-int edge_bwd_blocks(int64_t N);
+int edge_bwd_blocks(int64_t N, int Na);
 void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *rev_rc,
                        const float *kappa, const float4 *gst, int nphip, int want_cbar, float *cbar, double *Fc,
                        int64_t e_lo, int64_t e_hi, int do_forces, int accumulate /* kappa holds edges [e_lo, e_hi) */);

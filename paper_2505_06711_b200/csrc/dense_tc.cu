@@ -54,7 +54,7 @@ constexpr int B_SLOT = 2 * 128 * KC * 4; // 32 KB (N <= 128)
 constexpr int SM_A = 0, SM_B = NASLOT * A_SLOT, SM_BAR = SM_B + NSTAGE * B_SLOT;
 constexpr int SM_TOTAL = SM_BAR + 256;
 constexpr uint32_t A_LBO = TM * 16;
-constexpr int NCOMPUTE = 256, NTHREADS = NCOMPUTE + 32, CTL_WARP = 8;
+constexpr int NCOMPUTE = 256, NTHREADS = NCOMPUTE + 64, CTL_WARP = 8, COPY_WARP = 9;   // warp 8 issues the MMAs, warp 9 the bulk copies
 constexpr uint32_t COL_BUF = 128;      // TMEM columns per group buffer
 constexpr int NBUF = 3;                // group buffers: one filling, one complete, one being drained
 constexpr uint32_t TMEM_COLS = 512;    // allocation (power of two >= NBUF * COL_BUF)
@@ -343,54 +343,64 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
     // running counters over the tiles of this CTA: steps (B ring, MMA barriers), groups (TMEM buffers), Q chunks (A ring)
     int sb = 0, gb = 0, qb = 0, it = 0;
 
+    // Two control warps, each walking its own warp-uniform control flow with one elected lane acting: the MMA warp only
+    // waits for operands / a free accumulator and issues (a tcgen05.mma is accepted at the pace of the tensor pipe, so
+    // anything else this warp did between two chunks would leave the pipe idle); the copy warp streams the weight
+    // chunks and the raw Q chunks ahead of it, paced by the ring barriers alone.
     if (warp_u == CTL_WARP) {
-        {   // the whole warp walks the control flow (warp-uniform: descriptors in uniform registers); one lane acts
-            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
-            const uint32_t stg = c.a0 + 3u * A_SLOT;
-            for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
-                const DenseTile tile = A.tiles[tile_idx];
-                const DenseWT W = A.w[tile.species];
-                const float *Qt = A.Q + (size_t)tile_idx * A.K1 * TM;
-                c.sb = sb; c.gb = gb;
-                auto issue_q = [&](int j_loc) {   // raw Q chunk -> staging buffer (J & 1)
-                    const int j = qb + j_loc, qs = j & 1;
-                    if (j >= 2) mbar_wait(c.bar(BAR_QEMPTY + qs), (uint32_t)(((j >> 1) - 1) & 1));
-                    if (elect_one()) {
-                        mbar_expect_tx(c.bar(BAR_QFULL + qs), A_HALF);
-                        bulk_g2s(stg + (uint32_t)qs * A_HALF, Qt + (size_t)j_loc * (KC * TM), A_HALF, c.bar(BAR_QFULL + qs));
-                    }
-                    __syncwarp();
-                };
-                auto copy_b = [&](int i) {
-                    if (i < n1) c.copy_b(i, W.g1 + (size_t)i * (2 * H1p * KC), H1p);
-                    else c.copy_b(i, W.g2 + (size_t)(i - n1) * (2 * H2p * KC), H2p);
-                };
-                copy_b(0);
-                if (total > 1) copy_b(1);
-                // the staging area doubles as the fourth operand slot of GEMM 2: wait for the previous tile to be done
-                if (it > 0) mbar_wait(c.bar(BAR_TDONE), (uint32_t)((it - 1) & 1));
-                issue_q(0);
-                if (n1 > 1) issue_q(1);
-                for (int i = 0; i < total; ++i) {
-                    if (i < n1) {
-                        const int j = qb + i, sa = j % NSTAGE;
-                        mbar_wait(c.bar(BAR_AFULL + sa), (uint32_t)((j / NSTAGE) & 1));
-                        if (i + 2 < n1) issue_q(i + 2);
-                        TC_TRACE(0, 0, 2 * i);
-                        const uint32_t a_col = COL_A + A_TSLOT * (uint32_t)(i & 1);
-                        if (A.tf32) c.mma_chunk_1x_ts(i, a_col, H1p, 0, i == 0, i == n1 - 1);
-                        else c.mma_chunk_ts(i, a_col, H1p, i);
-                    } else {
-                        mbar_wait(c.bar(BAR_AH + (i - n1)), (uint32_t)(it & 1));
-                        TC_TRACE(0, 0, 2 * i);
-                        if (A.tf32) c.mma_chunk_1x(i, i - n1, H2p, 1, i == n1, i == total - 1);
-                        else c.mma_chunk(i, i - n1, H2p, i);
-                    }
-                    TC_TRACE(0, 0, 2 * i + 1);
-                    if (i + 2 < total) copy_b(i + 2);
+        Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
+        for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+            c.sb = sb; c.gb = gb;
+            for (int i = 0; i < total; ++i) {
+                if (i < n1) {
+                    const int j = qb + i, sa = j % NSTAGE;
+                    mbar_wait(c.bar(BAR_AFULL + sa), (uint32_t)((j / NSTAGE) & 1));
+                    TC_TRACE(0, 0, 2 * i);
+                    const uint32_t a_col = COL_A + A_TSLOT * (uint32_t)(i & 1);
+                    if (A.tf32) c.mma_chunk_1x_ts(i, a_col, H1p, 0, i == 0, i == n1 - 1);
+                    else c.mma_chunk_ts(i, a_col, H1p, i);
+                } else {
+                    mbar_wait(c.bar(BAR_AH + (i - n1)), (uint32_t)(it & 1));
+                    TC_TRACE(0, 0, 2 * i);
+                    if (A.tf32) c.mma_chunk_1x(i, i - n1, H2p, 1, i == n1, i == total - 1);
+                    else c.mma_chunk(i, i - n1, H2p, i);
                 }
-                sb += total; gb += A.tf32 ? 2 : total; qb += n1;
+                TC_TRACE(0, 0, 2 * i + 1);
             }
+            sb += total; gb += A.tf32 ? 2 : total; qb += n1;
+        }
+    } else if (warp_u == COPY_WARP) {
+        Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
+        const uint32_t stg = c.a0 + 3u * A_SLOT;
+        for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+            const DenseTile tile = A.tiles[tile_idx];
+            const DenseWT W = A.w[tile.species];
+            const float *Qt = A.Q + (size_t)tile_idx * A.K1 * TM;
+            c.sb = sb; c.gb = gb;
+            auto issue_q = [&](int j_loc) {   // raw Q chunk -> staging buffer (J & 1)
+                const int j = qb + j_loc, qs = j & 1;
+                if (j >= 2) mbar_wait(c.bar(BAR_QEMPTY + qs), (uint32_t)(((j >> 1) - 1) & 1));
+                if (elect_one()) {
+                    mbar_expect_tx(c.bar(BAR_QFULL + qs), A_HALF);
+                    bulk_g2s(stg + (uint32_t)qs * A_HALF, Qt + (size_t)j_loc * (KC * TM), A_HALF, c.bar(BAR_QFULL + qs));
+                }
+                __syncwarp();
+            };
+            auto copy_b = [&](int i) {
+                if (i < n1) c.copy_b(i, W.g1 + (size_t)i * (2 * H1p * KC), H1p);
+                else c.copy_b(i, W.g2 + (size_t)(i - n1) * (2 * H2p * KC), H2p);
+            };
+            copy_b(0);
+            if (total > 1) copy_b(1);
+            // the staging area doubles as the fourth operand slot of GEMM 2: wait for the previous tile to be done
+            if (it > 0) mbar_wait(c.bar(BAR_TDONE), (uint32_t)((it - 1) & 1));
+            issue_q(0);
+            if (n1 > 1) issue_q(1);
+            for (int i = 0; i < total; ++i) {
+                if (i + 2 < n1) issue_q(i + 2);       // waits for the conversion of chunk i (its staging half)
+                if (i + 2 < total) copy_b(i + 2);     // waits for the MMAs of step i - 1 (its ring slot)
+            }
+            sb += total; gb += A.tf32 ? 2 : total; qb += n1;
         }
     } else {
         const int m = (warp & 3) * 32 + lane, hf = warp >> 2;
@@ -548,59 +558,61 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
     const int nblk = (A.K1 + 127) / 128, total = i3 + nblk * NCH1, ngroups = i3 + nblk * (NCH1 / GR3);
     int sb = 0, gb = 0, it = 0;                     // running steps / groups / tiles of this CTA (persistent kernel)
 
+    auto rows_of = [&](int i) { return i < o1 ? H2p : i < i3 ? H1p : min(128, A.K1 - ((i - i3) / NCH1) * 128); };
     if (warp_u == CTL_WARP) {
-        {   // the whole warp walks the control flow (warp-uniform); one elected lane acts
-            Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
-            for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
-                const DenseTile tile = A.tiles[tile_idx];
-                const DenseWT W = A.w[tile.species];
-                c.sb = sb; c.gb = gb;
-                auto rows_of = [&](int i) { return i < o1 ? H2p : i < i3 ? H1p : min(128, A.K1 - ((i - i3) / NCH1) * 128); };
-                auto copy_b = [&](int i) {
-                    if (i < o1) { c.copy_b(i, W.r1, H2p); return; }
-                    if (i < i3) { c.copy_b(i, W.r2 + (size_t)(i - o1) * (2 * H1p * KC), H1p); return; }
-                    const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1, nr = rows_of(i);
-                    c.copy_b(i, W.r3 + (size_t)nb * NCH1 * (2 * 128 * KC) + (size_t)kc * (2 * nr * KC), nr);
-                };
-                copy_b(0);
-                if (total > 1) copy_b(1);
-                for (int i = 0; i < total; ++i) {
-                    if (i < o1) {
-                        mbar_wait(c.bar(BAR_AFULL), (uint32_t)(it & 1));
-                        TC_TRACE(1, 0, 2 * i);
-                        if (A.tf32) c.mma_chunk_1x(i, 0, H2p, 0, true, true);
-                        else c.mma_chunk(i, 0, H2p, i);
-                    } else if (i < i3) {
-                        mbar_wait(c.bar(BAR_AH + (i - o1)), (uint32_t)(it & 1));
-                        TC_TRACE(1, 0, 2 * i);
-                        if (A.tf32) c.mma_chunk_1x(i, i - o1, H1p, o1, i == o1, i == i3 - 1);
-                        else c.mma_chunk(i, i - o1, H1p, i);
-                    } else if (A.tf32) {
-                        // R3, plain TF32: one accumulator per block of <= 128 output columns (K = H1p)
-                        if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
-                        const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1;
-                        c.mma_chunk_1x(i, kc, rows_of(i), o1 + 1 + nb, kc == 0, kc == NCH1 - 1);
+        // MMA warp (see k_dense_tc_fwd): waits for operands / a free accumulator and issues, nothing else
+        Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
+        for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+            c.sb = sb; c.gb = gb;
+            for (int i = 0; i < total; ++i) {
+                if (i < o1) {
+                    mbar_wait(c.bar(BAR_AFULL), (uint32_t)(it & 1));
+                    TC_TRACE(1, 0, 2 * i);
+                    if (A.tf32) c.mma_chunk_1x(i, 0, H2p, 0, true, true);
+                    else c.mma_chunk(i, 0, H2p, i);
+                } else if (i < i3) {
+                    mbar_wait(c.bar(BAR_AH + (i - o1)), (uint32_t)(it & 1));
+                    TC_TRACE(1, 0, 2 * i);
+                    if (A.tf32) c.mma_chunk_1x(i, i - o1, H1p, o1, i == o1, i == i3 - 1);
+                    else c.mma_chunk(i, i - o1, H1p, i);
+                } else if (A.tf32) {
+                    // R3, plain TF32: one accumulator per block of <= 128 output columns (K = H1p)
+                    if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
+                    const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1;
+                    c.mma_chunk_1x(i, kc, rows_of(i), o1 + 1 + nb, kc == 0, kc == NCH1 - 1);
+                } else {
+                    // R3: groups of GR3 chunks (K = 32 GR3 per accumulator); group index continues after R2
+                    if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
+                    const int kc = (i - i3) % NCH1, g = i3 + (i - i3) / GR3;
+                    TC_TRACE(1, 0, 2 * i);
+                    if (GR3 == 2) {
+                        c.mma_pair(i, kc, kc + 1, rows_of(i), g);
+                        TC_TRACE(1, 0, 2 * i + 1);
+                        ++i;
+                        continue;
                     } else {
-                        // R3: groups of GR3 chunks (K = 32 GR3 per accumulator); group index continues after R2
-                        if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
-                        const int kc = (i - i3) % NCH1, g = i3 + (i - i3) / GR3;
-                        TC_TRACE(1, 0, 2 * i);
-                        if (GR3 == 2) {
-                            if (i + 2 < total) copy_b(i + 2);          // in flight during this group's MMAs
-                            c.mma_pair(i, kc, kc + 1, rows_of(i), g);
-                            if (i + 3 < total) copy_b(i + 3);          // waits for the hi.hi MMAs of chunk i
-                            TC_TRACE(1, 0, 2 * i + 1);
-                            ++i;
-                            continue;
-                        } else {
-                            c.mma_chunk(i, kc, rows_of(i), g);
-                        }
+                        c.mma_chunk(i, kc, rows_of(i), g);
                     }
-                    TC_TRACE(1, 0, 2 * i + 1);
-                    if (i + 2 < total) copy_b(i + 2);
                 }
-                sb += total; gb += A.tf32 ? o1 + 1 + nblk : ngroups;
+                TC_TRACE(1, 0, 2 * i + 1);
             }
+            sb += total; gb += A.tf32 ? o1 + 1 + nblk : ngroups;
+        }
+    } else if (warp_u == COPY_WARP) {
+        // copy warp: the weight chunks of every step, as far ahead as the ring allows (a slot is free when the MMAs of
+        // the step three back have completed)
+        Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
+        for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
+            const DenseTile tile = A.tiles[tile_idx];
+            const DenseWT W = A.w[tile.species];
+            c.sb = sb; c.gb = gb;
+            for (int i = 0; i < total; ++i) {
+                if (i < o1) { c.copy_b(i, W.r1, H2p); continue; }
+                if (i < i3) { c.copy_b(i, W.r2 + (size_t)(i - o1) * (2 * H1p * KC), H1p); continue; }
+                const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1, nr = rows_of(i);
+                c.copy_b(i, W.r3 + (size_t)nb * NCH1 * (2 * 128 * KC) + (size_t)kc * (2 * nr * KC), nr);
+            }
+            sb += total; gb += A.tf32 ? o1 + 1 + nblk : ngroups;
         }
     } else {
         const int m = (warp & 3) * 32 + lane, hf = warp >> 2;

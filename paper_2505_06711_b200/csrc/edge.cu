@@ -922,7 +922,6 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 }
 
 // upper bound of the grid of the edge backward kernel (= entries of the virial partial array)
-int edge_bwd_blocks(int64_t N) { return (int)std::max<int64_t>(N, 1); }   // one-warp blocks in the one-edge-per-lane shape
 static int sm_count() {
     static int n_sm[64] = {};
     int dev = 0;
@@ -931,6 +930,13 @@ static int sm_count() {
     if (!n_sm[dev] && (cudaDeviceGetAttribute(&n_sm[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm[dev] <= 0))
         n_sm[dev] = 148;
     return n_sm[dev];
+}
+// upper bound of the grid of the edge backward kernel (= entries of the virial partial array): one-warp blocks, one per
+// atom, in the one-edge-per-lane shape; a persistent grid of MINB blocks per SM in the two-edges-per-lane shape
+int edge_bwd_blocks(int64_t N, int Na) {
+    const int64_t n = std::max<int64_t>(N, 1);
+    const bool two = Na % 2 == 0 && Na <= 10;               // BwdShape<NA>::NE == 2
+    return (int)(two ? std::min<int64_t>((n + EW - 1) / EW, (int64_t)3 * sm_count()) : n);
 }
 
 int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
