@@ -477,6 +477,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
             float o[16];
 #pragma unroll
             for (int c = 0; c < 16; ++c) o[c] = 0.f;
+            // z2 = acc + b2 (stash), h2 = SiLU(z2) in place
 #pragma unroll
             for (int k4 = 0; k4 < CW2 / 4; ++k4) {
                 const int col = hf * CW2 + k4 * 4;
@@ -484,21 +485,28 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 const float4 z = make_float4(acc2[k4 * 4] + b4.x, acc2[k4 * 4 + 1] + b4.y, acc2[k4 * 4 + 2] + b4.z,
                                              acc2[k4 * 4 + 3] + b4.w);
                 if (valid) *reinterpret_cast<float4 *>(zt + (size_t)((H1p + col) >> 2) * (TM * 4)) = z;
-                const float hv[4] = {silu_f(z.x), silu_f(z.y), silu_f(z.z), silu_f(z.w)};
-                if (A.nout == 1) {
-                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + col));
-                    o[0] = fmaf(hv[0], w4.x, o[0]); o[0] = fmaf(hv[1], w4.y, o[0]);
-                    o[0] = fmaf(hv[2], w4.z, o[0]); o[0] = fmaf(hv[3], w4.w, o[0]);
-                } else {
+                acc2[k4 * 4] = silu_f(z.x); acc2[k4 * 4 + 1] = silu_f(z.y);
+                acc2[k4 * 4 + 2] = silu_f(z.z); acc2[k4 * 4 + 3] = silu_f(z.w);
+            }
+            if (A.nout == 1) {          // energy layer: one column of W3, four partial sums
+                float o4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const float4 *wr = reinterpret_cast<const float4 *>(W.w3p + (size_t)(col + u) * 16);
+                for (int k4 = 0; k4 < CW2 / 4; ++k4) {
+                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(W.w3c0 + hf * CW2 + k4 * 4));
+                    o4[0] = fmaf(acc2[k4 * 4], w4.x, o4[0]); o4[1] = fmaf(acc2[k4 * 4 + 1], w4.y, o4[1]);
+                    o4[2] = fmaf(acc2[k4 * 4 + 2], w4.z, o4[2]); o4[3] = fmaf(acc2[k4 * 4 + 3], w4.w, o4[3]);
+                }
+                o[0] = (o4[0] + o4[1]) + (o4[2] + o4[3]);
+            } else {
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const float4 w4 = __ldg(wr + q);
-                            o[q * 4] = fmaf(hv[u], w4.x, o[q * 4]); o[q * 4 + 1] = fmaf(hv[u], w4.y, o[q * 4 + 1]);
-                            o[q * 4 + 2] = fmaf(hv[u], w4.z, o[q * 4 + 2]); o[q * 4 + 3] = fmaf(hv[u], w4.w, o[q * 4 + 3]);
-                        }
+                for (int c = 0; c < CW2; ++c) {
+                    const float4 *wr = reinterpret_cast<const float4 *>(W.w3p + (size_t)(hf * CW2 + c) * 16);
+                    const float hvc = acc2[c];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const float4 w4 = __ldg(wr + q);
+                        o[q * 4] = fmaf(hvc, w4.x, o[q * 4]); o[q * 4 + 1] = fmaf(hvc, w4.y, o[q * 4 + 1]);
+                        o[q * 4 + 2] = fmaf(hvc, w4.z, o[q * 4 + 2]); o[q * 4 + 3] = fmaf(hvc, w4.w, o[q * 4 + 3]);
                     }
                 }
             }
