@@ -54,7 +54,7 @@ constexpr int B_SLOT = 2 * 128 * KC * 4; // 32 KB (N <= 128)
 constexpr int SM_A = 0, SM_B = NASLOT * A_SLOT, SM_BAR = SM_B + NSTAGE * B_SLOT;
 constexpr int SM_TOTAL = SM_BAR + 256;
 constexpr uint32_t A_LBO = TM * 16;
-constexpr int NCOMPUTE = 256, NTHREADS = NCOMPUTE + 96, CTL_WARP = 8, COPY_WARP = 9, CTL2_WARP = 10;   // warps 8 and 10 issue the MMAs (alternate accumulator groups), warp 9 the bulk copies
+constexpr int NCOMPUTE = 256, NTHREADS = NCOMPUTE + 64, CTL_WARP = 8, COPY_WARP = 9;   // warp 8 issues the MMAs, warp 9 the bulk copies
 constexpr uint32_t COL_BUF = 128;      // TMEM columns per group buffer
 constexpr int NBUF = 3;                // group buffers: one filling, one complete, one being drained
 constexpr uint32_t TMEM_COLS = 512;    // allocation (power of two >= NBUF * COL_BUF)
@@ -139,7 +139,6 @@ struct Ctl {
     uint32_t bar0, a0, b0, tmem;
     int sb, gb;
     bool tf32;   // REANN_MLP_MODE=tf32: hi images only, one accumulator per GEMM (see mma_chunk_1x)
-    bool act = true;   // this warp issues the MMAs of the current group (the other MMA warp only follows the barriers)
     __device__ __forceinline__ uint32_t bar(int k) const { return bar0 + 8u * (uint32_t)k; }
     // stream the weight chunk of step i into its B slot (after the MMAs of step i-3 released it)
     __device__ __forceinline__ void copy_b(int i_loc, const float *src, int n_rows) const {
@@ -162,7 +161,7 @@ struct Ctl {
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        if (act && elect_one()) {
+        if (elect_one()) {
             issue(i, a_slot, n_rows, dm, true, false, true);
             issue(i, a_slot, n_rows, dm, false, true, false);
             tc_commit(bar(BAR_MMA + s));
@@ -179,7 +178,7 @@ struct Ctl {
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        if (act && elect_one()) {
+        if (elect_one()) {
             issue(i, a_slot, n_rows, dm, false, true, first);
             tc_commit(bar(BAR_MMA + s));
             if (last) tc_commit(bar(BAR_DFULL + d));
@@ -195,7 +194,7 @@ struct Ctl {
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        if (act && elect_one()) {
+        if (elect_one()) {
             issue_ts(i, a_col, n_rows, dm, true, false, true);
             issue_ts(i, a_col, n_rows, dm, false, true, false);
             tc_commit(bar(BAR_MMA + s));
@@ -210,7 +209,7 @@ struct Ctl {
         mbar_wait(bar(BAR_BFULL + s), (uint32_t)((i / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        if (act && elect_one()) {
+        if (elect_one()) {
             issue_ts(i, a_col, n_rows, dm, false, true, first);
             tc_commit(bar(BAR_MMA + s));
             if (last) tc_commit(bar(BAR_DFULL + d));
@@ -242,7 +241,7 @@ struct Ctl {
         mbar_wait(bar(BAR_BFULL + (i + 1) % NSTAGE), (uint32_t)(((i + 1) / NSTAGE) & 1));
         tc_fence_after();
         const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
-        if (act && elect_one()) {
+        if (elect_one()) {
             issue(i, a_slot0, n_rows, dm, true, false, true);
             issue(i + 1, a_slot1, n_rows, dm, true, false, false);
             issue(i, a_slot0, n_rows, dm, false, true, false);
@@ -348,17 +347,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
     // waits for operands / a free accumulator and issues (a tcgen05.mma is accepted at the pace of the tensor pipe, so
     // anything else this warp did between two chunks would leave the pipe idle); the copy warp streams the weight
     // chunks and the raw Q chunks ahead of it, paced by the ring barriers alone.
-    if (warp_u == CTL_WARP || warp_u == CTL2_WARP) {
-        // Both MMA warps follow every barrier (mbarrier waits go by phase parity: none may be skipped), but a group of
-        // MMAs is issued by one of them in turn: while one is held inside the issue of group g at the pace of the
-        // tensor pipe, the other has already passed the waits of group g + 1 and queues right behind it. Groups are
-        // independent accumulators. Plain TF32 (one accumulator per GEMM, order matters): warp 8 issues everything.
-        const int which = warp_u == CTL_WARP ? 0 : 1;
+    if (warp_u == CTL_WARP) {
         Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
         for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
             c.sb = sb; c.gb = gb;
             for (int i = 0; i < total; ++i) {
-                c.act = A.tf32 ? which == 0 : ((sb + i) & 1) == which;
                 if (i < n1) {
                     const int j = qb + i, sa = j % NSTAGE;
                     mbar_wait(c.bar(BAR_AFULL + sa), (uint32_t)((j / NSTAGE) & 1));
@@ -574,17 +567,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
     int sb = 0, gb = 0, it = 0;                     // running steps / groups / tiles of this CTA (persistent kernel)
 
     auto rows_of = [&](int i) { return i < o1 ? H2p : i < i3 ? H1p : min(128, A.K1 - ((i - i3) / NCH1) * 128); };
-    if (warp_u == CTL_WARP || warp_u == CTL2_WARP) {
-        // the two MMA warps (see k_dense_tc_fwd): both follow every barrier, accumulator groups are issued in turn
-        const int which = warp_u == CTL_WARP ? 0 : 1;
+    if (warp_u == CTL_WARP) {
+        // MMA warp (see k_dense_tc_fwd): waits for operands / a free accumulator and issues, nothing else
         Ctl c{bar0, smem_u32(smem + SM_A), smem_u32(smem + SM_B), tmem, 0, 0, A.tf32 != 0};
         for (int tile_idx = blockIdx.x; tile_idx < A.n_tiles; tile_idx += gridDim.x, ++it) {
             c.sb = sb; c.gb = gb;
             for (int i = 0; i < total; ++i) {
-                {   // group of step i: R1 / R2 one step each, R3 pairs of steps
-                    const int grp = i < i3 ? i : i3 + (i - i3) / GR3;
-                    c.act = A.tf32 ? which == 0 : ((gb + grp) & 1) == which;
-                }
                 if (i < o1) {
                     mbar_wait(c.bar(BAR_AFULL), (uint32_t)(it & 1));
                     TC_TRACE(1, 0, 2 * i);
