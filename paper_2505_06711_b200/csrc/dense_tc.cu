@@ -252,6 +252,46 @@ struct Ctl {
         }
         __syncwarp();
     }
+    // mma_pair with the hi image of the A operand in tensor memory (columns a_col0 / a_col1) and the lo image in the
+    // shared-memory slots: two of the three products per K step then read only B from shared memory
+    __device__ __forceinline__ void mma_pair_mixed(int i_loc, int a_slot0, int a_slot1, uint32_t a_col0, uint32_t a_col1, int n_rows,
+                                                   int g_loc) const {
+        const int i = sb + i_loc, g = gb + g_loc;
+        const int d = g % NBUF;
+        if (g >= NBUF) mbar_wait(bar(BAR_DEMPTY + d), (uint32_t)(((g / NBUF) - 1) & 1));
+        mbar_wait(bar(BAR_BFULL + i % NSTAGE), (uint32_t)((i / NSTAGE) & 1));
+        mbar_wait(bar(BAR_BFULL + (i + 1) % NSTAGE), (uint32_t)(((i + 1) / NSTAGE) & 1));
+        tc_fence_after();
+        const uint32_t dm = tmem + COL_BUF * (uint32_t)d;
+        if (elect_one()) {
+            issue_mixed(i, a_slot0, a_col0, n_rows, dm, true, false, true);
+            issue_mixed(i + 1, a_slot1, a_col1, n_rows, dm, true, false, false);
+            issue_mixed(i, a_slot0, a_col0, n_rows, dm, false, true, false);
+            tc_commit(bar(BAR_MMA + i % NSTAGE));
+            issue_mixed(i + 1, a_slot1, a_col1, n_rows, dm, false, true, false);
+            tc_commit(bar(BAR_MMA + (i + 1) % NSTAGE));
+            tc_commit(bar(BAR_DFULL + d));
+        }
+        __syncwarp();
+    }
+    __device__ __forceinline__ void issue_mixed(int i, int a_slot, uint32_t a_col, int n_rows, uint32_t dm, bool corr, bool main,
+                                                bool fresh) const {
+        const int s = i % NSTAGE;
+        const uint32_t idesc = make_idesc(n_rows);
+        const uint32_t a_lo = a0 + (uint32_t)a_slot * A_SLOT + A_HALF, a_hi = tmem + a_col;
+        const uint32_t b_lbo = (uint32_t)n_rows * 16;
+        const uint32_t b_hi = b0 + (uint32_t)s * B_SLOT, b_lo = b_hi + (uint32_t)n_rows * KC * 4;
+#pragma unroll
+        for (int kk = 0; kk < KC / 8; ++kk) {
+            const uint64_t al = make_desc(a_lo + kk * 2 * A_LBO, A_LBO);
+            const uint64_t bh = make_desc(b_hi + kk * 2 * b_lbo, b_lbo), bl = make_desc(b_lo + kk * 2 * b_lbo, b_lbo);
+            if (corr) {
+                umma_tf32(dm, al, bh, idesc, (fresh && kk == 0) ? 0u : 1u);
+                umma_tf32_ts(dm, a_hi + kk * 8, bl, idesc, 1u);
+            }
+            if (main) umma_tf32_ts(dm, a_hi + kk * 8, bh, idesc, (fresh && !corr && kk == 0) ? 0u : 1u);
+        }
+    }
     // the MMAs of one chunk: corrections (A_lo B_hi + A_hi B_lo) and / or main (A_hi B_hi); fresh: overwrite D first
     __device__ __forceinline__ void issue(int i, int a_slot, int n_rows, uint32_t dm, bool corr, bool main, bool fresh) const {
         const int s = i % NSTAGE;
@@ -594,7 +634,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                     const int kc = (i - i3) % NCH1, g = i3 + (i - i3) / GR3;
                     TC_TRACE(1, 0, 2 * i);
                     if (GR3 == 2) {
-                        c.mma_pair(i, kc, kc + 1, rows_of(i), g);
+                        c.mma_pair_mixed(i, kc, kc + 1, COL_A + KC * (uint32_t)kc, COL_A + KC * (uint32_t)(kc + 1), rows_of(i), g);
                         TC_TRACE(1, 0, 2 * i + 1);
                         ++i;
                         continue;
@@ -709,7 +749,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                     const float xv[4] = {valid ? h1b[k4 * 4] * dsilu_f(z.x) : 0.f, valid ? h1b[k4 * 4 + 1] * dsilu_f(z.y) : 0.f,
                                          valid ? h1b[k4 * 4 + 2] * dsilu_f(z.z) : 0.f, valid ? h1b[k4 * 4 + 3] * dsilu_f(z.w) : 0.f};
                     store_split4(a_base + (col >> 5) * A_SLOT, (col & 31) >> 2, m, xv);
+                    // R3 reads the hi image from tensor memory (column = K index), the lo image from the slot
+                    uint32_t hb[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { float h, l; split_tf32(xv[u], h, l); hb[u] = __float_as_uint(h); }
+                    tmem_st4(tl + COL_A + (uint32_t)col, hb);
                 }
+                tmem_wait_st();
+                tc_fence_before();
                 fence_async_smem();
                 mbar_arrive(bar0 + 8 * BAR_ARES);
             }
