@@ -355,6 +355,21 @@ __device__ __forceinline__ void store_operand(const float *x, unsigned char *a_b
 #pragma unroll
     for (int c = 0; c < (CW + 31) / 32; ++c) mbar_arrive(bar0 + 8 * (BAR_AH + (col0 >> 5) + c));
 }
+// The same, four columns at a time from inside the activation loop: x4 = columns [col0 + 4 k4, + 4) of row m. A 32-column
+// chunk is published as soon as this thread's share of it is written, so that the next GEMM starts on the first chunks
+// while the threads are still working on the later ones.
+template <int CW>
+__device__ __forceinline__ void store4_publish(const float *x4, unsigned char *a_base, uint32_t bar0, int col0, int k4, int m) {
+    const int col = col0 + 4 * k4;
+    store_split4(a_base + (col >> 5) * A_SLOT, (col & 31) >> 2, m, x4);
+    if (((col + 4) & 31) == 0 || k4 == CW / 4 - 1) {
+        fence_async_smem();
+        mbar_arrive(bar0 + 8 * (BAR_AH + (col >> 5)));
+    }
+}
+// Order in which the K chunks of a GEMM whose A operand comes out of an activation phase are consumed: the two column
+// halves of the compute threads finish their chunks in parallel (0 and NCH/2 first), so the chunks are taken alternately
+__host__ __device__ constexpr int chunk_order(int k, int nch) { return nch >= 4 ? ((k & 1) ? nch / 2 + k / 2 : k / 2) : k; }
 __host__ __device__ constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 // ============================================================================ forward
@@ -400,10 +415,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                     if (A.tf32) c.mma_chunk_1x_ts(i, a_col, H1p, 0, i == 0, i == n1 - 1);
                     else c.mma_chunk_ts(i, a_col, H1p, i);
                 } else {
-                    mbar_wait(c.bar(BAR_AH + (i - n1)), (uint32_t)(it & 1));
+                    const int kq = chunk_order(i - n1, NCH1);
+                    mbar_wait(c.bar(BAR_AH + kq), (uint32_t)(it & 1));
                     TC_TRACE(0, 0, 2 * i);
-                    if (A.tf32) c.mma_chunk_1x(i, i - n1, H2p, 1, i == n1, i == total - 1);
-                    else c.mma_chunk(i, i - n1, H2p, i);
+                    if (A.tf32) c.mma_chunk_1x(i, kq, H2p, 1, i == n1, i == total - 1);
+                    else c.mma_chunk(i, kq, H2p, i);
                 }
                 TC_TRACE(0, 0, 2 * i + 1);
             }
@@ -428,7 +444,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
             };
             auto copy_b = [&](int i) {
                 if (i < n1) c.copy_b(i, W.g1 + (size_t)i * (2 * H1p * KC), H1p);
-                else c.copy_b(i, W.g2 + (size_t)(i - n1) * (2 * H2p * KC), H2p);
+                else c.copy_b(i, W.g2 + (size_t)chunk_order(i - n1, NCH1) * (2 * H2p * KC), H2p);
             };
             copy_b(0);
             if (total > 1) copy_b(1);
@@ -498,10 +514,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 const float4 z = make_float4(acc1[k4 * 4] + b4.x, acc1[k4 * 4 + 1] + b4.y, acc1[k4 * 4 + 2] + b4.z,
                                              acc1[k4 * 4 + 3] + b4.w);
                 if (valid) *reinterpret_cast<float4 *>(zt + (size_t)(col >> 2) * (TM * 4)) = z;
-                acc1[k4 * 4] = silu_f(z.x); acc1[k4 * 4 + 1] = silu_f(z.y);
-                acc1[k4 * 4 + 2] = silu_f(z.z); acc1[k4 * 4 + 3] = silu_f(z.w);
+                const float h4[4] = {silu_f(z.x), silu_f(z.y), silu_f(z.z), silu_f(z.w)};
+                store4_publish<CW1>(h4, a_base, bar0, hf * CW1, k4, m);
             }
-            store_operand<CW1>(acc1, a_base, bar0, hf * CW1, m);
             if (tid == 0) TC_TRACE(0, 1, 102);
             // ---- GEMM 2: z2 = h1 W2 ----
             float acc2[CW2];
@@ -619,10 +634,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                     if (A.tf32) c.mma_chunk_1x(i, 0, H2p, 0, true, true);
                     else c.mma_chunk(i, 0, H2p, i);
                 } else if (i < i3) {
-                    mbar_wait(c.bar(BAR_AH + (i - o1)), (uint32_t)(it & 1));
+                    const int kq = chunk_order(i - o1, NCH2);
+                    mbar_wait(c.bar(BAR_AH + kq), (uint32_t)(it & 1));
                     TC_TRACE(1, 0, 2 * i);
-                    if (A.tf32) c.mma_chunk_1x(i, i - o1, H1p, o1, i == o1, i == i3 - 1);
-                    else c.mma_chunk(i, i - o1, H1p, i);
+                    if (A.tf32) c.mma_chunk_1x(i, kq, H1p, o1, i == o1, i == i3 - 1);
+                    else c.mma_chunk(i, kq, H1p, i);
                 } else if (A.tf32) {
                     // R3, plain TF32: one accumulator per block of <= 128 output columns (K = H1p)
                     if (i == i3) mbar_wait(c.bar(BAR_ARES), (uint32_t)(it & 1));
@@ -656,7 +672,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
             c.sb = sb; c.gb = gb;
             for (int i = 0; i < total; ++i) {
                 if (i < o1) { c.copy_b(i, W.r1, H2p); continue; }
-                if (i < i3) { c.copy_b(i, W.r2 + (size_t)(i - o1) * (2 * H1p * KC), H1p); continue; }
+                if (i < i3) { c.copy_b(i, W.r2 + (size_t)chunk_order(i - o1, NCH2) * (2 * H1p * KC), H1p); continue; }
                 const int nb = (i - i3) / NCH1, kc = (i - i3) % NCH1, nr = rows_of(i);
                 c.copy_b(i, W.r3 + (size_t)nb * NCH1 * (2 * 128 * KC) + (size_t)kc * (2 * nr * KC), nr);
             }
@@ -717,12 +733,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_bwd(TcBwdArgs A) {
                 }
 #pragma unroll
                 for (int k4 = 0; k4 < CW2 / 4; ++k4) {
-                    x[k4 * 4] = valid ? x[k4 * 4] * dsilu_f(z2[k4].x) : 0.f;
-                    x[k4 * 4 + 1] = valid ? x[k4 * 4 + 1] * dsilu_f(z2[k4].y) : 0.f;
-                    x[k4 * 4 + 2] = valid ? x[k4 * 4 + 2] * dsilu_f(z2[k4].z) : 0.f;
-                    x[k4 * 4 + 3] = valid ? x[k4 * 4 + 3] * dsilu_f(z2[k4].w) : 0.f;
+                    const float x4[4] = {valid ? x[k4 * 4] * dsilu_f(z2[k4].x) : 0.f, valid ? x[k4 * 4 + 1] * dsilu_f(z2[k4].y) : 0.f,
+                                         valid ? x[k4 * 4 + 2] * dsilu_f(z2[k4].z) : 0.f, valid ? x[k4 * 4 + 3] * dsilu_f(z2[k4].w) : 0.f};
+                    store4_publish<CW2>(x4, a_base, bar0, hf * CW2, k4, m);
                 }
-                store_operand<CW2>(x, a_base, bar0, hf * CW2, m);
             }
             if (tid == 0) TC_TRACE(1, 1, 101);
             // ---- GEMM R2: h1bar = z2bar W2^T; z1bar = h1bar SiLU'(z1) -> resident A operand of GEMM R3 ----
