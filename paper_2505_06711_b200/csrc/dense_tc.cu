@@ -528,6 +528,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 for (int kc = 0; kc < NCH1; ++kc) drain_group<CW2>(acc2, bar0, tl, gb + n1 + kc, hf * CW2, true);
             }
             if (tid == 0) TC_TRACE(0, 1, 103);
+            // every MMA of the tile has completed (its last group is drained): the staging area may take the next tile's
+            // first Q chunks while this tile's second activation phase runs
+            if (tid == 0) mbar_arrive(bar0 + 8 * BAR_TDONE);
             // ---- z2 (stash), h2 = SiLU(z2), out = h2 W3 + b3 in FP32 (partial over this column half) ----
             float o[16];
 #pragma unroll
@@ -585,9 +588,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_dense_tc_fwd(TcFwdArgs A) {
                 }
             }
             if (tid == 0) TC_TRACE(0, 1, 104);
-            // tile done: the operand slots (and the exchange area) may be reused by the next tile
+            // tile done: the exchange area (operand slot 0) is next written in the first activation phase of the next
+            // tile, which every thread reaches only through that tile's GEMM 1 barriers
             compute_sync();
-            if (tid == 0) mbar_arrive(bar0 + 8 * BAR_TDONE);
             sb += total; gb += A.tf32 ? 2 : total; qb += n1;
         }
     }
