@@ -593,16 +593,6 @@ __device__ __forceinline__ void edge_bwd_pass(int64_t e0, int64_t end, const uin
     }
 }
 
-__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async4(void *dst_smem, const void *src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N_>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
-
 // Persistent warps: a warp walks over atoms (stride = warps of the grid); bbar_i and the records of the row's first
 // 64 edges of the NEXT atom arrive by cp.async while the current atom is processed (double-buffered in shared
 // memory, no registers held), so an atom starts without waiting on DRAM.

@@ -9,6 +9,8 @@
 //   row-major (SIMT path, dense.cu):               [p][KQ = nqp], row p belongs to atom sp_list[p].
 // Column q = l * NPp + pair(n, n'), pair(n, n') = n nphi - n (n - 1) / 2 + (n' - n); columns that
 // are padding are written as zeros.
+#include <algorithm>
+
 #include "common.cuh"
 #include "edge_common.cuh"
 
@@ -67,6 +69,24 @@ __device__ __forceinline__ RowId row_of_block(const DenseTile *__restrict__ tile
         if (r.p >= N) r.p = -1;
     }
     return r;
+}
+// the same for group g of 8 rows (persistent kernels walk over groups): tile-quad mode g = (tile, group of 8 rows)
+__device__ __forceinline__ RowId row_of_group(const DenseTile *__restrict__ tiles, int64_t N, int64_t g, int warp) {
+    RowId r;
+    if (tiles) {
+        r.tile = (int)(g >> 4); r.r0 = (int)(g & 15) * 8;
+        const DenseTile t = tiles[r.tile];
+        r.p = (r.r0 + warp < t.count) ? (int64_t)t.start + r.r0 + warp : -1;
+    } else {
+        r.tile = 0; r.r0 = 0;
+        r.p = g * GW + warp;
+        if (r.p >= N) r.p = -1;
+    }
+    return r;
+}
+__device__ __forceinline__ int64_t quad_index_g(const DenseTile *tiles, const RowId &r, int64_t g, int r8, int q4, int KQ) {
+    if (tiles) return ((int64_t)r.tile * (KQ >> 2) + q4) * DENSE_TC_TM + r.r0 + r8;
+    return (g * GW + r8) * (KQ >> 2) + q4;
 }
 // float4 index in global memory of (row r8 of this block, column quad q4)
 __device__ __forceinline__ int64_t quad_index(const DenseTile *tiles, const RowId &r, int r8, int q4, int KQ) {
@@ -206,161 +226,164 @@ struct BwdCfg {
     static constexpr int PER_WARP = NA * TS + NPHIP * NA;             // floats: bT | outs
 };
 
+// Persistent: a block walks over groups of 8 rows (one warp = one row); the Qbar rows and the b rows of the NEXT group
+// arrive by cp.async while the current group is computed (double-buffered in shared memory), so the kernel streams at
+// the pace of HBM instead of waiting out a DRAM round trip per group.
 template <int NPHIP, int NA>
-__global__ void __launch_bounds__(GW * 32, 4) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
+__global__ void __launch_bounds__(GW * 32, 3) k_gram_bwd(int64_t N, const int32_t *__restrict__ sp_list,
                                                       const DenseTile *__restrict__ tiles,
                                                       const float *__restrict__ b, const float *__restrict__ Qbar,
-                                                      float *__restrict__ bbar, int nphi, int NPp, int KQ, const int32_t *__restrict__ skip) {
+                                                      float *__restrict__ bbar, int nphi, int NPp, int KQ, int64_t n_groups,
+                                                      const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
     using C = BwdCfg<NPHIP, NA>;
-    constexpr int NB = NPHIP * NA;
+    constexpr int NB = NPHIP * NA, WORK = NA == 20 ? NB : C::PER_WARP;
     extern __shared__ __align__(16) float sm[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, QS = KQ + 4;
-    float *bT = sm + warp * C::PER_WARP, *outs = bT + NA * C::TS, *q0 = sm + GW * C::PER_WARP, *qs = q0 + warp * QS;
-    const RowId row = row_of_block(tiles, N, warp);
-    if (!tiles && (int64_t)blockIdx.x * GW >= N) return;
-    // ---- block: the 8 Qbar rows, full lines ----
-    {
-        const float4 *Q4 = reinterpret_cast<const float4 *>(Qbar);
-        const int nq4 = KQ >> 2;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, QS = KQ + 4, RS = QS + NB;   // row of a buffer: Qbar row | b row
+    float *work = sm + (size_t)2 * GW * RS + warp * WORK;
+    const float4 *Q4 = reinterpret_cast<const float4 *>(Qbar);
+    const int nq4 = KQ >> 2;
+    auto issue = [&](int64_t g, int buf) {
+        float *in = sm + (size_t)buf * GW * RS;
+        const RowId row = row_of_group(tiles, N, g, warp);
         if (tiles) {
             for (int idx = threadIdx.x; idx < GW * nq4; idx += GW * 32) {
                 const int q4 = idx >> 3, r8 = idx & 7;
-                *reinterpret_cast<float4 *>(q0 + r8 * QS + q4 * 4) = __ldg(Q4 + quad_index(tiles, row, r8, q4, KQ));
+                edge::cp_async16(in + r8 * RS + q4 * 4, Q4 + quad_index_g(tiles, row, g, r8, q4, KQ));
             }
         } else {
             for (int idx = threadIdx.x; idx < GW * nq4; idx += GW * 32) {
                 const int r8 = idx / nq4, q4 = idx - r8 * nq4;
-                if ((int64_t)blockIdx.x * GW + r8 < N)
-                    *reinterpret_cast<float4 *>(q0 + r8 * QS + q4 * 4) = __ldg(Q4 + quad_index(tiles, row, r8, q4, KQ));
+                if (g * GW + r8 < N) edge::cp_async16(in + r8 * RS + q4 * 4, Q4 + quad_index_g(tiles, row, g, r8, q4, KQ));
             }
         }
-    }
-    int64_t atom = 0;
-    if constexpr (NA == 20) {
-        // bbar_l = mu . (G_l B_l) per l on the tensor cores: M = n (16), K = n' (two steps of 8), N = the monomials of degree l
-        // in tiles of 8 (l = 0: 1 of 8 columns used, l = 1: 3, l = 2: 6, l = 3: 8 + 2). A fragments = G_l gathered from the
-        // triangular Qbar row, B fragments = b (row-major in shared memory, no transposed copy), 3xTF32.
-        float *bs = bT;                                  // row-major b_i [n][a] in the first NB floats of the warp's area
         if (row.p >= 0) {
-            atom = sp_list[row.p];
-            const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
-#pragma unroll
-            for (int f = lane; f < NB / 4; f += 32) reinterpret_cast<float4 *>(bs)[f] = __ldg(bi + f);
+            const float4 *bi = reinterpret_cast<const float4 *>(b + (int64_t)sp_list[row.p] * NB);
+            for (int f = lane; f < NB / 4; f += 32) edge::cp_async16(in + warp * RS + QS + f * 4, bi + f);
         }
-        __syncthreads();
-        if (row.p < 0) return;
-        const int g8 = lane >> 2, t4 = lane & 3;
-        int gi[2][4];
-        float gf[2][4];
+    };
+    // lane constants of the tensor-core path: triangular offsets and (1 + delta) factors of this lane's A-fragment elements
+    const int g8 = lane >> 2, t4 = lane & 3;
+    int gi[2][4];
+    float gf[2][4];
 #pragma unroll
-        for (int k = 0; k < 2; ++k)
+    for (int k = 0; k < 2; ++k)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int n = g8 + 8 * (c & 1), m = 8 * k + t4 + 4 * (c >> 1);       // a0 (g, t), a1 (g+8, t), a2 (g, t+4), a3 (g+8, t+4)
-                const int lo = min(n, m), hi = max(n, m);
-                const bool ok = n < nphi && m < nphi;
-                gi[k][c] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
-                gf[k][c] = ok ? (n == m ? 2.0f : 1.0f) : 0.0f;
-            }
-        constexpr int NTL = 5;
-        constexpr int NT_A0[NTL] = {0, 1, 4, 10, 18}, NT_CNT[NTL] = {1, 3, 6, 8, 2}, NT_L[NTL] = {0, 1, 2, 3, 3};
-        uint32_t ah[2][4], al[2][4];
-#pragma unroll
-        for (int nt = 0; nt < NTL; ++nt) {
-            if (nt == 0 || NT_L[nt] != NT_L[nt - 1]) {
-                const float *ql = qs + NT_L[nt] * NPp;
-#pragma unroll
-                for (int k = 0; k < 2; ++k)
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) edge::split_bits(ql[gi[k][c]] * gf[k][c], ah[k][c], al[k][c]);
-            }
-            float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            const int a = NT_A0[nt] + g8;
-            const bool va = g8 < NT_CNT[nt];
-            uint32_t bh[2][2], bl[2][2];
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                const int r0 = 8 * k + t4, r1 = r0 + 4;
-                edge::split_bits((va && r0 < NPHIP) ? bs[r0 * NA + a] : 0.f, bh[k][0], bl[k][0]);
-                edge::split_bits((va && r1 < NPHIP) ? bs[r1 * NA + a] : 0.f, bh[k][1], bl[k][1]);
-            }
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                if (k == 1 && NPHIP <= 8) continue;
-                edge::mma_tf32(acc, al[k], bh[k][0], bh[k][1]);
-                edge::mma_tf32(acc, ah[k], bl[k][0], bl[k][1]);
-            }
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                if (k == 1 && NPHIP <= 8) continue;
-                edge::mma_tf32(acc, ah[k], bh[k][0], bh[k][1]);
-            }
-            // C fragment: rows n = g, g + 8; columns a = a0 + 2t, + 1
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int n = g8 + 8 * (c >> 1), col = 2 * t4 + (c & 1);
-                if (col < NT_CNT[nt] && n < NPHIP) outs[n * NA + NT_A0[nt] + col] = c_mu[NT_A0[nt] + col] * acc[c];
-            }
+        for (int c = 0; c < 4; ++c) {
+            const int n = g8 + 8 * (c & 1), m = 8 * k + t4 + 4 * (c >> 1);       // a0 (g, t), a1 (g+8, t), a2 (g, t+4), a3 (g+8, t+4)
+            const int lo = min(n, m), hi = max(n, m);
+            const bool ok = n < nphi && m < nphi;
+            gi[k][c] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
+            gf[k][c] = ok ? (n == m ? 2.0f : 1.0f) : 0.0f;
         }
-    } else {
+    int64_t g = blockIdx.x;
+    int buf = 0;
+    if (g < n_groups) issue(g, 0);
+    edge::cp_async_commit();
+    for (; g < n_groups; g += gridDim.x, buf ^= 1) {
+        if (g + gridDim.x < n_groups) issue(g + gridDim.x, buf ^ 1);
+        edge::cp_async_commit();
+        edge::cp_async_wait<1>();
+        __syncthreads();                       // the Qbar rows were brought in by all threads of the block
+        const RowId row = row_of_group(tiles, N, g, warp);
         if (row.p >= 0) {
-            atom = sp_list[row.p];
-            const float4 *bi = reinterpret_cast<const float4 *>(b + atom * NB);
+            const int64_t atom = sp_list[row.p];
+            const float *qs = sm + (size_t)buf * GW * RS + warp * RS, *bs = qs + QS;
+            if constexpr (NA == 20) {
+                // bbar_l = mu . (G_l B_l) per l on the tensor cores: M = n (16), K = n' (two steps of 8), N = the monomials of
+                // degree l in tiles of 8 (l = 0: 1 of 8 columns used, l = 1: 3, l = 2: 6, l = 3: 8 + 2). A fragments = G_l
+                // gathered from the triangular Qbar row, B fragments = b (row-major, as it arrived), 3xTF32.
+                float *outs = work;
+                constexpr int NTL = 5;
+                constexpr int NT_A0[NTL] = {0, 1, 4, 10, 18}, NT_CNT[NTL] = {1, 3, 6, 8, 2}, NT_L[NTL] = {0, 1, 2, 3, 3};
+                uint32_t ah[2][4], al[2][4];
 #pragma unroll
-            for (int f = lane; f < NB / 4; f += 32) {
-                const float4 v = __ldg(bi + f);
-                const float va[4] = {v.x, v.y, v.z, v.w};
+                for (int nt = 0; nt < NTL; ++nt) {
+                    if (nt == 0 || NT_L[nt] != NT_L[nt - 1]) {
+                        const float *ql = qs + NT_L[nt] * NPp;
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int e = f * 4 + u;
-                    bT[(e % NA) * C::TS + e / NA] = va[u];
+                        for (int k = 0; k < 2; ++k)
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) edge::split_bits(ql[gi[k][c]] * gf[k][c], ah[k][c], al[k][c]);
+                    }
+                    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+                    const int a = NT_A0[nt] + g8;
+                    const bool va = g8 < NT_CNT[nt];
+                    uint32_t bh[2][2], bl[2][2];
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        const int r0 = 8 * k + t4, r1 = r0 + 4;
+                        edge::split_bits((va && r0 < NPHIP) ? bs[r0 * NA + a] : 0.f, bh[k][0], bl[k][0]);
+                        edge::split_bits((va && r1 < NPHIP) ? bs[r1 * NA + a] : 0.f, bh[k][1], bl[k][1]);
+                    }
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        if (k == 1 && NPHIP <= 8) continue;
+                        edge::mma_tf32(acc, al[k], bh[k][0], bh[k][1]);
+                        edge::mma_tf32(acc, ah[k], bl[k][0], bl[k][1]);
+                    }
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        if (k == 1 && NPHIP <= 8) continue;
+                        edge::mma_tf32(acc, ah[k], bh[k][0], bh[k][1]);
+                    }
+                    // C fragment: rows n = g, g + 8; columns a = a0 + 2t, + 1
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const int n = g8 + 8 * (c >> 1), col = 2 * t4 + (c & 1);
+                        if (col < NT_CNT[nt] && n < NPHIP) outs[n * NA + NT_A0[nt] + col] = c_mu[NT_A0[nt] + col] * acc[c];
+                    }
+                }
+            } else {
+                float *bT = work, *outs = work + NA * C::TS;
+                for (int e = lane; e < NB; e += 32) bT[(e % NA) * C::TS + e / NA] = bs[e];
+                __syncwarp();
+                const int n = lane / C::PARTS, a0 = (lane % C::PARTS) * C::CNT;
+                if (n < NPHIP) {
+                    // triangular offsets of G[n, k] and the (1 + delta) factor; 0 for padded rows / columns
+                    int idx[NPHIP];
+                    float fac[NPHIP];
+#pragma unroll
+                    for (int k = 0; k < NPHIP; ++k) {
+                        const int lo = min(n, k), hi = max(n, k);
+                        const bool ok = n < nphi && k < nphi;
+                        idx[k] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
+                        fac[k] = ok ? (k == n ? 2.0f : 1.0f) : 0.0f;
+                    }
+                    float G[NPHIP];
+                    int lcur = -1;
+#pragma unroll
+                    for (int ai = 0; ai < C::CNT; ++ai) {
+                        const int a = a0 + ai;
+                        if (a < NA) {
+                            const int l = l_of(a);
+                            if (l != lcur) {
+                                const float *ql = qs + l * NPp;
+#pragma unroll
+                                for (int k = 0; k < NPHIP; ++k) G[k] = ql[idx[k]] * fac[k];
+                                lcur = l;
+                            }
+                            float s = 0.f;
+#pragma unroll
+                            for (int k4 = 0; k4 < NPHIP / 4; ++k4) {
+                                const float4 v = *reinterpret_cast<const float4 *>(bT + a * C::TS + 4 * k4);
+                                s = fmaf(G[4 * k4], v.x, s); s = fmaf(G[4 * k4 + 1], v.y, s);
+                                s = fmaf(G[4 * k4 + 2], v.z, s); s = fmaf(G[4 * k4 + 3], v.w, s);
+                            }
+                            outs[n * NA + a] = c_mu[a] * s;
+                        }
+                    }
                 }
             }
+            __syncwarp();
+            float4 *bo = reinterpret_cast<float4 *>(bbar + atom * NB);
+            const float *outs = NA == 20 ? work : work + NA * C::TS;
+#pragma unroll
+            for (int f = lane; f < NB / 4; f += 32) bo[f] = reinterpret_cast<const float4 *>(outs)[f];
         }
-        __syncthreads();
-        if (row.p < 0) return;
-        const int n = lane / C::PARTS, a0 = (lane % C::PARTS) * C::CNT;
-        if (n < NPHIP) {
-            // triangular offsets of G[n, k] and the (1 + delta) factor; 0 for padded rows / columns
-            int idx[NPHIP];
-            float fac[NPHIP];
-#pragma unroll
-            for (int k = 0; k < NPHIP; ++k) {
-                const int lo = min(n, k), hi = max(n, k);
-                const bool ok = n < nphi && k < nphi;
-                idx[k] = ok ? lo * nphi - (lo * (lo - 1)) / 2 + (hi - lo) : 0;
-                fac[k] = ok ? (k == n ? 2.0f : 1.0f) : 0.0f;
-            }
-            float G[NPHIP];
-            int lcur = -1;
-#pragma unroll
-            for (int ai = 0; ai < C::CNT; ++ai) {
-                const int a = a0 + ai;
-                if (a < NA) {
-                    const int l = l_of(a);
-                    if (l != lcur) {
-                        const float *ql = qs + l * NPp;
-#pragma unroll
-                        for (int k = 0; k < NPHIP; ++k) G[k] = ql[idx[k]] * fac[k];
-                        lcur = l;
-                    }
-                    float s = 0.f;
-#pragma unroll
-                    for (int k4 = 0; k4 < NPHIP / 4; ++k4) {
-                        const float4 v = *reinterpret_cast<const float4 *>(bT + a * C::TS + 4 * k4);
-                        s = fmaf(G[4 * k4], v.x, s); s = fmaf(G[4 * k4 + 1], v.y, s);
-                        s = fmaf(G[4 * k4 + 2], v.z, s); s = fmaf(G[4 * k4 + 3], v.w, s);
-                    }
-                    outs[n * NA + a] = c_mu[a] * s;
-                }
-            }
-        }
+        __syncthreads();                       // every warp is done with this buffer before the next prefetch refills it
     }
-    __syncwarp();
-    float4 *bo = reinterpret_cast<float4 *>(bbar + atom * NB);
-#pragma unroll
-    for (int f = lane; f < NB / 4; f += 32) bo[f] = reinterpret_cast<const float4 *>(outs)[f];
+    edge::cp_async_wait<0>();
 }
 
 template <class K>
@@ -373,6 +396,14 @@ int set_smem(K kernel, size_t smem, size_t &attr) {
         attr = smem;
     }
     return REANN_OK;
+}
+
+static int gram_grid(int64_t n_groups, size_t smem) {
+    int dev = 0, n_sm = 148;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) n_sm = 148;
+    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (size_t)(220 * 1024) / smem));
+    return (int)std::min<int64_t>(n_groups, (int64_t)per_sm * n_sm);
 }
 
 template <int NPHIP, int NA>
@@ -391,11 +422,13 @@ int run_gram_bwd(const LaunchCtx &ctx, const ModelDims &md, int64_t N, const int
                  int n_tiles, const float *b, const float *Qbar, float *bbar) {
     using C = BwdCfg<NPHIP, NA>;
     const int KQ = tiles ? md.K1 : md.nqp;
-    const size_t smem = sizeof(float) * GW * (size_t)(C::PER_WARP + KQ + 4);
+    constexpr int NB = NPHIP * NA, WORK = NA == 20 ? NB : C::PER_WARP;
+    const size_t smem = sizeof(float) * GW * (size_t)(2 * (KQ + 4 + NB) + WORK);
     static size_t attr = 48 * 1024;
     if (int rc = set_smem(k_gram_bwd<NPHIP, NA>, smem, attr)) return rc;
-    const unsigned grid = tiles ? (unsigned)n_tiles * 16u : div_up(N, GW);
-    LAUNCH(ctx, (k_gram_bwd<NPHIP, NA>), grid, GW * 32, smem, N, sp_list, tiles, b, Qbar, bbar, md.nphi, md.NPp, KQ, ctx.skip);
+    const int64_t n_groups = tiles ? (int64_t)n_tiles * 16 : (N + GW - 1) / GW;
+    LAUNCH(ctx, (k_gram_bwd<NPHIP, NA>), (unsigned)gram_grid(n_groups, smem), GW * 32, smem, N, sp_list, tiles, b, Qbar, bbar, md.nphi, md.NPp,
+           KQ, n_groups, ctx.skip);
     return REANN_OK;
 }
 
