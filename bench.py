@@ -306,19 +306,19 @@ def main():
     F_h = torch.empty((n, 3), dtype=torch.float64).pin_memory()
     E_h = torch.empty(1, dtype=torch.float64).pin_memory()
     V_h = torch.empty(9, dtype=torch.float64).pin_memory()
-    pos_h.copy_(pos.cpu()); vel_h = vel.cpu().numpy().copy(); inv_m_h = (1.0 / cfg["masses"])[:, None]
+    pos_h.copy_(pos.cpu()); vel_t = vel.cpu().clone()
+    half_kick = (0.5 * dt_fs * acc / torch.tensor(cfg["masses"]))[:, None]      # [n, 1]
     pos_np, F_np, E_np, V_np = pos_h.numpy(), F_h.numpy(), E_h.numpy(), V_h.numpy()
     m.energy_forces(pos_np, box, E_np, F_np, V_np)
+    m.energy_forces(pos_np, box, E_np, F_np, V_np)            # second call: the graph over the staging buffers exists
     Ke = max(3, min(K, 10))
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    half_kick = 0.5 * dt_fs * acc * inv_m_h                   # [n, 1]; host-side integrator without temporaries
-    tmp = np.empty_like(vel_h)
-    for _ in range(Ke):
-        np.multiply(F_np, half_kick, out=tmp); vel_h += tmp   # host-side integrator (caller's job in e2e use)
-        np.multiply(vel_h, dt_fs, out=tmp); pos_np += tmp
+    for _ in range(Ke):                                       # host-side velocity Verlet (the caller's job in e2e use; torch CPU ops, all host cores)
+        vel_t.addcmul_(F_h, half_kick)
+        pos_h.add_(vel_t, alpha=dt_fs)
         m.energy_forces(pos_np, box, E_np, F_np, V_np)        # H2D pos, kernels, D2H E/F/virial, stream sync
-        np.multiply(F_np, half_kick, out=tmp); vel_h += tmp
+        vel_t.addcmul_(F_h, half_kick)
     t_e2e = time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e)
     e2e = {"value": world * n * Ke / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(n * 24),

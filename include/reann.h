@@ -23,9 +23,10 @@
  *    compact-edge buffers are checked on the device; the kernels after the check return at once
  *    when either fails) and synchronises the stream ONCE, at the end, to read that flag word: a
  *    rebuild or a buffer growth is followed by a second pass inside the same call. When the
- *    call returns, the outputs are complete (device or host pointers alike). With device
- *    pointers the steady-state launch sequence is a CUDA graph, re-captured after every rebuild
- *    (REANN_GRAPH=0 switches it off). The handle never works on the legacy default stream (a
+ *    call returns, the outputs are complete (device or host pointers alike). The steady-state
+ *    launch sequence is a CUDA graph, re-captured after every rebuild and whenever the device
+ *    addresses it works on change (the caller's device pointers, or the handle's staging buffers
+ *    when host pointers are passed; REANN_GRAPH=0 switches it off). The handle never works on the legacy default stream (a
  *    graph cannot be captured there): until reann_set_stream gives it a stream, or when that
  *    stream is 0, it uses a blocking stream of its own, which is ordered after earlier work of
  *    the default stream. Systems whose per-edge stash is held in chunks synchronise once more.

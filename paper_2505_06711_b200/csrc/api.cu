@@ -724,9 +724,11 @@ extern "C" int reann_energy_forces(reann_t *h, const double *pos, const double *
         int32_t flag = 0;
         int64_t n_rc = 0;
         if (!chunked) {
-            // ---------------- fast path: a CUDA graph of the steady-state launch sequence when every pointer is a
-            // device pointer (replayed while the list, the buffers and the caller's pointers stay the same) ----------------
-            const bool graphable = h->use_graph && !h->profiling && !o.E_host && !o.F_host && !o.V_host && pos == d_pos;
+            // ---------------- fast path: a CUDA graph of the steady-state launch sequence (replayed while the list, the
+            // buffers and the device addresses the kernels work on stay the same) ----------------
+            // host pointers too: the kernels then work on the handle's staging buffers (fixed device addresses), the copies
+            // to and from the caller's memory are enqueued around the graph launch
+            const bool graphable = h->use_graph && !h->profiling;
             const reann::GraphKey key{d_pos, o.dE, o.dF, o.dV, h->n_rebuilds, h->cap_rc, h->stream};
             if (graphable && h->gexec && memcmp(&key, &h->gkey, sizeof(key)) == 0) {
                 CU(h, cudaGraphLaunch(h->gexec, h->stream));
