@@ -357,7 +357,7 @@ extern "C" void reann_destroy(reann_t *h) {
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
                       &h->geom, &h->rev_rc, &h->c_ext, &h->b, &h->z_stash, &h->bbar, &h->cbar, &h->kappa, &h->gst,
                       &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch, &h->Qbuf,
-                      &h->halo_caller, &h->xch_idx, &h->xch_val, &h->md_state, &h->md_partial, &h->md_E};
+                      &h->halo_caller, &h->xch_idx, &h->xch_val, &h->md_state, &h->md_partial, &h->md_E, &h->nbr_mask};
     for (DevBuf *b : bufs) dev_free(h, *b);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);

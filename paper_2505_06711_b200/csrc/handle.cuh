@@ -53,6 +53,7 @@ struct reann {
     DevBuf rev;                   // uint32 [E_list] index of the reverse entry
     DevBuf sp_list;               // int32 [N] internal indices grouped by species
     DevBuf scratch_a, scratch_b, scratch_c, scan_ws;
+    DevBuf nbr_mask;              // uint32 [N][27 MB]: ballot words of the count pass of the list build
 
     // ---- per-evaluation buffers ----
     DevBuf pos_stage;             // double [N][3] when the caller passes host positions

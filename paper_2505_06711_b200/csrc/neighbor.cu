@@ -61,6 +61,14 @@ __global__ void k_wrap_cell(const double *__restrict__ pos, int64_t N, BoxP B, i
     atomicAdd(&cell_count[key], 1);
 }
 
+__global__ void k_max_i32(const int32_t *__restrict__ v, int64_t n, int32_t *__restrict__ out) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int m = i < n ? v[i] : 0;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+
 __global__ void k_scatter(const int32_t *__restrict__ cellkey, int64_t N, const int64_t *__restrict__ cell_start,
                           int32_t *__restrict__ cell_fill, int32_t *__restrict__ perm) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -70,16 +78,31 @@ __global__ void k_scatter(const int32_t *__restrict__ cellkey, int64_t N, const 
     perm[cell_start[key] + slot] = (int32_t)i;
 }
 
-// one thread per cell: insertion sort by caller index -> deterministic internal order
+// one warp per cell: rank sort by caller index (a cell holds a few dozen atoms) -> deterministic internal order
 __global__ void k_sort_cells(int32_t *__restrict__ perm, const int64_t *__restrict__ cell_start, int64_t ncell) {
-    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const int64_t c = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (c >= ncell) return;
-    int64_t a = cell_start[c], b = cell_start[c + 1];
-    for (int64_t p = a + 1; p < b; ++p) {
-        int32_t v = perm[p];
-        int64_t q = p - 1;
-        while (q >= a && perm[q] > v) { perm[q + 1] = perm[q]; --q; }
-        perm[q + 1] = v;
+    const int64_t a = cell_start[c], b = cell_start[c + 1];
+    const int n = (int)(b - a);
+    if (n <= 1) return;
+    if (n <= 64) {
+        const int v0 = lane < n ? perm[a + lane] : 0x7fffffff, v1 = lane + 32 < n ? perm[a + 32 + lane] : 0x7fffffff;
+        int r0 = 0, r1 = 0;
+        for (int q = 0; q < n; ++q) {
+            const int w = __shfl_sync(0xffffffffu, q < 32 ? v0 : v1, q & 31);
+            r0 += w < v0; r1 += w < v1;
+        }
+        __syncwarp();
+        if (lane < n) perm[a + r0] = v0;
+        if (lane + 32 < n) perm[a + r1] = v1;
+    } else if (lane == 0) {                      // very dense cell: insertion sort by one lane
+        for (int64_t p = a + 1; p < b; ++p) {
+            int32_t v = perm[p];
+            int64_t q = p - 1;
+            while (q >= a && perm[q] > v) { perm[q + 1] = perm[q]; --q; }
+            perm[q + 1] = v;
+        }
     }
 }
 
@@ -167,7 +190,7 @@ __device__ __forceinline__ bool pair_in(const XRec &a, const XRec &b, double shx
 }
 
 // Warp per atom over the 27-cell stencil. FILL = false: count; FILL = true: collect ext indices in
-// shared memory, rank-sort ascending, write the CSR row.
+// shared memory (in ascending order where the stencil cells are distinct, else rank-sorted), write the CSR row.
 template <bool FILL>
 __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ xrec, int64_t N, Grid g,
                                                        const int32_t *__restrict__ cell_rank,
@@ -176,7 +199,9 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
                                                        int32_t *__restrict__ row_cnt,
                                                        unsigned long long *__restrict__ n_rc_total,
                                                        const int64_t *__restrict__ row_ptr, int32_t *__restrict__ col,
-                                                       int32_t *__restrict__ err_flag) {
+                                                       int32_t *__restrict__ err_flag, uint32_t *__restrict__ mask, int MB) {
+    // mask != nullptr: the count pass leaves the ballot word of every batch of 32 candidates (27 cells x MB batches per
+    // atom), and the fill pass reads them back instead of gathering the records and testing the distances again
     __shared__ int32_t rowbuf[FILL ? NB_WARPS * ROWCAP : 1];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t i = (int64_t)blockIdx.x * NB_WARPS + warp;
@@ -186,7 +211,29 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
     cell_of(g.B, me.x, me.y, me.z, g.ncx, g.ncy, g.ncz, &cx, &cy, &cz);
     int cnt = 0, cnt_rc = 0;
     int32_t *buf = rowbuf + (FILL ? warp * ROWCAP : 0);
-    for (int o = 0; o < 27; ++o) {
+    // Fill pass with at least three cells per direction: the 27 stencil cells are distinct, so visiting first the
+    // unshifted ones and then the shifted ones, each kind by ascending Morton rank, yields the row already sorted by
+    // ext index (internal indices are cell-rank-major, image indices owner-major and all above N) -- no sort needed.
+    const bool presorted = FILL && g.ncx >= 3 && g.ncy >= 3 && g.ncz >= 3;
+    __shared__ int8_t order_s[FILL ? NB_WARPS : 1][32];
+    if (FILL && presorted) {
+        int key = 0x7fffffff;
+        if (lane < 27) {
+            const int ox = lane / 9 - 1, oy = (lane / 3) % 3 - 1, oz = lane % 3 - 1;
+            int ax = cx + ox, ay = cy + oy, az = cz + oz;
+            bool sh = false;
+            if (ax < 0) { ax += g.ncx; sh = true; } else if (ax >= g.ncx) { ax -= g.ncx; sh = true; }
+            if (ay < 0) { ay += g.ncy; sh = true; } else if (ay >= g.ncy) { ay -= g.ncy; sh = true; }
+            if (az < 0) { az += g.ncz; sh = true; } else if (az >= g.ncz) { az -= g.ncz; sh = true; }
+            key = cell_rank[(ax * g.ncy + ay) * g.ncz + az] | (sh ? 0x40000000 : 0);      // ncell <= 2^30
+        }
+        int r = 0;
+        for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, key, q) < key;
+        if (lane < 27) order_s[warp][r] = (int8_t)lane;
+        __syncwarp();
+    }
+    for (int oi = 0; oi < 27; ++oi) {
+        const int o = (FILL && presorted) ? order_s[warp][oi] : oi;
         int ox = o / 9 - 1, oy = (o / 3) % 3 - 1, oz = o % 3 - 1;
         int ax = cx + ox, ay = cy + oy, az = cz + oz, sx = 0, sy = 0, sz = 0;
         if (ax < 0) { ax += g.ncx; sx = -1; } else if (ax >= g.ncx) { ax -= g.ncx; sx = 1; }
@@ -197,15 +244,23 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
         double shx, shy, shz;
         box_shift(g.B, (double)sx, (double)sy, (double)sz, shx, shy, shz);
         const int code = shift_code(sx, sy, sz);
-        for (int64_t jb = c0; jb < c1; jb += 32) {
+        int bi = 0;
+        for (int64_t jb = c0; jb < c1; jb += 32, ++bi) {
             const int64_t j = jb + lane;
             bool in = false, in_rc = false;
-            if (j < c1 && !(j == i && code == 13)) {
-                double d2;
-                in = pair_in(me, xrec[j], shx, shy, shz, g.R2, &d2);
-                in_rc = d2 < g.rc2;
+            unsigned m;
+            if (FILL && mask) {
+                m = mask[(size_t)i * (27 * MB) + o * MB + bi];
+                in = (m >> lane) & 1u;
+            } else {
+                if (j < c1 && !(j == i && code == 13)) {
+                    double d2;
+                    in = pair_in(me, xrec[j], shx, shy, shz, g.R2, &d2);
+                    in_rc = d2 < g.rc2;
+                }
+                m = __ballot_sync(0xffffffffu, in);
+                if (!FILL && mask && lane == 0) mask[(size_t)i * (27 * MB) + o * MB + bi] = m;
             }
-            const unsigned m = __ballot_sync(0xffffffffu, in);
             if (FILL) {
                 if (in) {
                     int slot = cnt + __popc(m & ((1u << lane) - 1));
@@ -230,7 +285,11 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
     __syncwarp();
     if (cnt > ROWCAP) return; // flagged in the count pass
     const int64_t base = row_ptr[i];
-    for (int e = lane; e < cnt; e += 32) {
+    if (presorted) {
+        for (int e = lane; e < cnt; e += 32) col[base + e] = buf[e];
+        return;
+    }
+    for (int e = lane; e < cnt; e += 32) {       // small boxes (a cell met with several shifts): rank sort
         const int32_t v = buf[e];
         int rank = 0;
         for (int q = 0; q < cnt; ++q) rank += (buf[q] < v);
@@ -372,10 +431,11 @@ int neighbor_build(reann *h, const double *d_pos) {
     // A1: wrap, cell key, counting sort in Morton cell order, deterministic inside each cell
     LAUNCH(ctx, k_wrap_cell, div_up(N, TPB), TPB, 0, d_pos, N, B, g.ncx, g.ncy, g.ncz,
            (const int32_t *)h->cell_rank.p, (int32_t *)h->wshift.p, cellkey, cell_count);
+    LAUNCH(ctx, k_max_i32, div_up(ncell, TPB), TPB, 0, (const int32_t *)cell_count, ncell, flags + 6);
     exclusive_scan_i32_to_i64(ctx, cell_count, (int64_t *)h->cell_start.p, ncell, h->scan_ws.p);
     LAUNCH(ctx, k_scatter, div_up(N, TPB), TPB, 0, cellkey, N, (const int64_t *)h->cell_start.p, cell_fill,
            (int32_t *)h->perm.p);
-    LAUNCH(ctx, k_sort_cells, div_up(ncell, 64), 64, 0, (int32_t *)h->perm.p, (const int64_t *)h->cell_start.p, ncell);
+    LAUNCH(ctx, k_sort_cells, div_up(ncell, 4), 128, 0, (int32_t *)h->perm.p, (const int64_t *)h->cell_start.p, ncell);
     LAUNCH(ctx, k_local_records, div_up(N, TPB), TPB, 0, (const int32_t *)h->perm.p, d_pos,
            (const int32_t *)h->wshift.p, (const int32_t *)h->species_caller.p, N, B, (XRec *)h->xrec.p,
            (int32_t *)h->inv_perm.p, (double *)h->pos_build.p);
@@ -408,11 +468,22 @@ int neighbor_build(reann *h, const double *d_pos) {
            (int32_t *)h->img_index.p);
 
     // A3: count -> scan -> fill (+ row sort) -> reverse index
+    // ballot words of the count pass for the fill pass: 27 x MB words per atom (MB = batches of 32 that cover the fullest
+    // cell); skipped (the fill pass then repeats the pair tests) when they would take more than 4 GB
+    int max_cell = 0;
+    CU(h, cudaMemcpyAsync(&max_cell, flags + 6, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
+    CU(h, cudaStreamSynchronize(h->stream));
+    const int MB = std::max(1, (max_cell + 31) / 32);
+    uint32_t *mask = nullptr;
+    if ((size_t)N * 27 * MB * sizeof(uint32_t) <= ((size_t)4 << 30)) {
+        RC(dev_ensure(h, h->nbr_mask, (size_t)N * 27 * MB * sizeof(uint32_t)));
+        mask = (uint32_t *)h->nbr_mask.p;
+    }
     int32_t *row_cnt = (int32_t *)h->scratch_a.p;
     unsigned long long *n_rc_total = (unsigned long long *)(flags + 4);
     LAUNCH(ctx, k_nbr<false>, div_up(N, NB_WARPS), NB_WARPS * 32, 0, (const XRec *)h->xrec.p, N, g,
            (const int32_t *)h->cell_rank.p, (const int64_t *)h->cell_start.p, (const int32_t *)h->img_index.p, row_cnt,
-           n_rc_total, (const int64_t *)nullptr, (int32_t *)nullptr, flags);
+           n_rc_total, (const int64_t *)nullptr, (int32_t *)nullptr, flags, mask, MB);
     exclusive_scan_i32_to_i64(ctx, row_cnt, (int64_t *)h->row_ptr.p, N, h->scan_ws.p);
     int64_t E = 0;
     CU(h, cudaMemcpyAsync(&E, (int64_t *)h->row_ptr.p + N, sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
@@ -430,7 +501,7 @@ int neighbor_build(reann *h, const double *d_pos) {
     LAUNCH(ctx, k_nbr<true>, div_up(N, NB_WARPS), NB_WARPS * 32, 0, (const XRec *)h->xrec.p, N, g,
            (const int32_t *)h->cell_rank.p, (const int64_t *)h->cell_start.p, (const int32_t *)h->img_index.p,
            (int32_t *)nullptr, (unsigned long long *)nullptr, (const int64_t *)h->row_ptr.p, (int32_t *)h->col.p,
-           flags);
+           flags, mask, MB);
     LAUNCH(ctx, k_rev, div_up(N, 4), 128, 0, (const XRec *)h->xrec.p, N, (const int64_t *)h->row_ptr.p,
            (const int32_t *)h->col.p, (const int32_t *)h->img_index.p, (uint32_t *)h->rev.p, flags);
 
