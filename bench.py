@@ -307,18 +307,18 @@ def main():
     E_h = torch.empty(1, dtype=torch.float64).pin_memory()
     V_h = torch.empty(9, dtype=torch.float64).pin_memory()
     pos_h.copy_(pos.cpu()); vel_t = vel.cpu().clone()
-    half_kick = (0.5 * dt_fs * acc / torch.tensor(cfg["masses"]))[:, None]      # [n, 1]
+    kick = (dt_fs * acc / torch.tensor(cfg["masses"]))[:, None].expand(n, 3).contiguous()   # [n, 3], full step
     pos_np, F_np, E_np, V_np = pos_h.numpy(), F_h.numpy(), E_h.numpy(), V_h.numpy()
     m.energy_forces(pos_np, box, E_np, F_np, V_np)
     m.energy_forces(pos_np, box, E_np, F_np, V_np)            # second call: the graph over the staging buffers exists
-    Ke = max(3, min(K, 10))
+    vel_t.addcmul_(F_h, kick, value=0.5)                      # v(t + dt/2): leapfrog form of velocity Verlet from here on
+    Ke = max(3, min(K, 25))
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    for _ in range(Ke):                                       # host-side velocity Verlet (the caller's job in e2e use; torch CPU ops, all host cores)
-        vel_t.addcmul_(F_h, half_kick)
-        pos_h.add_(vel_t, alpha=dt_fs)
+    for _ in range(Ke):                                       # host-side integrator (the caller's job in e2e use; torch CPU ops, all host cores)
+        pos_h.add_(vel_t, alpha=dt_fs)                        # x(t + dt)
         m.energy_forces(pos_np, box, E_np, F_np, V_np)        # H2D pos, kernels, D2H E/F/virial, stream sync
-        vel_t.addcmul_(F_h, half_kick)
+        vel_t.addcmul_(F_h, kick)                             # v(t + 3dt/2): the two half kicks on the same forces in one pass
     t_e2e = time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e)
     e2e = {"value": world * n * Ke / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(n * 24),

@@ -357,7 +357,7 @@ extern "C" void reann_destroy(reann_t *h) {
                       &h->scratch_c, &h->scan_ws, &h->pos_stage, &h->rank16, &h->rc_cnt, &h->rc_ptr, &h->col_rc,
                       &h->geom, &h->rev_rc, &h->c_ext, &h->b, &h->z_stash, &h->bbar, &h->cbar, &h->kappa, &h->gst,
                       &h->Ei, &h->Fc, &h->vir_part, &h->out_stage, &h->Ei_caller, &h->flags, &h->red_scratch, &h->Qbuf,
-                      &h->halo_caller, &h->xch_idx, &h->xch_val, &h->md_state, &h->md_partial, &h->md_E, &h->nbr_mask};
+                      &h->halo_caller, &h->xch_idx, &h->xch_val, &h->md_state, &h->md_partial, &h->md_E, &h->nbr_mask, &h->rcx};
     for (DevBuf *b : bufs) dev_free(h, *b);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
@@ -425,6 +425,7 @@ static int do_build(reann *h, const double *d_pos, const double *box9) {
         RC(dev_ensure(h, h->rank16, sizeof(uint16_t) * ((size_t)std::max<int64_t>(h->E_list, 1) + (size_t)h->E_list / 32 + 1024)));
     RC(dev_ensure(h, h->rc_cnt, sizeof(int32_t) * (size_t)(N + 1)));
     RC(dev_ensure(h, h->rc_ptr, sizeof(int64_t) * (size_t)(N + 1)));
+    RC(dev_ensure(h, h->rcx, sizeof(uint32_t) * (size_t)std::max<int64_t>(h->n_ext, 1)));
     RC(dev_ensure(h, h->scan_ws, scan_workspace_bytes(N + 1)));
     {
         const size_t need = sizeof(float) * (size_t)md.T * (size_t)std::max<int64_t>(h->n_ext, 1) * md.nphip;
@@ -570,8 +571,8 @@ static LayerPtrs layer_ptrs(reann *h) {
 static void enqueue_filter_fill(reann *h, const LaunchCtx &ctx) {
     const BoxP B = make_boxp(h->box_build);
     launch_filter_fill(ctx, (const XRec *)h->xrec.p, (const int64_t *)h->row_ptr.p, (const int32_t *)h->col.p,
-                       (const uint32_t *)h->rev.p, h->N, B, (const uint16_t *)h->rank16.p,
-                       (const int64_t *)h->rc_ptr.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
+                       (const uint32_t *)h->rev.p, h->N, h->n_ext, B, (const uint16_t *)h->rank16.p,
+                       (const int64_t *)h->rc_ptr.p, (uint32_t *)h->rcx.p, (uint32_t *)h->col_rc.p, (float4 *)h->geom.p, (uint32_t *)h->rev_rc.p);
 }
 
 // layer t of the forward pass (Eq. 1, Eq. 2): b^t, rho^t (radial-pair form), c^{t+1} of the local atoms or E_i

@@ -145,8 +145,8 @@ void launch_refresh(const LaunchCtx &ctx, XRec *xrec, int64_t n_ext, const int32
 void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
                          int64_t N, const BoxP &box, double rc2, uint16_t *rank16, int32_t *rc_cnt);
 void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
-                        const uint32_t *rev, int64_t N, const BoxP &box, const uint16_t *rank16,
-                        const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc);
+                        const uint32_t *rev, int64_t N, int64_t n_ext, const BoxP &box, const uint16_t *rank16,
+                        const int64_t *rc_ptr, uint32_t *rcx, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc);
 void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip);
 int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,

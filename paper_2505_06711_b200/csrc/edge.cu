@@ -97,14 +97,26 @@ __global__ void __launch_bounds__(RW * 32) k_filter_count(const XRec *__restrict
     if (lane == 0) rc_cnt[i] = cnt;
 }
 
+// offset of the compact row of the owner of every ext atom (ghosts: their owner's row), so that the fill pass below
+// finds the row of a reverse edge with one 4-byte gather that does not wait for the neighbour's record
+__global__ void k_rc_ext(const XRec *__restrict__ xrec, const int64_t *__restrict__ rc_ptr, int64_t N, int64_t n_ext,
+                         uint32_t *__restrict__ rcx, const int32_t *__restrict__ skip) {
+    SKIP_GUARD(skip);
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_ext) return;
+    rcx[k] = (uint32_t)rc_ptr[k < N ? k : (int64_t)xrec[k].owner];
+}
+
 // rc-filter, pass 2: compact rows (neighbour ext index | species<<28, edge vector + length in FP32
-// rounded once from the FP64 difference, index of the reverse compact edge)
+// rounded once from the FP64 difference, index of the reverse compact edge). Two levels of dependent loads per
+// iteration: (rank, col, rev) of the entry, then (record, rank of the reverse entry, row offset of the owner).
 __global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict__ xrec,
                                                          const int64_t *__restrict__ row_ptr,
                                                          const int32_t *__restrict__ col,
                                                          const uint32_t *__restrict__ rev, int64_t N, BoxP B,
                                                          const uint16_t *__restrict__ rank16,
                                                          const int64_t *__restrict__ rc_ptr,
+                                                         const uint32_t *__restrict__ rcx,
                                                          uint32_t *__restrict__ col_rc, float4 *__restrict__ geom,
                                                          uint32_t *__restrict__ rev_rc, const int32_t *__restrict__ skip) {
     SKIP_GUARD(skip);
@@ -113,7 +125,7 @@ __global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict_
     if (i >= N) return;
     const XRec me = xrec[i];
     const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1], c0 = rc_ptr[i];
-    // four list entries per lane and iteration: their (dependent) gathers are all in flight together
+    // four list entries per lane and iteration: their gathers are all in flight together
     constexpr int U = 4;
     for (int64_t eb = r0 + lane; eb < r1; eb += 32 * U) {
         uint16_t rk[U];
@@ -122,20 +134,15 @@ __global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict_
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int64_t e = eb + 32 * u;
-            rk[u] = e < r1 ? rank16[e] : (uint16_t)0xFFFF;
+            rk[u] = 0xFFFF; j[u] = 0; rv[u] = 0;
+            if (e < r1) { rk[u] = rank16[e]; j[u] = col[e]; rv[u] = rev[e]; }
         }
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (rk[u] != 0xFFFF) { j[u] = col[eb + 32 * u]; rv[u] = rev[eb + 32 * u]; }
         XRec o[U];
         uint16_t rrk[U];
+        uint32_t base[U];
 #pragma unroll
         for (int u = 0; u < U; ++u)
-            if (rk[u] != 0xFFFF) { o[u] = xrec[j[u]]; rrk[u] = rank16[rv[u]]; }
-        int64_t base[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (rk[u] != 0xFFFF) base[u] = rc_ptr[o[u].owner];
+            if (rk[u] != 0xFFFF) { o[u] = xrec[j[u]]; rrk[u] = rank16[rv[u]]; base[u] = rcx[j[u]]; }
 #pragma unroll
         for (int u = 0; u < U; ++u)
             if (rk[u] != 0xFFFF) {
@@ -144,7 +151,7 @@ __global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict_
                 const int64_t ce = c0 + rk[u];
                 col_rc[ce] = (uint32_t)j[u] | ((uint32_t)o[u].species << COL_SPECIES_SHIFT);
                 geom[ce] = make_float4((float)dx, (float)dy, (float)dz, (float)sqrt(d2));
-                rev_rc[ce] = (uint32_t)(base[u] + rrk[u]);
+                rev_rc[ce] = base[u] + rrk[u];
             }
     }
 }
@@ -847,9 +854,11 @@ void launch_filter_count(const LaunchCtx &ctx, const XRec *xrec, const int64_t *
     if (N > 0) LAUNCH(ctx, k_filter_count, div_up(N, RW), RW * 32, 0, xrec, row_ptr, col, N, box, rc2, rank16, rc_cnt);
 }
 void launch_filter_fill(const LaunchCtx &ctx, const XRec *xrec, const int64_t *row_ptr, const int32_t *col,
-                        const uint32_t *rev, int64_t N, const BoxP &box, const uint16_t *rank16,
-                        const int64_t *rc_ptr, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc) {
-    if (N > 0) LAUNCH(ctx, k_filter_fill, div_up(N, RW), RW * 32, 0, xrec, row_ptr, col, rev, N, box, rank16, rc_ptr, col_rc, geom, rev_rc, ctx.skip);
+                        const uint32_t *rev, int64_t N, int64_t n_ext, const BoxP &box, const uint16_t *rank16,
+                        const int64_t *rc_ptr, uint32_t *rcx, uint32_t *col_rc, float4 *geom, uint32_t *rev_rc) {
+    if (N <= 0) return;
+    LAUNCH(ctx, k_rc_ext, div_up(n_ext, 256), 256, 0, xrec, rc_ptr, N, n_ext, rcx, ctx.skip);
+    LAUNCH(ctx, k_filter_fill, div_up(N, RW), RW * 32, 0, xrec, row_ptr, col, rev, N, box, rank16, rc_ptr, rcx, col_rc, geom, rev_rc, ctx.skip);
 }
 void launch_ghost_gather(const LaunchCtx &ctx, float *c_ext, const XRec *xrec, int64_t N, int64_t n_ext, int nphip) {
     const int64_t work = (n_ext - N) * (nphip / 4);

@@ -60,6 +60,7 @@ struct reann {
     DevBuf rank16;                // uint16 [E_list]
     DevBuf rc_cnt;                // int32 [N]
     DevBuf rc_ptr;                // int64 [N+1]
+    DevBuf rcx;                   // uint32 [n_ext]: rc_ptr of the owner of every ext atom
     DevBuf col_rc, geom, rev_rc;  // uint32 / float4 / uint32 [cap_rc]
     int64_t cap_rc = 0, E_rc = 0;
     int stash_chunks = 1;         // kappa stash held for 1/stash_chunks of the atoms at a time (memory-limited systems)
