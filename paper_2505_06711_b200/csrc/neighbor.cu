@@ -216,46 +216,71 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
     // ext index (internal indices are cell-rank-major, image indices owner-major and all above N) -- no sort needed.
     const bool presorted = FILL && g.ncx >= 3 && g.ncy >= 3 && g.ncz >= 3;
     __shared__ int8_t order_s[FILL ? NB_WARPS : 1][32];
-    if (FILL && presorted) {
-        int key = 0x7fffffff;
-        if (lane < 27) {
-            const int ox = lane / 9 - 1, oy = (lane / 3) % 3 - 1, oz = lane % 3 - 1;
-            int ax = cx + ox, ay = cy + oy, az = cz + oz;
-            bool sh = false;
-            if (ax < 0) { ax += g.ncx; sh = true; } else if (ax >= g.ncx) { ax -= g.ncx; sh = true; }
-            if (ay < 0) { ay += g.ncy; sh = true; } else if (ay >= g.ncy) { ay -= g.ncy; sh = true; }
-            if (az < 0) { az += g.ncz; sh = true; } else if (az >= g.ncz) { az -= g.ncz; sh = true; }
-            key = cell_rank[(ax * g.ncy + ay) * g.ncz + az] | (sh ? 0x40000000 : 0);      // ncell <= 2^30
-        }
-        int r = 0;
-        for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, key, q) < key;
-        if (lane < 27) order_s[warp][r] = (int8_t)lane;
-        __syncwarp();
-    }
-    for (int oi = 0; oi < 27; ++oi) {
-        const int o = (FILL && presorted) ? order_s[warp][oi] : oi;
-        int ox = o / 9 - 1, oy = (o / 3) % 3 - 1, oz = o % 3 - 1;
+    // lane o < 27 looks up stencil cell o once (rank, first atom, atom count, shift code): one chain of two dependent
+    // loads for the whole stencil, and the loop below gets them by shuffle, so its only loads are the candidates' records
+    // (or the count pass's ballot words), fetched one batch ahead
+    int l_c0 = 0, l_n = 0, l_code = 13, l_key = 0x7fffffff;
+    if (lane < 27) {
+        const int ox = lane / 9 - 1, oy = (lane / 3) % 3 - 1, oz = lane % 3 - 1;
         int ax = cx + ox, ay = cy + oy, az = cz + oz, sx = 0, sy = 0, sz = 0;
         if (ax < 0) { ax += g.ncx; sx = -1; } else if (ax >= g.ncx) { ax -= g.ncx; sx = 1; }
         if (ay < 0) { ay += g.ncy; sy = -1; } else if (ay >= g.ncy) { ay -= g.ncy; sy = 1; }
         if (az < 0) { az += g.ncz; sz = -1; } else if (az >= g.ncz) { az -= g.ncz; sz = 1; }
         const int key = cell_rank[(ax * g.ncy + ay) * g.ncz + az];
-        const int64_t c0 = cell_start[key], c1 = cell_start[key + 1];
-        double shx, shy, shz;
-        box_shift(g.B, (double)sx, (double)sy, (double)sz, shx, shy, shz);
-        const int code = shift_code(sx, sy, sz);
-        int bi = 0;
-        for (int64_t jb = c0; jb < c1; jb += 32, ++bi) {
-            const int64_t j = jb + lane;
+        const int64_t c0 = cell_start[key];
+        l_c0 = (int)c0;
+        l_n = (int)(cell_start[key + 1] - c0);
+        l_code = shift_code(sx, sy, sz);
+        l_key = key | (l_code != 13 ? 0x40000000 : 0);      // ncell <= 2^30
+    }
+    int l_o = lane;                                          // stencil cell visited at position `lane`
+    if (FILL && presorted) {
+        int r = 0;
+        for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, l_key, q) < l_key;
+        if (lane < 27) order_s[warp][r] = (int8_t)lane;
+        __syncwarp();
+        l_o = lane < 27 ? order_s[warp][lane] : lane;
+    }
+    // parameters in visiting order: lane p holds those of the p-th visited cell
+    const int v_c0 = __shfl_sync(0xffffffffu, l_c0, l_o), v_n = __shfl_sync(0xffffffffu, l_n, l_o),
+              v_code = __shfl_sync(0xffffffffu, l_code, l_o);
+    const bool use_mask = FILL && mask != nullptr;
+    const uint32_t *mrow = mask ? mask + (size_t)i * (27 * MB) : nullptr;
+    XRec nxt = me;
+    unsigned nxt_m = 0;
+    // state of the cell being visited (warp-uniform)
+    int oi = 0, bi = 0;
+    int c0 = __shfl_sync(0xffffffffu, v_c0, 0), n = __shfl_sync(0xffffffffu, v_n, 0);
+    int code = __shfl_sync(0xffffffffu, v_code, 0), o = __shfl_sync(0xffffffffu, l_o, 0);
+    double shx, shy, shz;
+    box_shift(g.B, (double)(code / 9 - 1), (double)((code / 3) % 3 - 1), (double)(code % 3 - 1), shx, shy, shz);
+    if (use_mask) { if (n > 0) nxt_m = mrow[o * MB]; }
+    else if (lane < n) nxt = xrec[c0 + lane];
+    while (oi < 27) {
+        const int k = 32 * bi + lane;                        // candidate k of the cell
+        const int64_t j = (int64_t)c0 + k;
+        const XRec cur = nxt;
+        unsigned m = nxt_m;
+        // next batch (of this cell, else the first one of the next cell) in flight while this one is tested
+        const bool more = 32 * (bi + 1) < n;
+        int c0n = c0, nn = n, coden = code, on = o;
+        if (more) {
+            if (use_mask) nxt_m = mrow[o * MB + bi + 1];
+            else if (k + 32 < n) nxt = xrec[j + 32];
+        } else if (oi + 1 < 27) {
+            c0n = __shfl_sync(0xffffffffu, v_c0, oi + 1); nn = __shfl_sync(0xffffffffu, v_n, oi + 1);
+            coden = __shfl_sync(0xffffffffu, v_code, oi + 1); on = __shfl_sync(0xffffffffu, l_o, oi + 1);
+            if (use_mask) { if (nn > 0) nxt_m = mrow[on * MB]; }
+            else if (lane < nn) nxt = xrec[c0n + lane];
+        }
+        if (n > 0) {                                         // warp-uniform: the batch holds candidates
             bool in = false, in_rc = false;
-            unsigned m;
-            if (FILL && mask) {
-                m = mask[(size_t)i * (27 * MB) + o * MB + bi];
+            if (use_mask) {
                 in = (m >> lane) & 1u;
             } else {
-                if (j < c1 && !(j == i && code == 13)) {
+                if (k < n && !(j == i && code == 13)) {
                     double d2;
-                    in = pair_in(me, xrec[j], shx, shy, shz, g.R2, &d2);
+                    in = pair_in(me, cur, shx, shy, shz, g.R2, &d2);
                     in_rc = d2 < g.rc2;
                 }
                 m = __ballot_sync(0xffffffffu, in);
@@ -263,8 +288,8 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
             }
             if (FILL) {
                 if (in) {
-                    int slot = cnt + __popc(m & ((1u << lane) - 1));
-                    int32_t e = (code == 13) ? (int32_t)j : img_index[j * 27 + code];
+                    const int slot = cnt + __popc(m & ((1u << lane) - 1));
+                    const int32_t e = (code == 13) ? (int32_t)j : img_index[j * 27 + code];
                     if (e < 0) atomicOr(err_flag, 2);
                     if (slot < ROWCAP) buf[slot] = e;
                 }
@@ -272,6 +297,12 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_nbr(const XRec *__restrict__ 
                 cnt_rc += __popc(__ballot_sync(0xffffffffu, in_rc));
             }
             cnt += __popc(m);
+        }
+        if (more) ++bi;
+        else {
+            ++oi; bi = 0;
+            if (coden != code) box_shift(g.B, (double)(coden / 9 - 1), (double)((coden / 3) % 3 - 1), (double)(coden % 3 - 1), shx, shy, shz);
+            c0 = c0n; n = nn; code = coden; o = on;
         }
     }
     if (!FILL) {
