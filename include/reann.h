@@ -204,6 +204,27 @@ typedef struct {
 int reann_md_run(reann_t *h, double *pos, double *vel, const double *inv_mass, const double *box9, int64_t n_steps,
                  double dt, double acc_unit, double kT, double tau, double *F, double *virial, reann_md_state_t *st);
 
+/*
+ * ---- An entry point that allocates nothing ----
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it): the step of the neighbour build that turns per-atom neighbour counts into the CSR row pointers of the
+ * list ("neighbor list" of PAPER.md:57-59, section 2.2), with no handle and no allocation.
+ *   row_ptr[0] = 0, row_ptr[i + 1] = counts[0] + ... + counts[i]      (exact, 64-bit sums)
+ *   counts  [n_rows]      int32, DEVICE pointer, read only (may be NULL when n_rows == 0);
+ *   row_ptr [n_rows + 1]  int64, DEVICE pointer, written; both stay the caller's;
+ *   cuda_stream           cudaStream_t to enqueue on (NULL = the default stream); the call does not synchronise.
+ * Same kernels as the handle's build; their workspace (block totals and offsets) is a file-scope device array of
+ * fixed size instead of a cudaMalloc'ed buffer: 133 120 bytes that every GPU loading the library holds until the
+ * process exits. Limit: n_rows <= REANN_NOALLOC_MAX_ROWS; larger -> REANN_ERR_UNSUPPORTED, nothing launched.
+ * Calls no cudaMalloc / cudaFree or allocating library routine. All calls on one device share the array: calls that
+ * overlap on the GPU (different streams without ordering between them, or different host threads) RACE -- order
+ * them. The array keeps the previous call's contents; no word of it is read before this call has written it.
+ * Errors: REANN_ERR_ARG (NULL pointer, n_rows < 0), REANN_ERR_UNSUPPORTED (over the limit), REANN_ERR_CUDA;
+ * the text is returned by reann_last_error(NULL) on the calling thread.
+ */
+#define REANN_NOALLOC_MAX_ROWS (1 << 24)
+int reann_row_ptr_noalloc(const int32_t *counts, int64_t n_rows, int64_t *row_ptr, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,8 @@ EXPORTS = ["reann_create", "reann_build_neighbors", "reann_energy_forces", "rean
            "reann_get_neighbors", "reann_get_neighbor_rows", "reann_get_stats", "reann_set_profiling", "reann_set_stream",
            "reann_get_atomic_energies", "reann_verlet", "reann_set_halo", "reann_step_begin", "reann_step_forward",
            "reann_coeff_get", "reann_coeff_set", "reann_step_backward", "reann_cbar_get", "reann_cbar_add", "reann_step_end",
-           "reann_md_run"]
+           "reann_md_run", "reann_row_ptr_noalloc"]
+REANN_NOALLOC_MAX_ROWS = 1 << 24
 
 
 class ReannError(RuntimeError):
@@ -96,6 +97,8 @@ def lib() -> ctypes.CDLL:
         L.reann_verlet.argtypes = [vp, vp, vp, vp, vp, dbl, dbl, ctypes.c_int]
         L.reann_md_run.restype = ctypes.c_int
         L.reann_md_run.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, vp, vp, ctypes.POINTER(MdState)]
+        L.reann_row_ptr_noalloc.restype = ctypes.c_int
+        L.reann_row_ptr_noalloc.argtypes = [vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -174,6 +177,12 @@ def reann_get_neighbors(h, n_atoms: int):
     sh = np.zeros((max(n.value, 1), 3), dtype=np.int8)
     _check(h, lib().reann_get_neighbors(h, ctypes.byref(n), _ptr(row_ptr), _ptr(j), _ptr(sh)))
     return row_ptr, j[:n.value], sh[:n.value]
+
+
+def reann_row_ptr_noalloc(counts, n_rows: int, row_ptr, cuda_stream=None) -> None:
+    """row_ptr[0] = 0, row_ptr[i+1] = counts[0] + ... + counts[i] on the device, allocating nothing (reann.h):
+    counts int32 [n_rows] and row_ptr int64 [n_rows+1] are DEVICE tensors / addresses of the caller."""
+    _check(None, lib().reann_row_ptr_noalloc(_ptr(counts), int(n_rows), _ptr(row_ptr), _ptr(cuda_stream)))
 
 
 def reann_get_neighbor_rows(h, atoms):
