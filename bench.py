@@ -380,7 +380,8 @@ def main():
         nb_bytes = 24.0 * n + 32.0 * n_ext + 8.0 * E_list + 8.0 * n
         roofline["other_kernels"].append({"bound": "hbm", "kernel": "neighbor_build", "achieved": nb_bytes / (t_build * 1e-3) / 1e9,
                                           "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": nb_bytes / (t_build * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                                          "traffic": None, "peak_source": peak_of["hbm"][2], "ms_per_launch": t_build,
+                                          "traffic": traffic.get("neighbor_build"),   # k_nbr<count> + k_nbr<fill> + k_rev of the capture
+                                          "peak_source": peak_of["hbm"][2], "ms_per_launch": t_build,
                                           "launches_per_step": (s1["n_rebuilds"] - s0["n_rebuilds"]) / K,
                                           "algorithmic_per_launch": nb_bytes, "algorithmic_unit": "bytes"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
