@@ -339,15 +339,16 @@ def main():
         # Algorithmic work PER LAUNCH and launches per step of every kernel group (SURVEY.md 8(d) per-unit figures x
         # units): 1 FMA = 2 flop. dense groups = contraction (radial-pair form) + MLP GEMMs;
         # n_out is N_phi for the T-1 coefficient layers and 1 for the last. rev_gather has two launch kinds: layers
-        # t >= 1 read rev (4 B) + g_e (16 B) + kappa_e (4 N_phi B) per edge and write cbar; the t = 0 launch reads
-        # rev + g_e only (c^0 is constant) and writes nothing per atom but the forces.
+        # t >= 1 read rev (4 B) + kappa_e (4 N_phi B) per edge and write cbar (the g_e stash is summed over the layers
+        # by k_edge_bwd and gathered once); the t = 0 launch reads rev + the summed g_e (c^0 is constant,
+        # PAPER.md:76) and writes nothing per atom but the forces.
         nout_avg = ((T - 1) * nphi + 1) / T
         dense_flops = 2.0 * n * (n_q * H1 + H1 * H2 + H2 * nout_avg)
         work = {"ms_edge_fwd": ("alu", 2.0 * E_rc * nphi * Na, T), "ms_edge_bwd": ("alu", 4.0 * E_rc * nphi * Na, T),
                 "ms_dense_fwd": ("tensor", dense_flops, T), "ms_dense_bwd": ("tensor", dense_flops, T),
                 "ms_rev_gather_t0": ("hbm", float(E_rc) * (4 + 16) + n * 24.0, 1)}
         if T > 1:
-            work["ms_rev_gather"] = ("hbm", float(E_rc) * (4 * nphip + 16 + 4) + n * (4.0 * nphip + 8), T - 1)
+            work["ms_rev_gather"] = ("hbm", float(E_rc) * (4 * nphip + 4) + n * (4.0 * nphip + 8), T - 1)
         sm_max = peaks.get("sm_max_mhz", 1965.0)
         alu_peak = N_SM * FP32_FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         # TF32 peak = measured BF16 dense peak x the guide's nominal TF32/BF16 ratio (1.13 / 2.25 PFLOP/s);

@@ -643,14 +643,15 @@ static int enqueue_backward_layer(reann *h, const LaunchCtx &ctx, Marks &mk, int
                                 (const float4 *)h->geom.p, p.c_ext + t * p.cstride, (const float *)h->rcen.p,
                                 (const float *)h->alpha.p, (const float *)h->bbar.p, (float *)h->kappa.p,
                                 (float4 *)h->gst.p, want_vir ? (double *)h->vir_part.p : nullptr, ch_atom[(size_t)c],
-                                ch_atom[(size_t)c + 1], ch_edge[(size_t)c]);
+                                ch_atom[(size_t)c + 1], ch_edge[(size_t)c], !last);
         if (rcode) return set_err(h, rcode, "edge backward: unsupported (n_gauss, L) combination");
         mk.mark(t >= 1 ? 7 : 9);
-        // forces need the complete g_e stash: with the last chunk; cbar: = for the first chunk, += after
+        // the top layer stores g_e, the layers below add theirs to it, so the stash holds the sum over the layers after
+        // layer 0 and the forces are gathered once, there, with its last chunk; cbar: = for the first chunk, += after
         if (t >= 1 || c == C - 1)
             launch_rev_gather(ctx, N, (const int64_t *)h->rc_ptr.p, (const uint32_t *)h->rev_rc.p, (const float *)h->kappa.p,
                               (const float4 *)h->gst.p, md.nphip, t >= 1, (float *)h->cbar.p, (double *)h->Fc.p,
-                              ch_edge[(size_t)c], ch_edge[(size_t)c + 1], c == C - 1, c > 0);
+                              ch_edge[(size_t)c], ch_edge[(size_t)c + 1], t == 0 && c == C - 1, c > 0);
     }
     return REANN_OK;
 }

@@ -154,7 +154,8 @@ int launch_edge_fwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N,
 int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
                     const float *alpha, const float *bbar, float *kappa, float4 *gst, double *vir_part,
-                    int64_t a0, int64_t a1, int64_t e_lo /* atoms [a0, a1), a0 % 4 == 0; kappa holds edges from e_lo on */);
+                    int64_t a0, int64_t a1, int64_t e_lo /* atoms [a0, a1), a0 % 4 == 0; kappa holds edges from e_lo on */,
+                    bool g_add /* gst += g_e (layers below the top one: the stash then holds the sum over the layers) */);
 int edge_bwd_blocks(int64_t N, int Na);
 void launch_rev_gather(const LaunchCtx &ctx, int64_t N, const int64_t *rc_ptr, const uint32_t *rev_rc,
                        const float *kappa, const float4 *gst, int nphip, int want_cbar, float *cbar, double *Fc,

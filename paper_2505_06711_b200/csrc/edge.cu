@@ -573,7 +573,7 @@ __device__ __forceinline__ void edge_bwd_pass(int64_t e0, int64_t end, const uin
         for (int k = 0; k < NE; ++k) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) radial[k] = fmaf(yn[k][u], Sn[k][u], radial[k]);
-            if (want_kappa && have[k])
+            if ((want_kappa & BWD_KAPPA) && have[k])
                 reinterpret_cast<float4 *>(kappa + (e[k] - e_lo) * (int64_t)NPHIP)[n4] =
                     make_float4(Rn[k][0] * Sn[k][0], Rn[k][1] * Sn[k][1], Rn[k][2] * Sn[k][2], Rn[k][3] * Sn[k][3]);
             cvc[k] = cvn[k];
@@ -590,7 +590,8 @@ __device__ __forceinline__ void edge_bwd_pass(int64_t e0, int64_t end, const uin
         const float rr = __fdividef(radial[k], g[k].w);
         gx = fmaf(rr, g[k].x, gx); gy = fmaf(rr, g[k].y, gy); gz = fmaf(rr, g[k].z, gz);
         if (have[k]) {
-            gst[e[k]] = make_float4(gx, gy, gz, 0.f);
+            if (want_kappa & BWD_G_ADD) red_add_f32x4(gst + e[k], gx, gy, gz, 0.f);
+            else gst[e[k]] = make_float4(gx, gy, gz, 0.f);
             if constexpr (VIR) {
                 aV[0] -= g[k].x * gx; aV[1] -= g[k].x * gy; aV[2] -= g[k].x * gz;
                 aV[3] -= g[k].y * gx; aV[4] -= g[k].y * gy; aV[5] -= g[k].y * gz;
@@ -941,11 +942,11 @@ int edge_bwd_blocks(int64_t N, int Na) {
 int launch_edge_bwd(const LaunchCtx &ctx, const ModelDims &md, int t, int64_t N, const int64_t *rc_ptr,
                     const uint32_t *col_rc, const float4 *geom, const float *c_ext, const float *rcen,
                     const float *alpha, const float *bbar, float *kappa, float4 *gst, double *vir_part,
-                    int64_t a0, int64_t a1, int64_t e_lo) {
+                    int64_t a0, int64_t a1, int64_t e_lo, bool g_add) {
     if (N <= 0 || a1 <= a0) return REANN_OK;
     const AtomChunk ch{a0, a1, e_lo};
     RadialTab rt{rcen + (size_t)t * md.S * md.nphip, alpha + (size_t)t * md.S * md.nphip, (float)(1.0 / md.rc)};
-    const int want_kappa = t >= 1;
+    const int want_kappa = (t >= 1 ? BWD_KAPPA : 0) | (g_add ? BWD_G_ADD : 0);
 #define M(NP, NA_, PN_, PA_) {                                                                                    \
     /* two edges per lane: persistent warps, one wave of resident blocks; else one atom per warp (measured faster) */ \
     const unsigned nblk_all = div_up(a1 - a0, BwdShape<NA_>::WPB);                                                \

@@ -77,6 +77,14 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N_>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 
+// g_e stash accumulated over the layers: one 16-byte reduction per edge, resolved in L2, nothing returned (no register is
+// held for the old value and no latency is exposed). Every address receives exactly one add per launch and launches
+// are ordered on the stream, so the sum is deterministic.
+__device__ __forceinline__ void red_add_f32x4(float4 *dst, float x, float y, float z, float w) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+constexpr int BWD_KAPPA = 1, BWD_G_ADD = 2;   // flag word of k_edge_bwd: write the kappa stash / add g_e to the stash instead of storing it
+
 struct StashChunk { // reverse gather: kappa holds the edges [e_lo, e_hi); forces once; cbar = or +=
     int64_t e_lo, e_hi;
     int do_forces, accumulate;
