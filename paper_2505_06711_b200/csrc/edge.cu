@@ -603,14 +603,22 @@ __device__ __forceinline__ void edge_bwd_pass(int64_t e0, int64_t end, const uin
 
 // Persistent warps: a warp walks over atoms (stride = warps of the grid); bbar_i and the records of the row's first
 // 64 edges of the NEXT atom arrive by cp.async while the current atom is processed (double-buffered in shared
-// memory, no registers held), so an atom starts without waiting on DRAM.
+// memory, no registers held), so an atom starts without waiting on DRAM. One-warp blocks (N_a > 10) stage the records of
+// the row's first 96 edges with bbar_i, so the later passes of a row do not wait for theirs either.
 // two edges per lane where the registers allow three blocks per SM with it (N_a <= 10); at N_a = 20 the pair of edges
 // costs a quarter of the resident warps and measured slower (1.09 vs 1.03 ms on config 3)
+#ifndef REANN_BWD_MINB
+#define REANN_BWD_MINB 16
+#endif
+#ifndef REANN_BWD_NREC
+#define REANN_BWD_NREC 96
+#endif
 template <int NA>
 struct BwdShape {
     static constexpr int NE = (NA % 2 == 0 && NA <= 10) ? 2 : 1;
     static constexpr int WPB = NE == 2 ? EW : 1;        // warps per block: one where a warp takes one atom and leaves (no waiting for block mates)
-    static constexpr int MINB = NE == 2 ? 3 : 16;
+    static constexpr int MINB = NE == 2 ? 3 : REANN_BWD_MINB;
+    static constexpr int NREC = NE == 2 ? 64 : REANN_BWD_NREC;   // staged edge records per row
 };
 
 template <int NPHIP, int NA, bool VIR>
@@ -624,8 +632,9 @@ __global__ void __launch_bounds__(BwdShape<NA>::WPB * 32, BwdShape<NA>::MINB) k_
     SKIP_GUARD(skip);
     constexpr int NB = NPHIP * NA, WPB = BwdShape<NA>::WPB;
     __shared__ __align__(16) float bb_s[WPB][2][NB];
-    __shared__ __align__(16) float4 g_s[WPB][2][64];
-    __shared__ uint32_t cj_s[WPB][2][64];
+    constexpr int NREC = BwdShape<NA>::NREC;            // records of the row's first NREC edges are staged with bbar_i
+    __shared__ __align__(16) float4 g_s[WPB][2][NREC];
+    __shared__ uint32_t cj_s[WPB][2][NREC];
     __shared__ __align__(16) float tab_s[2][REANN_MAX_S * NPHIP];
     __shared__ float vir_s[VIR ? WPB : 1][9];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -641,7 +650,7 @@ __global__ void __launch_bounds__(BwdShape<NA>::WPB * 32, BwdShape<NA>::MINB) k_
         const float4 *src = reinterpret_cast<const float4 *>(bbar + a * (int64_t)NB);
         for (int k = lane; k < NB / 4; k += 32) cp_async16(reinterpret_cast<float4 *>(bb_s[warp][buf]) + k, src + k);
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
+        for (int k = 0; k < NREC / 32; ++k) {
             const int64_t e = b0 + lane + 32 * k;
             if (e < b1) { cp_async16(&g_s[warp][buf][lane + 32 * k], geom + e); cp_async4(&cj_s[warp][buf][lane + 32 * k], col_rc + e); }
         }
@@ -664,19 +673,26 @@ __global__ void __launch_bounds__(BwdShape<NA>::WPB * 32, BwdShape<NA>::MINB) k_
         __syncwarp();
         int64_t p0 = beg;                                    // first edge of the pass (warp-uniform)
         while (p0 < end) {
-            const bool first = p0 == beg;
-            const float4 *gp = first ? &g_s[warp][buf][lane] : nullptr;
-            const uint32_t *cp = first ? &cj_s[warp][buf][lane] : nullptr;
-            if constexpr (BwdShape<NA>::NE == 2) {
+            if constexpr (BwdShape<NA>::NE == 2) {       // two-edge shape: the first pass of a row reads the staged records
+                const bool first = p0 == beg;
+                const float4 *gp = first ? &g_s[warp][buf][lane] : nullptr;
+                const uint32_t *cp = first ? &cj_s[warp][buf][lane] : nullptr;
                 if (end - p0 > 32) {
                     edge_bwd_pass<NPHIP, NA, VIR, 2>(p0 + lane, end, col_rc, geom, c_ext, tab_s[0], tab_s[1], rt.inv_rc,
                                                      bb_s[warp][buf], want_kappa, kappa, gst, ch.e_lo, aV, gp, cp);
                     p0 += 64;
                     continue;
                 }
+                edge_bwd_pass<NPHIP, NA, VIR, 1>(p0 + lane, end, col_rc, geom, c_ext, tab_s[0], tab_s[1], rt.inv_rc,
+                                                 bb_s[warp][buf], want_kappa, kappa, gst, ch.e_lo, aV, gp, cp);
+            } else {                                     // every pass whose edges are all among the staged records reads them there
+                const int off = (int)(p0 - beg);
+                const bool st = off + 32 <= NREC;
+                const float4 *gp = st ? &g_s[warp][buf][off + lane] : nullptr;
+                const uint32_t *cp = st ? &cj_s[warp][buf][off + lane] : nullptr;
+                edge_bwd_pass<NPHIP, NA, VIR, 1>(p0 + lane, end, col_rc, geom, c_ext, tab_s[0], tab_s[1], rt.inv_rc,
+                                                 bb_s[warp][buf], want_kappa, kappa, gst, ch.e_lo, aV, gp, cp);
             }
-            edge_bwd_pass<NPHIP, NA, VIR, 1>(p0 + lane, end, col_rc, geom, c_ext, tab_s[0], tab_s[1], rt.inv_rc,
-                                             bb_s[warp][buf], want_kappa, kappa, gst, ch.e_lo, aV, gp, cp);
             p0 += 32;
         }
         __syncwarp();                                        // every lane is done with bb_s[buf] before it is refilled
@@ -699,7 +715,7 @@ __global__ void __launch_bounds__(BwdShape<NA>::WPB * 32, BwdShape<NA>::MINB) k_
             double s = 0.0;
 #pragma unroll
             for (int w = 0; w < WPB; ++w) s += (double)vir_s[w][threadIdx.x];
-            vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x] += s;
+            atomicAdd(&vir_part[(int64_t)blockIdx.x * 9 + threadIdx.x], s);   // result unused = RED: one add per address and launch, no wait for the old value
         }
     }
 }
@@ -724,9 +740,22 @@ __global__ void __launch_bounds__(RW * 32) k_rev_gather(int64_t N, const int64_t
     const int64_t beg = rc_ptr[k], end = rc_ptr[k + 1];
     if (ch.do_forces) {
         double f0 = 0.0, f1 = 0.0, f2 = 0.0;
-        for (int64_t e = beg + lane; e < end; e += 32) {
-            const float4 g = gst[rev_rc[e]], o = gst[e];
-            f0 += (double)(o.x - g.x); f1 += (double)(o.y - g.y); f2 += (double)(o.z - g.z);
+        // four edges per lane and iteration: the index loads, then the eight stash loads, are in flight together
+        constexpr int U = 4;
+        for (int64_t eb = beg + lane; eb < end; eb += 32 * U) {
+            uint32_t r[U];
+            float4 g[U], o[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) r[u] = eb + 32 * u < end ? rev_rc[eb + 32 * u] : 0u;
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                g[u] = o[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (eb + 32 * u < end) { g[u] = gst[r[u]]; o[u] = gst[eb + 32 * u]; }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {       // same order of additions as one edge per iteration
+                f0 += (double)(o[u].x - g[u].x); f1 += (double)(o[u].y - g[u].y); f2 += (double)(o[u].z - g[u].z);
+            }
         }
 #pragma unroll
         for (int d = 16; d >= 1; d >>= 1) {
