@@ -110,7 +110,10 @@ __global__ void k_rc_ext(const XRec *__restrict__ xrec, const int64_t *__restric
 // rc-filter, pass 2: compact rows (neighbour ext index | species<<28, edge vector + length in FP32
 // rounded once from the FP64 difference, index of the reverse compact edge). Two levels of dependent loads per
 // iteration: (rank, col, rev) of the entry, then (record, rank of the reverse entry, row offset of the owner).
-__global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict__ xrec,
+// Bound by the latency of its gathers: 64 registers (16 two-warp blocks per SM) with two entries per lane in flight
+// measured best on config 3 (prep 0.55 -> 0.50 ms per step against four entries at 94 registers = 10 blocks per SM;
+// one entry or 20+ blocks spill and are slower).
+__global__ void __launch_bounds__(RW * 32, 16) k_filter_fill(const XRec *__restrict__ xrec,
                                                          const int64_t *__restrict__ row_ptr,
                                                          const int32_t *__restrict__ col,
                                                          const uint32_t *__restrict__ rev, int64_t N, BoxP B,
@@ -125,8 +128,8 @@ __global__ void __launch_bounds__(RW * 32) k_filter_fill(const XRec *__restrict_
     if (i >= N) return;
     const XRec me = xrec[i];
     const int64_t r0 = row_ptr[i], r1 = row_ptr[i + 1], c0 = rc_ptr[i];
-    // four list entries per lane and iteration: their gathers are all in flight together
-    constexpr int U = 4;
+    // two list entries per lane and iteration: their gathers are all in flight together
+    constexpr int U = 2;
     for (int64_t eb = r0 + lane; eb < r1; eb += 32 * U) {
         uint16_t rk[U];
         int32_t j[U];
